@@ -1,0 +1,299 @@
+"""Pins of the oracle's matrix elements against closed forms, invariances and brute force.
+
+P-numbers refer to SURVEY.md 8(c) / DESIGN.md "Pins".  Nothing here compares the oracle with itself
+through the same code path: closed forms are retyped from the textbook formulas, invariances relate
+DIFFERENT inputs, and the colour brute force uses explicit Gell-Mann matrices without the trace basis.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2503_21935_b200 import inputs as I
+from helpers import read_golden
+
+GOLD = read_golden("worked_points.txt")
+GG = ["gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg"]
+NGL = {"gg_tt": 2, "gg_ttg": 3, "gg_ttgg": 4, "gg_ttggg": 5}
+
+
+def mdot(a, b):
+    return a[..., 0] * b[..., 0] - (a[..., 1:] * b[..., 1:]).sum(-1)
+
+
+def two_body(cos, m, e=750.0):
+    s = math.sqrt(1 - cos * cos)
+    pp = math.sqrt(e * e - m * m)
+    return np.array([[e, 0, 0, e], [e, 0, 0, -e], [e, pp * s, 0, pp * cos], [e, -pp * s, 0, -pp * cos]])
+
+
+# ---------------------------------------------------------------- e+ e- -> mu+ mu-
+def ew():
+    alpha = 1 / 132.507
+    mz, gf = 91.188, 1.16639e-5
+    mw2 = mz**2 / 2 + math.sqrt(mz**4 / 4 - math.pi * alpha * mz**2 / (math.sqrt(2) * gf))
+    sw2 = 1 - mw2 / mz**2
+    e = math.sqrt(4 * math.pi * alpha)
+    sc = math.sqrt(sw2 * (1 - sw2))
+    return e, e / sc * (-0.5 + sw2), e / sc * sw2, math.sqrt(mw2), sw2
+
+
+def eemumu_closed(mom, qed_only=False):
+    e, gl, gr, _, _ = ew()
+    s = mdot(mom[:, 0] + mom[:, 1], mom[:, 0] + mom[:, 1])
+    t = mdot(mom[:, 1] - mom[:, 3], mom[:, 1] - mom[:, 3])   # (p_e- - p_mu-)^2
+    u = mdot(mom[:, 1] - mom[:, 2], mom[:, 1] - mom[:, 2])   # (p_e- - p_mu+)^2
+    bw = 0 if qed_only else 1 / (s - 91.188**2 + 1j * 91.188 * 2.441)
+    A = lambda x, y: e * e / s + x * y * bw
+    return u**2 * (abs(A(gl, gl)) ** 2 + abs(A(gr, gr)) ** 2) + t**2 * (abs(A(gl, gr)) ** 2 + abs(A(gr, gl)) ** 2)
+
+
+def test_P0_electroweak_inputs():
+    e, gl, gr, mw, sw2 = ew()
+    assert abs(mw - GOLD["mw"]) < 1e-5 and abs(sw2 - GOLD["sw2"]) < 1e-9
+    assert abs(e - GOLD["ee"]) < 1e-9 and abs(gl - GOLD["gl"]) < 1e-9 and abs(gr - GOLD["gr"]) < 1e-9
+
+
+def test_P1_eemumu_worked_value():
+    mom = two_body(0.5, 0.0)[None]
+    assert O.me("ee_mumu", mom, 1.0)[0] == pytest.approx(GOLD["ee_mumu_me"], rel=1e-13)
+    assert eemumu_closed(mom)[0] == pytest.approx(GOLD["ee_mumu_me"], rel=1e-13)
+    assert eemumu_closed(mom, qed_only=True)[0] == pytest.approx(GOLD["ee_mumu_me_qed_only"], rel=1e-13)
+
+
+def test_P1_eemumu_closed_form_per_event():
+    mom = I.make_momenta("ee_mumu", 2048, seed=1)
+    got = O.me("ee_mumu", mom, 1.0)
+    assert np.abs(got / eemumu_closed(mom) - 1).max() < 1e-12
+    # Lorentz-transformed frames (general directions, P6)
+    mom2 = I.lorentz_transform(mom[:256], seed=3)
+    assert np.abs(O.me("ee_mumu", mom2, 1.0) / got[:256] - 1).max() < 1e-11
+
+
+def test_P2_eemumu_cross_section():
+    # sigma = 1/(2s) * (1/8pi) * 1/2 int dcos ME(cos): Gauss-Legendre is exact for the quadratic in cos
+    x, w = np.polynomial.legendre.leggauss(8)
+    mom = np.stack([two_body(c, 0.0) for c in x])
+    me = O.me("ee_mumu", mom, 1.0)
+    s = 1500.0**2
+    sigma = (w * me).sum() / 2 / (2 * s) / (8 * math.pi) * GOLD["gev2_to_pb"]
+    assert sigma == pytest.approx(GOLD["ee_mumu_sigma_pb"], rel=2e-7)
+
+
+def test_P10_eemumu_four_helicities():
+    mom = I.make_momenta("ee_mumu", 64, seed=1)
+    mh = O.me_helicities("ee_mumu", mom, 1.0)
+    nz = (mh > 1e-20 * mh.max()).sum(axis=1)
+    assert (nz == 4).all()
+    ht = O.helicity_table("ee_mumu")
+    good = O.good_helicities("ee_mumu", mom, 1.0)
+    # chirality: opposite helicities on each massless fermion line
+    for h in range(16):
+        assert bool(good[h]) == (ht[h, 0] == -ht[h, 1] and ht[h, 2] == -ht[h, 3])
+
+
+# ---------------------------------------------------------------- g g -> t tbar closed form
+def ggtt_closed(mom, gs, mt=173.0):
+    s = mdot(mom[:, 0] + mom[:, 1], mom[:, 0] + mom[:, 1])
+    t1 = 2 * mdot(mom[:, 0], mom[:, 2]) / s
+    t2 = 2 * mdot(mom[:, 1], mom[:, 2]) / s
+    rho = 4 * mt * mt / s
+    return gs**4 * (1 / (6 * t1 * t2) - 3 / 8) * (t1**2 + t2**2 + rho - rho**2 / (4 * t1 * t2))
+
+
+def test_P3_ggtt_worked_values():
+    mom = two_body(0.5, 173.0)[None]
+    gs = GOLD["gg_tt_gs"]
+    assert gs == pytest.approx(math.sqrt(4 * math.pi * 0.118), rel=1e-14)
+    assert O.me("gg_tt", mom, gs, params=dict(wt=0.0))[0] == pytest.approx(GOLD["gg_tt_me_w0"], rel=1e-13)
+    assert ggtt_closed(mom, gs)[0] == pytest.approx(GOLD["gg_tt_me_w0"], rel=1e-13)
+    assert O.me("gg_tt", mom, gs)[0] == pytest.approx(GOLD["gg_tt_me_w"], rel=1e-12)
+
+
+def test_P3_ggtt_closed_form_per_event():
+    mom = I.make_momenta("gg_tt", 2048, seed=1)
+    gs = I.make_gs(2048, seed=1)
+    got = O.me("gg_tt", mom, gs, params=dict(wt=0.0))
+    rel = np.abs(got / ggtt_closed(mom, gs) - 1)
+    # forward/backward points (tau_i -> rho/4) lose digits to cancellation in BOTH expressions
+    assert rel.max() < 1e-10 and np.median(rel) < 1e-14
+    # other top masses, including the massless limit of the formula
+    for mt in (0.0, 50.0, 400.0):
+        m2 = I.make_momenta("gg_tt", 64, seed=2, mt=mt)
+        got = O.me("gg_tt", m2, 1.1, params=dict(wt=0.0, mt=mt))
+        assert np.abs(got / ggtt_closed(m2, 1.1, mt) - 1).max() < 1e-11
+
+
+def test_P4_ggtt_cross_section():
+    x, w = np.polynomial.legendre.leggauss(400)
+    mom = np.stack([two_body(c, 173.0) for c in x])
+    gs = GOLD["gg_tt_gs"]
+    me = O.me("gg_tt", mom, gs, params=dict(wt=0.0))
+    s = 1500.0**2
+    beta = math.sqrt(1 - 4 * 173.0**2 / s)
+    sigma = (w * me).sum() / 2 * beta / (16 * math.pi * s) * GOLD["gev2_to_pb"]
+    rho = 4 * 173.0**2 / s
+    closed = (math.pi * 0.118**2 / (3 * s)) * ((1 + rho + rho**2 / 16) * math.log((1 + beta) / (1 - beta))
+                                                - beta * (7 / 4 + 31 * rho / 16)) * GOLD["gev2_to_pb"]
+    assert closed == pytest.approx(GOLD["gg_tt_sigma_pb"], rel=2e-7)
+    assert sigma == pytest.approx(closed, rel=1e-11)
+
+
+def test_P10_ggtt_helicities():
+    mom = I.make_momenta("gg_tt", 256, seed=1)
+    ht = O.helicity_table("gg_tt")
+    good0 = O.good_helicities("gg_tt", mom, 1.2, params=dict(wt=0.0))
+    # Gamma_t = 0, CM frame: like-helicity gluons with opposite-helicity t tbar vanish -> 12 good
+    assert good0.sum() == 12
+    for h in range(16):
+        vanishing = ht[h, 0] == ht[h, 1] and ht[h, 2] == -ht[h, 3]
+        assert bool(good0[h]) == (not vanishing)
+    # with the width (reading R4) all 16 pass the 1e-12 criterion (the 4 extra sit near 1.5e-8)
+    good = O.good_helicities("gg_tt", mom, 1.2)
+    assert good.sum() == 16
+    mh = O.me_helicities("gg_tt", mom, 1.2)
+    frac = (mh / mh.sum(1, keepdims=True))[:, good0 == 0]
+    assert 1e-10 < frac.max() < 1e-6
+
+
+# ---------------------------------------------------------------- all gg processes
+@pytest.mark.parametrize("proc", GG)
+def test_P5_ward_identity(proc):
+    """eps -> k for any one gluon makes EVERY colour-flow amplitude vanish (Gamma_t = 0)."""
+    i = O.info(proc)
+    nev = 3 if proc != "gg_ttggg" else 1
+    mom = I.make_momenta(proc, nev, seed=11)
+    hels = [0, 5, i["ncomb"] - 1, i["ncomb"] // 3] if proc != "gg_ttggg" else [0, 77]
+    for e in range(nev):
+        for h in hels:
+            j0 = O.jamps(proc, mom[e], 1.2, h, params=dict(wt=0.0))
+            for leg in [0, 1] + list(range(4, i["npar"])):
+                jw = O.jamps(proc, mom[e], 1.2, h, ward_leg=leg, params=dict(wt=0.0))
+                # natural size of the replaced amplitude: |k| ~ E_leg times the physical amplitude
+                assert np.abs(jw).max() < 1e-10 * mom[e, leg, 0] * np.abs(j0).max()
+    # and the identity is really a statement about the width: it fails visibly for Gamma_t != 0
+    jw = O.jamps(proc, mom[0], 1.2, hels[0], ward_leg=0)
+    j0 = O.jamps(proc, mom[0], 1.2, hels[0])
+    assert np.abs(jw).max() > 1e-9 * mom[0, 0, 0] * np.abs(j0).max()
+
+
+@pytest.mark.parametrize("proc", GG)
+def test_P6_lorentz_invariance(proc):
+    nev = {"gg_tt": 64, "gg_ttg": 32, "gg_ttgg": 8, "gg_ttggg": 2}[proc]
+    mom = I.make_momenta(proc, nev, seed=5)
+    gs = I.make_gs(nev, seed=5)
+    a = O.me(proc, mom, gs, params=dict(wt=0.0))
+    b = O.me(proc, I.lorentz_transform(mom, seed=9), gs, params=dict(wt=0.0))
+    assert np.abs(b / a - 1).max() < 1e-9
+
+
+@pytest.mark.parametrize("proc", GG)
+def test_P9_coupling_scaling(proc):
+    nev = 2
+    mom = I.make_momenta(proc, nev, seed=6)
+    a = O.me(proc, mom, math.sqrt(4 * math.pi * 0.10))
+    b = O.me(proc, mom, math.sqrt(4 * math.pi * 0.13))
+    assert np.abs(b / a / (1.3 ** NGL[proc]) - 1).max() < 1e-12
+
+
+@pytest.mark.parametrize("proc", ["gg_ttg", "gg_ttgg", "gg_ttggg"])
+def test_P12_bose_and_charge_symmetry(proc):
+    nev = 2 if proc != "gg_ttggg" else 1
+    mom = I.make_momenta(proc, nev, seed=8)
+    a = O.me(proc, mom, 1.2)
+    if mom.shape[1] > 5:
+        m2 = mom.copy()
+        m2[:, [4, 5]] = m2[:, [5, 4]]          # exchange two final-state gluons
+        assert np.abs(O.me(proc, m2, 1.2) / a - 1).max() < 1e-11
+    m3 = mom.copy()
+    m3[:, [0, 1]] = m3[:, [1, 0]]              # exchange the incoming gluons
+    assert np.abs(O.me(proc, m3, 1.2) / a - 1).max() < 1e-11
+    m4 = mom.copy()
+    m4[:, [2, 3]] = m4[:, [3, 2]]              # t <-> tbar (charge conjugation)
+    assert np.abs(O.me(proc, m4, 1.2) / a - 1).max() < 1e-11
+
+
+@pytest.mark.parametrize("proc", ["gg_tt", "gg_ttg", "gg_ttgg"])
+def test_P13_parity(proc):
+    mom = I.make_momenta(proc, 2, seed=4)
+    i = O.info(proc)
+    mh = O.me_helicities(proc, mom, 1.2)
+    mp = mom.copy()
+    mp[:, :, 1:] *= -1
+    mhp = O.me_helicities(proc, mp, 1.2)
+    flip = (i["ncomb"] - 1) - np.arange(i["ncomb"])      # all helicities reversed
+    assert np.abs(mhp[:, flip] / mh - 1).max() < 1e-9
+
+
+@pytest.mark.parametrize("proc", ["gg_tt", "gg_ttg", "gg_ttgg"])
+def test_P14_explicit_colour_brute_force(proc):
+    """sum over 8^n*9 explicit colour assignments (Gell-Mann T, f from commutators) == J^dagger C J."""
+    i = O.info(proc)
+    mom = I.make_momenta(proc, 1, seed=13)[0]
+    C = O.color_matrix(proc)
+    hels = [3, i["ncomb"] - 2] if proc != "gg_ttgg" else [22]
+    for h in hels:
+        j = O.jamps(proc, mom, 1.2, h)
+        dec = (j.conj() @ C @ j).real
+        assert O.brute_color(proc, mom, 1.2, h) == pytest.approx(dec, rel=1e-11)
+
+
+@pytest.mark.parametrize("proc", ["gg_ttg", "gg_ttgg"])
+def test_P10_filtered_sum_equals_full_sum(proc):
+    mom = I.make_momenta(proc, 64, seed=1)
+    gs = I.make_gs(64, seed=1)
+    good = O.good_helicities(proc, mom, gs)
+    full = O.me(proc, mom, gs)
+    filt = O.me(proc, mom, gs, mask=good)
+    assert np.abs(filt / full - 1).max() < 1e-12
+
+
+@pytest.mark.parametrize("proc", GG[:3])
+def test_P11_massless_mhv(proc):
+    """m_t = 0: |J_sigma|^2 for MHV helicities equals the Parke-Taylor form; all-plus/all-minus vanish."""
+    i = O.info(proc)
+    n = NGL[proc]
+    npar = i["npar"]
+    mom = I.make_momenta(proc, 3, seed=21, mt=0.0)
+    ht = O.helicity_table(proc)
+    flows = O.color_table(proc)
+    par = dict(mt=0.0, wt=0.0)
+    gs = 1.3
+    sij = lambda a, b: abs(2 * mdot(a, b))
+    ratios = []
+    for e in range(3):
+        p = mom[e]
+        for h in range(i["ncomb"]):
+            lam = ht[h]
+            # all-outgoing helicities: flip the incoming gluons
+            out = lam.copy()
+            out[0] *= -1
+            out[1] *= -1
+            gl = [0, 1] + list(range(4, npar))
+            j = O.jamps(proc, p, gs, h, params=par)
+            scale = gs**n / 1500.0 ** (n - 2)
+            if lam[2] == lam[3]:
+                assert np.abs(j).max() < 1e-9 * scale      # helicity conservation on the massless line
+                continue
+            gh = [out[g] for g in gl]
+            if all(x == gh[0] for x in gh):
+                assert np.abs(j).max() < 1e-9 * scale      # all-plus / all-minus
+                continue
+            # exactly one gluon opposite to the others, and it must be "negative" when quark is -, antiquark +
+            qm = lam[2] == -1      # quark helicity -, antiquark +
+            want = -1 if qm else 1
+            special = [g for g in gl if out[g] == want]
+            if len(special) != 1:
+                continue
+            gI = special[0]
+            for c in range(i["ncol"]):
+                order = [2] + list(flows[c]) + [3]
+                den = sij(p[3], p[2])
+                for a, b in zip(order[:-1], order[1:]):
+                    den *= sij(p[a], p[b])
+                pt = gs ** (2 * n) * sij(p[2], p[gI]) ** 3 * sij(p[3], p[gI]) / den
+                ratios.append(abs(j[c]) ** 2 / pt)
+    ratios = np.array(ratios)
+    assert len(ratios) > 10
+    assert np.abs(ratios / 2.0**n - 1).max() < 1e-8
