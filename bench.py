@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""bench.py -- MEs/s of the gg -> t tbar g g hot path on B200 (BASELINE.json metric), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--nevt E] [--precision fp64|fp32|mixed]
+                    [--process gg_ttgg] [--sweep] [--no-extras] [--impl reference]
+
+A "step" is one pass of the whole hot path (me_compute: load, wavefunctions, diagrams, jamps, colour
+sum, helicity loop, helicity/colour selection, store) over one batch of seeded RAMBO events.
+`value` times the C-ABI call with inputs resident in HBM (CUDA events on the launch stream);
+`e2e` times me_compute_host with pinned HOST buffers (H2D + kernel + D2H inside the timed region).
+Multi-GPU (torchrun): events are independent, ranks run replicas on disjoint seeded batches, no
+collective on the data path ("scaling": "weak").  --impl reference times the CPU oracle.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2503_21935_b200 import inputs as I  # noqa: E402
+
+METRIC = "matrix elements/sec (MEs/s) for gg->ttbar gg on 1 B200"
+UNIT = "MEs/s"
+ALPHAS = {"ee_mumu": 0.118, "gg_tt": 0.118, "gg_ttg": 0.118, "gg_ttgg": None, "gg_ttggg": 0.118}
+DTYPE = {"fp64": "f64", "fp32": "f32", "mixed": "f64+f32"}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--nevt", type=int, default=1 << 20, help="events per step (per GPU)")
+    ap.add_argument("--process", default="gg_ttgg")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"])
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--sweep", action="store_true", help="add the events-per-launch sweep 2^14..2^22")
+    ap.add_argument("--no-extras", action="store_true", help="skip fp32/mixed lines, cpu_baseline and e2e")
+    return ap.parse_args()
+
+
+def flops_per_me(process, ngood):
+    """Algorithmic FLOPs per ME of the generated code (FMA = 2), counted by the generator (gen/flops.json)."""
+    path = os.path.join(ROOT, "paper_2503_21935_b200", "csrc", "gen", "flops.json")
+    with open(path) as f:
+        d = json.load(f)[process]
+    return d["per_event"] + ngood * d["per_helicity"], d
+
+
+def make_inputs(process, nevt, seed, start=0):
+    mom = I.make_momenta(process, nevt, seed=seed, start=start)
+    gs = I.make_gs(nevt, seed=seed, alphas=ALPHAS[process], start=start)
+    rh, rc = I.make_rnd(nevt, seed=seed, start=start)
+    return mom, gs, rh, rc
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            self.t.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons, pw = [], [], set(), []
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def time_device(torch, m, bufs, steps, warmup, select=True):
+    """ms per step of me_compute with device-resident inputs: CUDA events on the launch stream."""
+    mom, gs, rh, rc, out, sh, sc = bufs
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        m.compute(mom, gs, rh if select else None, rc if select else None, out=out, selhel=sh if select else None,
+                  selcol=sc if select else None, stream=stream)
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    ev[0].record(stream)
+    for k in range(steps):
+        m.compute(mom, gs, rh if select else None, rc if select else None, out=out, selhel=sh if select else None,
+                  selcol=sc if select else None, stream=stream)
+        ev[k + 1].record(stream)
+    torch.cuda.synchronize()
+    per = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
+    return ev[0].elapsed_time(ev[steps]), per
+
+
+def cpu_baseline(process, seconds_target=15.0):
+    """The oracle as it stands, on this box's host cores, on a bounded sample of the same workload."""
+    from oracle import oracle as O
+    n0 = {"ee_mumu": 16384, "gg_tt": 16384, "gg_ttg": 4096, "gg_ttgg": 256, "gg_ttggg": 16}[process]
+    mom, gs, _, _ = make_inputs(process, n0, seed=1)
+    O.me(process, mom[:8], gs[:8])
+    t = time.perf_counter(); O.me(process, mom, gs); dt = time.perf_counter() - t
+    n = int(max(n0, min(1 << 20, n0 * seconds_target / max(dt, 1e-3))))
+    mom, gs, _, _ = make_inputs(process, n, seed=1)
+    mask = O.good_helicities(process, mom[:n0], gs[:n0])
+    t = time.perf_counter(); O.me(process, mom, gs, mask=mask); dt = time.perf_counter() - t
+    return {"value": n / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+            "sample": f"first {n} events of the seeded {process} batch (seed 1), good helicities only, {dt:.1f} s"}
+
+
+def run_reference(a):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    process = a.process
+    n0 = {"ee_mumu": 16384, "gg_tt": 16384, "gg_ttg": 4096, "gg_ttgg": 512, "gg_ttggg": 16}[process]
+    mom, gs, _, _ = make_inputs(process, n0, seed=1)
+    mask = O.good_helicities(process, mom[: min(n0, 256)], gs[: min(n0, 256)])
+    for _ in range(a.warmup):
+        O.me(process, mom[: max(8, n0 // 8)], gs[: max(8, n0 // 8)], mask=mask)
+    t = time.perf_counter()
+    for _ in range(a.steps):
+        O.me(process, mom, gs, mask=mask)
+    dt = time.perf_counter() - t
+    val = a.steps * n0 / dt
+    sample = f"each step = first {n0} events of the seeded {process} batch (bounded sample of the {a.nevt}-event workload)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
+        "warmup": a.warmup, "ms_per_step": 1e3 * dt / a.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": process, "events_per_step": n0, "precision": "fp64"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    a = parse()
+    if a.impl == "reference":
+        return run_reference(a)
+    import torch
+    import torch.distributed as dist
+
+    from paper_2503_21935_b200.me import MatrixElement, fma_peak
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    process, nevt = a.process, a.nevt
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # seeded inputs: rank r takes events [r*nevt, (r+1)*nevt) of the stream (disjoint shards, no exchange)
+    mom_h, gs_h, rh_h, rc_h = make_inputs(process, nevt, seed=1, start=rank * nevt)
+    t = lambda x: torch.from_numpy(x).to(dev)
+    bufs = (t(mom_h), t(gs_h), t(rh_h), t(rc_h), torch.empty(nevt, dtype=torch.float64, device=dev),
+            torch.empty(nevt, dtype=torch.int32, device=dev), torch.empty(nevt, dtype=torch.int32, device=dev))
+
+    def bench_precision(prec, steps, warmup, n=nevt):
+        m = MatrixElement(process, prec, device=local)
+        b = bufs if n == nevt else tuple(x[:n].contiguous() for x in bufs)
+        mask = m.filter_helicities(b[0], b[1])
+        barrier()
+        with ClockSampler(local) as cs:
+            total_ms, per = time_device(torch, m, b, steps, warmup)
+        barrier()
+        info = m.launch_info()
+        return m, mask, total_ms, per, cs.summary(), info
+
+    m, mask, total_ms, per, clocks, info = bench_precision(a.precision, a.steps, a.warmup)
+    tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    total_ms = float(tmax.item())
+    ms_per_step = total_ms / a.steps
+    value = world * nevt / (ms_per_step * 1e-3)
+    ngood = int(mask.sum())
+    fl, fl_detail = flops_per_me(process, ngood)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": DTYPE[a.precision], "data": "synthetic",
+        "config": {"workload": process, "events_per_step_per_gpu": nevt, "precision": a.precision,
+                   "inputs": "seeded RAMBO sqrt(s)=1500 GeV, alpha_s~U[0.10,0.13], helicity+colour selection on",
+                   "l2": "momenta+randoms+outputs per step = %.0f MB %s the 126 MB L2" % (
+                       nevt * (m.npar * 32 + 40) / 1e6, ">" if nevt * (m.npar * 32 + 40) > 126e6 else "<"),
+                   "good_helicities": ngood, "launch": info, "parallelism": f"replicas x{world}"},
+        "clocks": clocks, "gpu_launches": a.steps,
+    }
+    if rank == 0:
+        prec_peak = "fp32" if a.precision == "fp32" else "fp64"
+        peak = fma_peak(prec_peak, local)
+        kernel_ms = float(np.mean(per))
+        achieved = fl * nevt / (kernel_ms * 1e-3) * 1e-12
+        line["roofline"] = {
+            "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+            "flops_per_me": fl, "flops_source": "generator count of the emitted straight-line code (FMA = 2): "
+            f"{fl_detail['per_helicity']} per helicity x {ngood} good helicities + {fl_detail['per_event']} per event",
+            "peak_source": f"me_fma_peak({prec_peak}): register-resident FMA chain measured on this GPU in this run",
+            "nominal_peak": 148 * (64 if prec_peak == "fp64" else 128) * 2 * 1.965e-3,
+            "kernel_ms": kernel_ms,
+        }
+    m.close()
+    if rank == 0 and not a.no_extras:
+        # e2e: host buffers (pinned) -> me_compute_host -> host results
+        pin = lambda x: torch.from_numpy(x).pin_memory()
+        hm, hg, hr, hc = pin(mom_h), pin(gs_h), pin(rh_h), pin(rc_h)
+        ho = torch.empty(nevt, dtype=torch.float64).pin_memory()
+        hsh = torch.empty(nevt, dtype=torch.int32).pin_memory()
+        hsc = torch.empty(nevt, dtype=torch.int32).pin_memory()
+        m = MatrixElement(process, a.precision, device=local)
+        m.set_good_helicities(mask)
+        for _ in range(max(1, a.warmup)):
+            m.compute_host(hm, hg, hr, hc, out=ho, selhel=hsh, selcol=hsc)
+        t0 = time.perf_counter()
+        for _ in range(a.steps):
+            m.compute_host(hm, hg, hr, hc, out=ho, selhel=hsh, selcol=hsc)
+        dt = time.perf_counter() - t0
+        m.close()
+        line["e2e"] = {"value": a.steps * nevt / dt, "unit": UNIT,
+                       "h2d_bytes_per_step": int(mom_h.nbytes + gs_h.nbytes + rh_h.nbytes + rc_h.nbytes),
+                       "d2h_bytes_per_step": int(nevt * 16), "api": "me_compute_host (pinned host buffers)"}
+        others = {}
+        for prec in ("fp64", "fp32", "mixed"):
+            if prec == a.precision:
+                continue
+            m2, mk2, tot2, per2, clk2, info2 = bench_precision(prec, max(2, a.steps // 2), a.warmup)
+            ms2 = tot2 / max(2, a.steps // 2)
+            pk = fma_peak("fp32" if prec == "fp32" else "fp64", local)
+            ach = fl * nevt / (ms2 * 1e-3) * 1e-12
+            others[prec] = {"value": nevt / (ms2 * 1e-3), "unit": UNIT, "ms_per_step": ms2, "launch": info2,
+                            "roofline_frac": ach / pk, "peak_tflops": pk, "clocks": clk2}
+            m2.close()
+        line["other_precisions"] = others
+        if a.sweep:
+            sw = {}
+            for prec in ("fp64", "fp32"):
+                for lg in range(14, 23):
+                    n = 1 << lg
+                    if n > nevt:
+                        break
+                    m3, _, tot3, _, _, _ = bench_precision(prec, 3, 3, n)
+                    sw[f"{prec}:{n}"] = n / (tot3 / 3 * 1e-3)
+                    m3.close()
+            line["sweep_mes_per_s"] = sw
+        line["cpu_baseline"] = cpu_baseline(process)
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

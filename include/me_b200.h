@@ -1,0 +1,112 @@
+/* me_b200.h -- C ABI of the B200 matrix-element library (libme_b200.so).
+ *
+ * The boundary follows the paper's statement of the problem: a "multi-event API" made of "reentrant
+ * stateless functions with well-defined input and output data" (Fig. 1 caption)
+ * that can be used "as a CUDACPP ME library ... in frameworks other than MG5aMC":
+ * momenta[nevt][npar][4] (fp64) plus the per-event strong coupling in, ME[nevt] out, plus optional
+ * per-event helicity and colour selection from supplied uniform random numbers (BASELINE.json
+ * north_star).  What is computed: "from the particle momenta, the matrix element (ME) ... is computed"
+ * as Feynman diagrams + the colour-matrix quadratic form, summed over
+ * helicity combinations:
+ *
+ *     ME = (1/denom) * sum_{h good} sum_{s,t} conj(J_s(h)) C_st J_t(h)
+ *
+ * Conventions (readings R1-R16)
+ *   - all `d_*` arguments are DEVICE pointers owned by the caller (8-byte aligned; int32 outputs 4-byte);
+ *     everything else is a HOST pointer.  `stream` is a cudaStream_t passed as void*; work is enqueued
+ *     on it and NOT synchronised unless stated.  The library allocates device memory only in
+ *     me_create / me_filter_helicities (scratch, freed by me_destroy).
+ *   - momenta: [nevt][npar][4] doubles, (E, px, py, pz) in GeV, particle order = process string order,
+ *     particles 0,1 incoming; for the gg processes 2 = t, 3 = tbar, 4.. = g; for ee_mumu
+ *     0 = e+, 1 = e-, 2 = mu+, 3 = mu-.  No special frame is assumed.
+ *   - gs: [nevt] doubles, g_s = sqrt(4 pi alpha_s) per event (ignored by ee_mumu, may be NULL there).
+ *   - helicity index h (0-based): row of the table returned by me_helicity_table; row h has
+ *     lambda_k = +1 if bit (npar-1-k) of h is set, else -1 (particle 0 slowest).
+ *   - colour index c (0-based): row of me_color_table, the permutations of the gluon particle indices
+ *     in lexicographic order (string from t to tbar).  ee_mumu: ncol = 1.
+ *   - every function returns 0 on success or a negative ME_ERR_* code; me_last_error gives a
+ *     NUL-terminated description of the last failure of that handle (or of me_create if h == NULL).
+ *     No C++ exception crosses the boundary.  A handle may be used from one host thread at a time;
+ *     different handles are independent.
+ */
+#ifndef ME_B200_H
+#define ME_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct me_handle me_handle;
+
+/* physics parameters; NULL in me_create selects the BASELINE.json values */
+typedef struct me_params {
+  double mt;    /* top mass [GeV]                      173.0     */
+  double wt;    /* top width [GeV], fixed-width scheme 1.4915    */
+  double mz;    /* Z mass [GeV]                        91.188    */
+  double wz;    /* Z width [GeV]                       2.441     */
+  double aewm1; /* 1/alpha_EM                          132.507   */
+  double gf;    /* Fermi constant [GeV^-2]             1.16639e-5 */
+} me_params;
+
+enum { ME_FP64 = 0, ME_FP32 = 1, ME_MIXED = 2 };
+
+enum {
+  ME_OK = 0,
+  ME_ERR_ARG = -1,        /* NULL / misaligned pointer, negative nevt, bad enum */
+  ME_ERR_PROCESS = -2,    /* unknown process name */
+  ME_ERR_NO_HELICITIES = -3, /* me_compute before me_filter_helicities / me_set_good_helicities */
+  ME_ERR_CUDA = -4,       /* CUDA runtime error (text in me_last_error) */
+  ME_ERR_NOMEM = -5
+};
+
+/* process: "ee_mumu" | "gg_tt" | "gg_ttg" | "gg_ttgg" | "gg_ttggg"; precision: ME_FP64/ME_FP32/ME_MIXED
+ * (mixed = Feynman diagrams in fp64, colour quadratic form in fp32); device: CUDA ordinal. */
+int me_create(me_handle** out, const char* process, int precision, const me_params* params, int device);
+int me_destroy(me_handle* h);
+const char* me_last_error(const me_handle* h);
+
+/* sizes: any output pointer may be NULL */
+int me_info(const me_handle* h, int* npar, int* ncomb, int* ncol, int* ndiag, int* denom);
+/* out[ncomb][npar], entries +-1 */
+int me_helicity_table(const me_handle* h, int8_t* out);
+/* out[ncol][ngluon]: gluon particle indices in string order (nothing written for ee_mumu) */
+int me_color_table(const me_handle* h, int8_t* out);
+/* out[ncol][ncol], the real symmetric colour matrix C */
+int me_color_matrix(const me_handle* h, double* out);
+
+/* One-time good-helicity filter (BASELINE.json north_star (e); reading R10): evaluates ALL helicities in
+ * fp64 on the first min(nevt, 16384) events and keeps h iff max_e |M_h|^2 / sum_h' |M_h'|^2 > 1e-12.
+ * Synchronises the stream (it is an initialisation call). */
+int me_filter_helicities(me_handle* h, const double* d_momenta, const double* d_gs, int64_t nevt, void* stream);
+/* mask[ncomb], 1 = good */
+int me_get_good_helicities(const me_handle* h, int* ngood, uint8_t* mask);
+int me_set_good_helicities(me_handle* h, const uint8_t* mask);
+
+/* The hot path.  d_me[nevt] receives ME (fp64 in every build).  If d_rndhel and d_selhel are given,
+ * d_selhel[nevt] receives the first good h with r_hel * S < sum_{h' <= h} |M_h'|^2 (last good one if
+ * rounding leaves none); likewise d_rndcol/d_selcol with the weights w_c = sum_{h good} |J_c(h)|^2
+ * (reading R11).  Enqueues on `stream`, does not synchronise, allocates nothing in steady state. */
+int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const double* d_rndhel,
+               const double* d_rndcol, int64_t nevt, double* d_me, int32_t* d_selhel, int32_t* d_selcol,
+               void* stream);
+
+/* Same call with HOST buffers (pinned or pageable): copies in, computes, copies out and synchronises.
+ * This is the end-to-end path bench.py times as `e2e`. */
+int me_compute_host(me_handle* h, const double* momenta, const double* gs, const double* rndhel,
+                    const double* rndcol, int64_t nevt, double* me, int32_t* selhel, int32_t* selcol);
+
+/* launch geometry of the last me_compute (for reports): threads per block, blocks, registers per thread,
+ * bytes of local (spill) memory per thread of the kernel used */
+int me_launch_info(const me_handle* h, int* threads, int* blocks, int* regs, int* local_bytes);
+
+/* Measured FMA peak of the device: a register-resident dependent-FMA-chain microbenchmark (best of 5
+ * launches of a few ms, synchronous).  precision ME_FP64 or ME_FP32; *tflops receives TFLOP/s with
+ * FMA = 2 FLOP.  This is the denominator of the roofline fractions. */
+int me_fma_peak(int precision, int device, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -56,7 +56,8 @@ class Emitter:
         st = self.st
         self.w("// p: momenta[npar][4] of one event (fp64, E px py pz); invariants are formed in fp64 from")
         self.w("// pairwise products 2 k_i.k_j so that collinear/soft denominators do not cancel (DESIGN.md).")
-        self.w("template <typename T, typename LOAD> ME_HD static void setup(LOAD p, double mt, double wt, Event<T>& ev) {")
+        self.w("template <typename T, typename LOAD> ME_HD static void setup(LOAD p, const me::DevParams& par, Event<T>& ev) {")
+        self.w("const double mt = par.mt, wt = par.wt;")
         self.ind += 1
         self.w(f"double kd[{st.npar}][4];")
         self.w(f"for (int i = 0; i < {st.npar}; i++)")
@@ -111,8 +112,8 @@ class Emitter:
             out = "false" if g < 2 else "true"
             self.w(f"const me::vec4<T> t{st.trees_on[(g,)][0]} = me::polvec(ev.pol[{g}], "
                    f"((h >> {st.npar - 1 - g}) & 1) ? 1 : -1, {out});")
-        self.w(f"const me::spin4<T> psi0 = ev.ub[(h >> {st.npar - 1 - 2}) & 1];")
-        self.w(f"const me::spin4<T> vv = ev.v[(h >> {st.npar - 1 - 3}) & 1];")
+        self.w(f"const me::spin4<T> psi0 = me::select(((h >> {st.npar - 1 - 2}) & 1) != 0, ev.ub[1], ev.ub[0]);")
+        self.w(f"const me::spin4<T> vv = me::select(((h >> {st.npar - 1 - 3}) & 1) != 0, ev.v[1], ev.v[0]);")
         # gluon trees
         done_groups = set()
         for t in st.trees:
@@ -189,6 +190,7 @@ class Emitter:
         self.w(f"// g g -> t tbar + {st.ngl - 2} g, {st.ndiag} Feynman diagrams, {len(st.flows)} colour flows.")
         self.w("#pragma once")
         self.w('#include "../me_ops.cuh"')
+        self.w('#include "../me_params.cuh"')
         self.w(f"struct Proc_{self.name} {{")
         self.ind += 1
         self.w(f"static constexpr int npar = {st.npar}, ncomb = {1 << st.npar}, ncol = {len(st.flows)}, "

@@ -1,0 +1,365 @@
+// me_api.cu -- the C ABI of include/me_b200.h: handles, tables, dispatch to the per-(process, precision)
+// launchers of me_proc.cu.  Host code only; no kernel lives here.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/me_b200.h"
+#include "me_kernels.cuh"
+
+typedef int (*launch_fn)(const me::LaunchArgs&, int mode, void* stream, me::LaunchInfo* info, int dry);
+
+#define ME_DECL(name)                                                                        \
+  int me_launch_##name##_p0(const me::LaunchArgs&, int, void*, me::LaunchInfo*, int);        \
+  int me_launch_##name##_p1(const me::LaunchArgs&, int, void*, me::LaunchInfo*, int);        \
+  int me_launch_##name##_p2(const me::LaunchArgs&, int, void*, me::LaunchInfo*, int);
+ME_DECL(ee_mumu)
+ME_DECL(gg_tt)
+ME_DECL(gg_ttg)
+ME_DECL(gg_ttgg)
+ME_DECL(gg_ttggg)
+
+namespace {
+
+struct ProcDesc {
+  const char* name;
+  int npar, ngl, ndiag;
+  launch_fn fn[3];
+};
+#define ME_ROW(name, npar, ngl, ndiag) \
+  { #name, npar, ngl, ndiag, { me_launch_##name##_p0, me_launch_##name##_p1, me_launch_##name##_p2 } }
+const ProcDesc kProcs[] = {
+    ME_ROW(ee_mumu, 4, 0, 2), ME_ROW(gg_tt, 4, 2, 3), ME_ROW(gg_ttg, 5, 3, 16),
+    ME_ROW(gg_ttgg, 6, 4, 123), ME_ROW(gg_ttggg, 7, 5, 1240),
+};
+
+thread_local std::string g_create_error;
+
+}  // namespace
+
+struct me_handle {
+  const ProcDesc* proc;
+  int precision, device;
+  int npar, ncomb, ncol, denom;
+  me::DevParams par;
+  bool have_good;
+  me::GoodList good;
+  // scratch
+  double* d_cum;
+  size_t cum_bytes;
+  unsigned long long* d_frac;
+  // staging for me_compute_host
+  void* d_stage;
+  size_t stage_bytes;
+  cudaStream_t own_stream;
+  me::LaunchInfo last;
+  mutable std::string err;
+};
+
+namespace {
+
+int fail(const me_handle* h, int code, const std::string& msg) {
+  if (h) h->err = msg; else g_create_error = msg;
+  return code;
+}
+int cuda_fail(const me_handle* h, cudaError_t e, const char* where) {
+  return fail(h, ME_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+int factorial(int n) { int r = 1; for (int k = 2; k <= n; k++) r *= k; return r; }
+
+// permutations of the gluon particle indices in lexicographic order (reading R8)
+void flows_of(const ProcDesc* p, int8_t* out) {
+  int gl[8], n = p->ngl;
+  for (int k = 0; k < n; k++) gl[k] = (k < 2) ? k : k + 2;
+  int idx[8];
+  for (int k = 0; k < n; k++) idx[k] = k;
+  int row = 0;
+  while (true) {
+    for (int k = 0; k < n; k++) out[row * n + k] = (int8_t)gl[idx[k]];
+    row++;
+    int i = n - 2;
+    while (i >= 0 && idx[i] > idx[i + 1]) i--;
+    if (i < 0) break;
+    int j = n - 1;
+    while (idx[j] < idx[i]) j--;
+    int t = idx[i]; idx[i] = idx[j]; idx[j] = t;
+    for (int a = i + 1, b = n - 1; a < b; a++, b--) { t = idx[a]; idx[a] = idx[b]; idx[b] = t; }
+  }
+}
+
+int ensure(me_handle* h, void** p, size_t* have, size_t want) {
+  if (*have >= want) return 0;
+  if (*p) cudaFree(*p);
+  *p = nullptr; *have = 0;
+  cudaError_t e = cudaMalloc(p, want);
+  if (e != cudaSuccess) return fail(h, ME_ERR_NOMEM, std::string("cudaMalloc: ") + cudaGetErrorString(e));
+  *have = want;
+  return 0;
+}
+
+bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) != 0; }
+
+}  // namespace
+
+extern "C" {
+
+int me_create(me_handle** out, const char* process, int precision, const me_params* params, int device) {
+  if (!out || !process) return fail(nullptr, ME_ERR_ARG, "me_create: null argument");
+  *out = nullptr;
+  if (precision < 0 || precision > 2) return fail(nullptr, ME_ERR_ARG, "me_create: precision must be 0, 1 or 2");
+  const ProcDesc* pd = nullptr;
+  for (const ProcDesc& p : kProcs)
+    if (!strcmp(p.name, process)) pd = &p;
+  if (!pd) return fail(nullptr, ME_ERR_PROCESS, std::string("me_create: unknown process '") + process + "'");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "me_create: cudaGetDeviceCount (no CUDA device; this library has no CPU path)");
+  if (device < 0 || device >= ndev) return fail(nullptr, ME_ERR_ARG, "me_create: bad device ordinal");
+  me_handle* h = new (std::nothrow) me_handle();
+  if (!h) return fail(nullptr, ME_ERR_NOMEM, "me_create: out of host memory");
+  h->proc = pd; h->precision = precision; h->device = device;
+  h->npar = pd->npar; h->ncomb = 1 << pd->npar; h->ncol = pd->ngl ? factorial(pd->ngl) : 1;
+  h->denom = pd->ngl ? 4 * 64 * factorial(pd->ngl - 2) : 4;
+  me_params P = {173.0, 1.4915, 91.188, 2.441, 132.507, 1.16639e-5};
+  if (params) P = *params;
+  h->par.mt = P.mt; h->par.wt = P.wt; h->par.mz = P.mz; h->par.wz = P.wz;
+  {  // (alpha, G_F, M_Z) scheme, reading R5
+    const double pi = 3.14159265358979323846, alpha = 1.0 / P.aewm1, mz2 = P.mz * P.mz;
+    const double mw2 = 0.5 * mz2 + std::sqrt(0.25 * mz2 * mz2 - pi * alpha * mz2 / (std::sqrt(2.0) * P.gf));
+    const double sw2 = 1.0 - mw2 / mz2, sc = std::sqrt(sw2 * (1.0 - sw2)), ee = std::sqrt(4.0 * pi * alpha);
+    h->par.ee2 = ee * ee; h->par.gl = ee / sc * (sw2 - 0.5); h->par.gr = ee / sc * sw2;
+  }
+  h->have_good = false; h->good.n = 0;
+  h->d_cum = nullptr; h->cum_bytes = 0; h->d_frac = nullptr; h->d_stage = nullptr; h->stage_bytes = 0;
+  h->own_stream = nullptr;
+  h->last = me::LaunchInfo{0, 0, 0, 0};
+  if ((e = cudaSetDevice(device)) != cudaSuccess || (e = cudaMalloc(&h->d_frac, 128 * sizeof(unsigned long long))) != cudaSuccess) {
+    int rc = cuda_fail(nullptr, e, "me_create");
+    delete h;
+    return rc;
+  }
+  *out = h;
+  return ME_OK;
+}
+
+int me_destroy(me_handle* h) {
+  if (!h) return ME_ERR_ARG;
+  cudaSetDevice(h->device);
+  if (h->d_cum) cudaFree(h->d_cum);
+  if (h->d_frac) cudaFree(h->d_frac);
+  if (h->d_stage) cudaFree(h->d_stage);
+  if (h->own_stream) cudaStreamDestroy(h->own_stream);
+  delete h;
+  return ME_OK;
+}
+
+const char* me_last_error(const me_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int me_info(const me_handle* h, int* npar, int* ncomb, int* ncol, int* ndiag, int* denom) {
+  if (!h) return ME_ERR_ARG;
+  if (npar) *npar = h->npar;
+  if (ncomb) *ncomb = h->ncomb;
+  if (ncol) *ncol = h->ncol;
+  if (ndiag) *ndiag = h->proc->ndiag;
+  if (denom) *denom = h->denom;
+  return ME_OK;
+}
+
+int me_helicity_table(const me_handle* h, int8_t* out) {
+  if (!h || !out) return fail(h, ME_ERR_ARG, "me_helicity_table: null argument");
+  for (int r = 0; r < h->ncomb; r++)
+    for (int k = 0; k < h->npar; k++) out[r * h->npar + k] = ((r >> (h->npar - 1 - k)) & 1) ? 1 : -1;
+  return ME_OK;
+}
+
+int me_color_table(const me_handle* h, int8_t* out) {
+  if (!h) return ME_ERR_ARG;
+  if (h->proc->ngl == 0) return ME_OK;
+  if (!out) return fail(h, ME_ERR_ARG, "me_color_table: null argument");
+  flows_of(h->proc, out);
+  return ME_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// colour matrix, helicity filter, compute
+// ------------------------------------------------------------------------------------------------
+#include "gen/me_tables.h"
+
+namespace {
+
+void cmat_of(const me_handle* h, const int** num, int* den) {
+  const char* n = h->proc->name;
+  if (!strcmp(n, "ee_mumu")) { *num = kCmat_ee_mumu; *den = kCden_ee_mumu; }
+  else if (!strcmp(n, "gg_tt")) { *num = kCmat_gg_tt; *den = kCden_gg_tt; }
+  else if (!strcmp(n, "gg_ttg")) { *num = kCmat_gg_ttg; *den = kCden_gg_ttg; }
+  else if (!strcmp(n, "gg_ttgg")) { *num = kCmat_gg_ttgg; *den = kCden_gg_ttgg; }
+  else { *num = kCmat_gg_ttggg; *den = kCden_gg_ttggg; }
+}
+
+int check_inputs(me_handle* h, const double* d_momenta, const double* d_gs, int64_t nevt, const char* who) {
+  if (!h) return ME_ERR_ARG;
+  if (nevt < 0) return fail(h, ME_ERR_ARG, std::string(who) + ": nevt < 0");
+  if (nevt > 0 && (!d_momenta || (h->proc->ngl && !d_gs))) return fail(h, ME_ERR_ARG, std::string(who) + ": null input pointer");
+  if (misaligned(d_momenta, 8) || misaligned(d_gs, 8)) return fail(h, ME_ERR_ARG, std::string(who) + ": misaligned input pointer");
+  return ME_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int me_color_matrix(const me_handle* h, double* out) {
+  if (!h || !out) return fail(h, ME_ERR_ARG, "me_color_matrix: null argument");
+  const int* num; int den;
+  cmat_of(h, &num, &den);
+  for (int i = 0; i < h->ncol * h->ncol; i++) out[i] = double(num[i]) / double(den);
+  return ME_OK;
+}
+
+int me_filter_helicities(me_handle* h, const double* d_momenta, const double* d_gs, int64_t nevt, void* stream) {
+  int rc = check_inputs(h, d_momenta, d_gs, nevt, "me_filter_helicities");
+  if (rc) return rc;
+  if (nevt == 0) return fail(h, ME_ERR_ARG, "me_filter_helicities: needs at least one event");
+  cudaError_t e = cudaSetDevice(h->device);
+  if (e != cudaSuccess) return cuda_fail(h, e, "me_filter_helicities");
+  cudaStream_t st = (cudaStream_t)stream;
+  if ((e = cudaMemsetAsync(h->d_frac, 0, 128 * sizeof(unsigned long long), st)) != cudaSuccess)
+    return cuda_fail(h, e, "me_filter_helicities: memset");
+  me::LaunchArgs a;
+  memset(&a, 0, sizeof(a));
+  a.mom = d_momenta; a.gs = d_gs; a.nevt = nevt < 16384 ? nevt : 16384;
+  a.fracmax = h->d_frac; a.par = h->par;
+  int ce = h->proc->fn[0](a, me::MODE_FILTER, stream, nullptr, 0);  // always the fp64 build (reading R10)
+  if (ce) return cuda_fail(h, (cudaError_t)ce, "me_filter_helicities: launch");
+  unsigned long long bits[128];
+  if ((e = cudaMemcpyAsync(bits, h->d_frac, sizeof(bits), cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+      (e = cudaStreamSynchronize(st)) != cudaSuccess)
+    return cuda_fail(h, e, "me_filter_helicities: readback");
+  h->good.n = 0;
+  for (int r = 0; r < h->ncomb; r++) {
+    double f;
+    memcpy(&f, &bits[r], sizeof(f));
+    if (f > 1e-12) h->good.h[h->good.n++] = (uint8_t)r;
+  }
+  h->have_good = true;
+  if (h->good.n == 0) return fail(h, ME_ERR_NO_HELICITIES, "me_filter_helicities: no helicity passed the filter");
+  return ME_OK;
+}
+
+int me_get_good_helicities(const me_handle* h, int* ngood, uint8_t* mask) {
+  if (!h) return ME_ERR_ARG;
+  if (!h->have_good) return fail(h, ME_ERR_NO_HELICITIES, "me_get_good_helicities: no helicity mask yet");
+  if (ngood) *ngood = h->good.n;
+  if (mask) {
+    memset(mask, 0, h->ncomb);
+    for (int i = 0; i < h->good.n; i++) mask[h->good.h[i]] = 1;
+  }
+  return ME_OK;
+}
+
+int me_set_good_helicities(me_handle* h, const uint8_t* mask) {
+  if (!h || !mask) return fail(h, ME_ERR_ARG, "me_set_good_helicities: null argument");
+  int n = 0;
+  for (int r = 0; r < h->ncomb; r++) n += mask[r] ? 1 : 0;
+  if (n == 0) return fail(h, ME_ERR_ARG, "me_set_good_helicities: empty mask");
+  h->good.n = 0;
+  for (int r = 0; r < h->ncomb; r++)
+    if (mask[r]) h->good.h[h->good.n++] = (uint8_t)r;
+  h->have_good = true;
+  return ME_OK;
+}
+
+int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const double* d_rndhel,
+               const double* d_rndcol, int64_t nevt, double* d_me, int32_t* d_selhel, int32_t* d_selcol,
+               void* stream) {
+  int rc = check_inputs(h, d_momenta, d_gs, nevt, "me_compute");
+  if (rc) return rc;
+  if (!h->have_good) return fail(h, ME_ERR_NO_HELICITIES, "me_compute: call me_filter_helicities or me_set_good_helicities first");
+  if (nevt > 0 && !d_me) return fail(h, ME_ERR_ARG, "me_compute: null output pointer");
+  if (misaligned(d_me, 8) || misaligned(d_rndhel, 8) || misaligned(d_rndcol, 8) || misaligned(d_selhel, 4) || misaligned(d_selcol, 4))
+    return fail(h, ME_ERR_ARG, "me_compute: misaligned pointer");
+  if ((d_selhel && !d_rndhel) || (d_selcol && !d_rndcol))
+    return fail(h, ME_ERR_ARG, "me_compute: a selection output needs its random-number input");
+  if (nevt == 0) return ME_OK;
+  cudaError_t e = cudaSetDevice(h->device);
+  if (e != cudaSuccess) return cuda_fail(h, e, "me_compute");
+  me::LaunchArgs a;
+  memset(&a, 0, sizeof(a));
+  a.mom = d_momenta; a.gs = d_gs; a.rndhel = d_rndhel; a.rndcol = d_rndcol; a.nevt = nevt;
+  a.me = d_me; a.selhel = d_selhel; a.selcol = d_selcol; a.par = h->par; a.good = h->good;
+  const int mode = (d_selhel || d_selcol) ? me::MODE_SELECT : me::MODE_ME;
+  launch_fn fn = h->proc->fn[h->precision];
+  me::LaunchInfo info;
+  int ce = fn(a, mode, stream, &info, 1);
+  if (ce) return cuda_fail(h, (cudaError_t)ce, "me_compute: launch geometry");
+  if (mode == me::MODE_SELECT) {
+    // running helicity sums [ngood][slots]; grows only when a larger grid is seen (no steady-state allocation)
+    size_t want = sizeof(double) * (size_t)h->good.n * (size_t)info.blocks * (size_t)info.threads;
+    void* p = h->d_cum;
+    rc = ensure(h, &p, &h->cum_bytes, want);
+    h->d_cum = (double*)p;
+    if (rc) return rc;
+    a.cum = h->d_cum;
+  }
+  a.blocks = info.blocks;
+  ce = fn(a, mode, stream, nullptr, 0);
+  if (ce) return cuda_fail(h, (cudaError_t)ce, "me_compute: launch");
+  h->last = info;
+  return ME_OK;
+}
+
+int me_compute_host(me_handle* h, const double* momenta, const double* gs, const double* rndhel,
+                    const double* rndcol, int64_t nevt, double* me_out, int32_t* selhel, int32_t* selcol) {
+  if (!h) return ME_ERR_ARG;
+  if (nevt < 0) return fail(h, ME_ERR_ARG, "me_compute_host: nevt < 0");
+  if (nevt == 0) return ME_OK;
+  if (!momenta || !me_out || (h->proc->ngl && !gs)) return fail(h, ME_ERR_ARG, "me_compute_host: null pointer");
+  cudaError_t e = cudaSetDevice(h->device);
+  if (e != cudaSuccess) return cuda_fail(h, e, "me_compute_host");
+  if (!h->own_stream && (e = cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking)) != cudaSuccess)
+    return cuda_fail(h, e, "me_compute_host: stream");
+  const size_t n = (size_t)nevt, bm = n * h->npar * 4 * 8, b8 = n * 8, b4 = n * 4;
+  // layout of the staging buffer: momenta | gs | rndhel | rndcol | me | selhel | selcol
+  const size_t want = bm + 4 * b8 + 2 * b4 + 64;
+  int rc = ensure(h, &h->d_stage, &h->stage_bytes, want);
+  if (rc) return rc;
+  char* base = (char*)h->d_stage;
+  double* d_mom = (double*)base;
+  double* d_gs = (double*)(base + bm);
+  double* d_rh = (double*)(base + bm + b8);
+  double* d_rc = (double*)(base + bm + 2 * b8);
+  double* d_me = (double*)(base + bm + 3 * b8);
+  int32_t* d_sh = (int32_t*)(base + bm + 4 * b8);
+  int32_t* d_sc = (int32_t*)(base + bm + 4 * b8 + b4);
+  cudaStream_t st = h->own_stream;
+  if ((e = cudaMemcpyAsync(d_mom, momenta, bm, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(h, e, "H2D momenta");
+  if (gs && (e = cudaMemcpyAsync(d_gs, gs, b8, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(h, e, "H2D gs");
+  const bool sh = selhel && rndhel, sc = selcol && rndcol;
+  if (sh && (e = cudaMemcpyAsync(d_rh, rndhel, b8, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(h, e, "H2D rndhel");
+  if (sc && (e = cudaMemcpyAsync(d_rc, rndcol, b8, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(h, e, "H2D rndcol");
+  rc = me_compute(h, d_mom, gs ? d_gs : nullptr, sh ? d_rh : nullptr, sc ? d_rc : nullptr, nevt, d_me,
+                  sh ? d_sh : nullptr, sc ? d_sc : nullptr, st);
+  if (rc) return rc;
+  if ((e = cudaMemcpyAsync(me_out, d_me, b8, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(h, e, "D2H me");
+  if (sh && (e = cudaMemcpyAsync(selhel, d_sh, b4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(h, e, "D2H selhel");
+  if (sc && (e = cudaMemcpyAsync(selcol, d_sc, b4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(h, e, "D2H selcol");
+  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: synchronize");
+  return ME_OK;
+}
+
+int me_launch_info(const me_handle* h, int* threads, int* blocks, int* regs, int* local_bytes) {
+  if (!h) return ME_ERR_ARG;
+  if (threads) *threads = h->last.threads;
+  if (blocks) *blocks = h->last.blocks;
+  if (regs) *regs = h->last.regs;
+  if (local_bytes) *local_bytes = h->last.local_bytes;
+  return ME_OK;
+}
+
+}  // extern "C"

@@ -204,6 +204,14 @@ template <typename T> ME_HD spin4<T> bar(const spin4<T>& u) {
   return r;
 }
 
+// branch-free choice between two register-resident spinors (no dynamic indexing -> no local memory)
+template <typename T> ME_HD spin4<T> select(bool first, const spin4<T>& a, const spin4<T>& b) {
+  spin4<T> r;
+#pragma unroll
+  for (int i = 0; i < 4; i++) r.c[i] = mk<T>(first ? a.c[i].re : b.c[i].re, first ? a.c[i].im : b.c[i].im);
+  return r;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Gluon currents
 // ---------------------------------------------------------------------------------------------

@@ -1,0 +1,140 @@
+"""CPU tests of the product's host side: the build-time generator (colour algebra, diagram structure),
+the C-ABI library's exported symbols, and the binding's refusal to run without a GPU.
+No oracle code is used to produce expected values here: pins are the SU(3) facts of
+tests/golden/color_matrix.txt and the diagram counts of BASELINE.json configs.
+"""
+import ctypes
+import os
+import re
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from helpers import read_golden
+from paper_2503_21935_b200.codegen import colour, diagrams
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+GOLD = read_golden("color_matrix.txt")
+
+
+@pytest.fixture(scope="module")
+def structures():
+    return {n: diagrams.build(n) for n in (2, 3, 4, 5)}
+
+
+def test_diagram_counts(structures):
+    # BASELINE.json configs: 3 / 16 / 123 / 1240 diagrams, 2 / 6 / 24 / 120 colours
+    assert [structures[n].ndiag for n in (2, 3, 4, 5)] == [3, 16, 123, 1240]
+    assert [len(structures[n].flows) for n in (2, 3, 4, 5)] == [2, 6, 24, 120]
+    assert [structures[n].denom for n in (2, 3, 4, 5)] == [256, 256, 512, 1536]
+
+
+def test_colour_matrix_pins(structures):
+    for n in (2, 3, 4, 5):
+        st = structures[n]
+        c = np.array(st.cmat_num, dtype=np.float64) / st.cmat_den
+        assert st.cmat_den == int(GOLD[f"den_{n}"])
+        assert np.array_equal(c, c.T)
+        ev = np.linalg.eigvalsh(c)
+        lo, hi = GOLD[f"eig_{n}"]
+        assert ev[0] > 0 and abs(ev[0] - lo) < 2e-3 * max(1, lo) and abs(ev[-1] - hi) < 1e-2
+        # diagonal = N_c C_F^n = 3 (4/3)^n
+        assert all(Fraction(st.cmat_num[i][i], st.cmat_den) == 3 * Fraction(4, 3) ** n for i in range(len(c)))
+    assert structures[2].cmat_num[0] == [int(x) for x in GOLD["row0_2"]]
+    assert structures[3].cmat_num[0] == [int(x) for x in GOLD["row0_3"]]
+    assert structures[4].cmat_num[0][:8] == [int(x) for x in GOLD["row0_4_head"]]
+    assert sorted(set(v for r in structures[4].cmat_num for v in r)) == sorted(int(x) for x in GOLD["distinct_4"])
+    offdiag = [structures[5].cmat_num[i][j] for i in range(120) for j in range(120) if i != j]
+    assert max(offdiag) == int(GOLD["max_offdiag_5"])
+    assert len(set(v for r in structures[5].cmat_num for v in r)) == int(GOLD["ndistinct_5"])
+
+
+def test_colour_matrix_group_structure(structures):
+    # C_{sigma tau} depends only on sigma^-1 tau
+    st = structures[4]
+    fl = st.flows
+    seen = {}
+    for i, s in enumerate(fl):
+        for j, t in enumerate(fl):
+            rel = tuple(s.index(x) for x in t)
+            assert seen.setdefault(rel, st.cmat_num[i][j]) == st.cmat_num[i][j]
+
+
+def test_fierz_against_explicit_generators():
+    # Tr(T^a T^b T^a T^b) summed = -2/3 and Tr(T^a T^a T^b T^b) = 16/3 for SU(3), from explicit matrices
+    lam = np.zeros((8, 3, 3), dtype=complex)
+    lam[0][0, 1] = lam[0][1, 0] = 1
+    lam[1][0, 1] = -1j; lam[1][1, 0] = 1j
+    lam[2][0, 0] = 1; lam[2][1, 1] = -1
+    lam[3][0, 2] = lam[3][2, 0] = 1
+    lam[4][0, 2] = -1j; lam[4][2, 0] = 1j
+    lam[5][1, 2] = lam[5][2, 1] = 1
+    lam[6][1, 2] = -1j; lam[6][2, 1] = 1j
+    lam[7] = np.diag([1, 1, -2]) / np.sqrt(3)
+    T = lam / 2
+    abab = sum(np.trace(T[a] @ T[b] @ T[a] @ T[b]) for a in range(8) for b in range(8)).real
+    aabb = sum(np.trace(T[a] @ T[a] @ T[b] @ T[b]) for a in range(8) for b in range(8)).real
+    c = colour.colour_matrix([(0, 1), (1, 0)])
+    assert abs(float(c[0][0]) - aabb) < 1e-12 and abs(float(c[0][1]) - abab) < 1e-12
+
+
+def test_commutator_signs_and_reflection(structures):
+    # [[a,b],c] = abc - bac - cab + cba
+    s = colour.commutator(colour.commutator(colour.leaf(0), colour.leaf(1)), colour.leaf(4))
+    assert dict(s) == {(0, 1, 4): 1, (1, 0, 4): -1, (4, 0, 1): -1, (4, 1, 0): 1}
+    # every tree's strings have unit coefficients; ordered currents exist for every canonical sequence
+    st = structures[4]
+    assert all(abs(c) == 1 for t in st.trees for c in t.strings.values())
+    assert len(st.ordered) == 6 + 12 + 12
+    # photon decoupling: the sum over all orderings of a tree's strings vanishes (commutators are traceless sums)
+    assert all(sum(t.strings.values()) == 0 for t in st.trees if t.kind != "leaf")
+
+
+def test_generated_sources_are_deterministic(tmp_path):
+    from paper_2503_21935_b200.codegen.generate import generate_all
+    a = generate_all(str(tmp_path / "a"), only=["gg_ttg"])
+    b = generate_all(str(tmp_path / "b"), only=["gg_ttg"])
+    assert open(a[0]).read() == open(b[0]).read()
+    txt = open(a[0]).read()
+    assert "vvv_current" in txt and "vvvv_currents" in txt and "row_prop" in txt and txt.count("J[") == 6
+
+
+def _declared_symbols():
+    hdr = open(os.path.join(ROOT, "include", "me_b200.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    return sorted(set(re.findall(r"\b(me_[a-z_]+)\s*\(", hdr)))
+
+
+def test_library_exports_every_declared_symbol():
+    """The C-ABI library loads on a machine without a GPU and exports everything include/me_b200.h declares."""
+    from paper_2503_21935_b200 import me
+    if not os.path.exists(me.LIB_PATH):
+        from paper_2503_21935_b200 import build
+        build.build()
+    lib = ctypes.CDLL(me.LIB_PATH)
+    names = _declared_symbols()
+    assert set(names) == set(me.EXPORTS)
+    for n in names:
+        assert hasattr(lib, n), f"{n} is declared in include/me_b200.h but not exported"
+
+
+def test_no_cpu_fallback_without_gpu():
+    """Without a CUDA device the product must fail loudly (no CPU path)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_2503_21935_b200 import me
+    if not os.path.exists(me.LIB_PATH):
+        pytest.skip("library not built")
+    with pytest.raises(me.MEError):
+        me.MatrixElement("gg_tt", "fp64")
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2503_21935_b200")
+    for root, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(root, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt and "me_oracle" not in txt, f
