@@ -14,7 +14,7 @@ import subprocess
 import sys
 from concurrent.futures import ThreadPoolExecutor
 
-from .codegen.generate import generate_all
+from .codegen.generate import GROUP_LAYOUT, generate_all
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
@@ -28,6 +28,8 @@ NVCC_BASE = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", 
 # launch configuration per (process, precision): threads per block, min blocks per SM (register cap)
 TUNE = {
     ("gg_ttggg", 0): (64, 1), ("gg_ttggg", 1): (64, 1), ("gg_ttggg", 2): (64, 1),
+    # lane-group layout: the block size is fixed by the layout, only min blocks/SM (the register cap) is tuned
+    ("gg_ttgg", 0): (128, 3), ("gg_ttgg", 1): (128, 5), ("gg_ttgg", 2): (128, 3),
 }
 DEFAULT_TUNE = (128, 1)
 
@@ -39,7 +41,8 @@ def _units():
             defs = [f"-DME_PROC={p}", f"-DME_PROC_UP={p.upper()}", f"-DME_PREC={prec}", f"-DME_NT={nt}", f"-DME_MINB={minb}"]
             if p == "ee_mumu":
                 defs.append("-DME_IS_EE_MUMU")
-            yield f"{p}_p{prec}", os.path.join(CSRC, "me_proc.cu"), defs
+            src = "me_proc_group.cu" if p in GROUP_LAYOUT else "me_proc.cu"
+            yield f"{p}_p{prec}", os.path.join(CSRC, src), defs
     yield "api", os.path.join(CSRC, "me_api.cu"), []
     yield "peak", os.path.join(CSRC, "me_peak.cu"), []
 
@@ -50,7 +53,9 @@ def _deps_hash(defs):
         for f in sorted(files):
             if f.endswith((".cu", ".cuh", ".h")):
                 # a unit depends on the shared headers and on its own generated header only
-                if f.startswith("proc_") and not any(f == f"proc_{d.split('=')[1]}.cuh" for d in defs if d.startswith("-DME_PROC=")):
+                if f.startswith(("proc_", "grp_", "cmat_")) and not any(
+                        f in (f"proc_{d.split('=')[1]}.cuh", f"grp_{d.split('=')[1]}.cuh", f"cmat_{d.split('=')[1]}.h")
+                        for d in defs if d.startswith("-DME_PROC=")):
                     continue
                 if f == "me_tables.h" and defs:
                     continue

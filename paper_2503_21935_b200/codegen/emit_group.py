@@ -1,0 +1,226 @@
+"""Emitter for the "lane-group" kernel layout (csrc/me_group.cuh): csrc/gen/grp_<name>.cuh.
+
+Layout: one CUDA block per event; a *group* of 2n lanes of one warp owns one
+combination of the n gluon helicities; the helicities of t and tbar are handled inside the group, so
+the gluon currents are computed once per gluon-helicity combination and shared by the four
+(h_t, h_tbar) combinations.  Within a group
+
+  * the colour-ordered gluon currents Jord(seq) are built level by level
+    (length 2, 3, ...), one canonical sequence per lane, from a table of (slot, slot, momentum,
+    sign) words: Jord(seq) = 1/K^2 [ sum_j V3(Jord(seq[:j]), Jord(seq[j:])) + sum_{i<j} V4(...)];
+  * lane (s1, h_t) walks the quark line (steps a3-a5) for the flows that start with gluon s1: the walk
+    is the same straight-line code for every s1 up to a relabelling of the gluons, so it is emitted
+    once in *relative* labels (0 = s1, 1.. = the other gluons in increasing order) and each lane
+    translates relative sequence ids to shared-memory slots through its role's table.
+
+Everything here is index bookkeeping; the arithmetic lives in csrc/me_ops.cuh / me_group.cuh.
+"""
+from __future__ import annotations
+
+import itertools
+
+
+def canonical(seq):
+    """(representative of {seq, reversed seq}, sign): Jord(rev) = (-1)^(len+1) Jord(seq)."""
+    seq = tuple(seq)
+    if len(seq) == 1 or seq[0] < seq[-1]:
+        return seq, 1
+    return tuple(reversed(seq)), (-1) ** (len(seq) + 1)
+
+
+def mask_of(seq):
+    m = 0
+    for i in seq:
+        m |= 1 << i
+    return m
+
+
+class Group:
+    def __init__(self, name: str, n: int):
+        self.name, self.n = name, n
+        idx = tuple(range(n))
+        self.flows = list(itertools.permutations(idx))
+        self.flow_index = {f: i for i, f in enumerate(self.flows)}
+        # slots: canonical sequences of length 1 .. n-1 (the full-length currents are contracted at once)
+        self.slot = {}
+        self.level_seqs = {}
+        for L in range(1, n + 1):
+            seqs = [s for c in itertools.combinations(idx, L) for s in itertools.permutations(c)
+                    if canonical(s)[0] == s]
+            self.level_seqs[L] = seqs
+            if L < n:
+                for s in seqs:
+                    self.slot[s] = len(self.slot)
+        self.nslot = len(self.slot)
+        assert self.nslot < 255 and len(self.flows) <= 128
+
+    def ref(self, seq):
+        can, sgn = canonical(seq)
+        return self.slot[can], sgn
+
+    # ------------------------------------------------------------------ gluon-current task tables
+    def level_table(self, L):
+        """Words per task: [header0, header1, v3 terms (L-1), v4 terms ((L-1)(L-2)/2)]."""
+        words = []
+        for seq in self.level_seqs[L]:
+            top = L == self.n
+            h0 = (255 if top else self.slot[seq]) | (mask_of(seq) << 8)
+            h1 = 0
+            if top:
+                rev = tuple(reversed(seq))
+                rs = (-1) ** (L + 1)
+                h1 = self.flow_index[seq] | (self.flow_index[rev] << 8) | ((1 << 31) if rs < 0 else 0)
+            words += [h0, h1]
+            for j in range(1, L):
+                a, b = seq[:j], seq[j:]
+                (sa, ga), (sb, gb) = self.ref(a), self.ref(b)
+                words.append(sa | (sb << 8) | (mask_of(a) << 16) | (mask_of(b) << 21) | ((1 << 31) if ga * gb < 0 else 0))
+            for i in range(1, L):
+                for j in range(i + 1, L):
+                    a, b, c = seq[:i], seq[i:j], seq[j:]
+                    (sa, ga), (sb, gb), (sc, gc) = self.ref(a), self.ref(b), self.ref(c)
+                    words.append(sa | (sb << 8) | (sc << 16) | ((1 << 31) if ga * gb * gc < 0 else 0))
+        return words
+
+    # ------------------------------------------------------------------ quark-line walk, relative labels
+    def rel_ids(self):
+        """ids of the relative sequences the walk refers to: paths (0, p1..pk) and suffixes over 1..n-1."""
+        n = self.n
+        ids = {}
+        rest = tuple(range(1, n))
+        for k in range(0, n):
+            for p in itertools.permutations(rest, k):
+                ids[(0,) + p] = len(ids)
+        for k in range(1, n):
+            for p in itertools.permutations(rest, k):
+                ids[p] = len(ids)
+        return ids
+
+    def role_table(self, s1, ids):
+        """word per relative sequence for the lanes whose first gluon is s1:
+        bits 0-7 slot, 8-12 subset mask, 16-22 flow (full-length paths), 31 sign."""
+        n = self.n
+        others = [i for i in range(n) if i != s1]
+        amap = {0: s1}
+        for k, o in enumerate(others):
+            amap[k + 1] = o
+        out = [0] * len(ids)
+        for rel, i in ids.items():
+            act = tuple(amap[r] for r in rel)
+            w = mask_of(act) << 8
+            if len(act) == n:
+                w |= self.flow_index[act] << 16
+            else:
+                slot, sgn = self.ref(act)
+                w |= slot | ((1 << 31) if sgn < 0 else 0)
+            out[i] = w
+        return out
+
+    def emit_walk(self, ids):
+        """Straight-line depth-first walk in relative labels (one lane = one (s1, h_t))."""
+        n = self.n
+        L = []
+        ind = [1]
+
+        def w(s):
+            L.append("  " * ind[0] + s)
+
+        w("template <typename T, class CTX> __device__ __forceinline__ static void walk(CTX& c) {")
+        ind[0] += 1
+        w("const me::spin4<T> psi_ext = c.psi0();")
+
+        def node(path):
+            k = len(path)  # number of gluons attached so far, including this node's last one
+            w("{")
+            ind[0] += 1
+            leaf = k == n
+            first = True
+            for j in range(0, k):
+                if leaf and j == 0:
+                    continue  # the all-gluon block was contracted with the t-tbar current in the tree phase
+                seq = path[j:]
+                stack = "psi_ext" if j == 0 else "psi_" + "_".join(str(x) for x in path[:j])
+                if first:
+                    w(f"me::spin4<T> X = me::row_slash({stack}, c.cur({ids[seq]}));")
+                    first = False
+                else:
+                    w(f"me::row_slash_add(X, {stack}, c.cur({ids[seq]}));")
+            if leaf:
+                w(f"c.leaf(X, {ids[path]});")
+            else:
+                name = "psi_" + "_".join(str(x) for x in path)
+                w(f"const me::spin4<T> {name} = c.prop(X, {ids[path]});")
+                for g in range(1, n):
+                    if g not in path:
+                        node(path + (g,))
+            ind[0] -= 1
+            w("}")
+
+        node((0,))
+        ind[0] -= 1
+        w("}")
+        return L
+
+    # ------------------------------------------------------------------ whole file
+    def emit(self, cmat_num, cmat_den, ndiag, denom):
+        n = self.n
+        ids = self.rel_ids()
+        out = []
+        o = out.append
+        o(f"// GENERATED by paper_2503_21935_b200/codegen (emit_group.py) -- do not edit.  Process {self.name}:")
+        o(f"// g g -> t tbar + {n - 2} g in the lane-group layout; {self.nslot} current slots, {len(self.flows)} flows.")
+        o("#pragma once")
+        o('#include "../me_ops.cuh"')
+        for L in range(2, n + 1):
+            tab = self.level_table(L)
+            o(f"__device__ const unsigned int kGrpLevel{L}_{self.name}[] = {{{', '.join(str(x) for x in tab)}}};")
+        roles = []
+        for s1 in range(n):
+            roles += self.role_table(s1, ids)
+        o(f"__device__ const unsigned int kGrpRole_{self.name}[] = {{{', '.join(str(x) for x in roles)}}};")
+        o(f"struct Grp_{self.name} {{")
+        o(f"  static constexpr int n = {n}, npar = {n + 2}, ncomb = {1 << (n + 2)}, ncol = {len(self.flows)}, "
+          f"ndiag = {ndiag}, denom = {denom}, cden = {cmat_den}, nslot = {self.nslot}, nrel = {len(ids)};")
+        o("  __device__ __forceinline__ static const unsigned int* level(int L) {")
+        o("    switch (L) {")
+        for L in range(2, n + 1):
+            o(f"      case {L}: return kGrpLevel{L}_{self.name};")
+        o("    }")
+        o("    return nullptr;")
+        o("  }")
+        o("  __device__ __forceinline__ static int ntask(int L) {")
+        o("    switch (L) {")
+        for L in range(2, n + 1):
+            o(f"      case {L}: return {len(self.level_seqs[L])};")
+        o("    }")
+        o("    return 0;")
+        o("  }")
+        o(f"  __device__ __forceinline__ static const unsigned int* role(int s1) {{ return kGrpRole_{self.name} + s1 * {len(ids)}; }}")
+        out += self.emit_walk(ids)
+        o("};")
+        return "\n".join(out) + "\n"
+
+    # ------------------------------------------------------------------ FLOP accounting (FMA = 2)
+    def flops(self):
+        """Algorithmic FLOPs of this layout per gluon-helicity combination (4 helicities) and per event."""
+        n = self.n
+        V3, V4, SL, SLA, PROP, COL, DOT = 110, 84, 64, 72, 82, 30, 30
+        tree = 0
+        for L in range(2, n + 1):
+            nt = len(self.level_seqs[L])
+            tree += nt * ((L - 1) * V3 + (L - 1) * (L - 2) // 2 * V4 + 8 * (L - 1 + (L - 1) * (L - 2) // 2) + 8)
+        tree += len(self.level_seqs[n]) * 4 * DOT
+        walk = 0
+        rest = n - 1
+        for k in range(1, n + 1):
+            nodes = 1
+            for i in range(k - 1):
+                nodes *= rest - i
+            terms = k - 1 if k == n else k
+            per = SL + (terms - 1) * SLA + (2 * COL + 4 if k == n else PROP)
+            walk += nodes * per
+        walk *= 2 * n  # lanes (s1, h_t)
+        ncol = len(self.flows)
+        colour = 4 * (2 * ncol * (ncol + 1) + 2)
+        return {"per_gluon_combination": tree + walk + colour, "tree": tree, "walk": walk, "colour": colour,
+                "combinations": 1 << n, "per_event": 8 * (n + 2) * (n + 1) // 2 + 40 * (n + 2) + 30 * (1 << n) + 4 * 60}

@@ -136,7 +136,7 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
   h->have_good = false; h->good.n = 0;
   h->d_cum = nullptr; h->cum_bytes = 0; h->d_frac = nullptr; h->d_stage = nullptr; h->stage_bytes = 0;
   h->own_stream = nullptr;
-  h->last = me::LaunchInfo{0, 0, 0, 0};
+  h->last = me::LaunchInfo{0, 0, 0, 0, 0};
   if ((e = cudaSetDevice(device)) != cudaSuccess || (e = cudaMalloc(&h->d_frac, 128 * sizeof(unsigned long long))) != cudaSuccess) {
     int rc = cuda_fail(nullptr, e, "me_create");
     delete h;
@@ -298,9 +298,9 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
   me::LaunchInfo info;
   int ce = fn(a, mode, stream, &info, 1);
   if (ce) return cuda_fail(h, (cudaError_t)ce, "me_compute: launch geometry");
-  if (mode == me::MODE_SELECT) {
+  if (mode == me::MODE_SELECT && info.cum_slots > 0) {
     // running helicity sums [ngood][slots]; grows only when a larger grid is seen (no steady-state allocation)
-    size_t want = sizeof(double) * (size_t)h->good.n * (size_t)info.blocks * (size_t)info.threads;
+    size_t want = sizeof(double) * (size_t)h->good.n * (size_t)info.cum_slots;
     void* p = h->d_cum;
     rc = ensure(h, &p, &h->cum_bytes, want);
     h->d_cum = (double*)p;

@@ -1,0 +1,443 @@
+// me_group.cuh -- the "lane-group" event kernel (layout B2) for g g -> t tbar + (n-2) g, n >= 4.
+//
+// One CUDA block per event.  A GROUP of LPG = 2n lanes of one warp owns one combination of the n gluon
+// helicities; the four (h_t, h_tbar) combinations are handled inside the group, so the gluon currents
+// are computed once per gluon-helicity combination instead of once per helicity.
+// Phases of a group (warp-synchronous, no block barrier until the final reduction):
+//   leaves  lane i < n      : polarisation vector of gluon i (a2)                       -> shared memory slot
+//   tree    lane = sequence : colour-ordered currents Jord(seq), |seq| = 2..n-1 (a3)    -> shared memory slot
+//           |seq| = n       : contracted at once with the four t-tbar currents Q(h_t,h_tbar) -> J init (a4, a5)
+//   walk    lane = (s1,h_t) : quark line for the flows that start with gluon s1 (a3-a5) -> J[flow][h_t][h_tbar]
+//   colour  lane = (h_t,h_tbar,re/im): x^T C x over the n! flows (a6)                   -> |M_h|^2
+// then the block sums the good helicities (a7), selects helicity / colour (a8) and stores (a9).
+// Operands of the walk are read from shared memory with 16-byte loads that are broadcast to the lanes of
+// a group, so one LDS.128 wavefront feeds 8 lanes; the running spinors stay in registers.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "me_kernels.cuh"
+
+namespace me {
+
+template <typename T, typename TC, int N>
+struct alignas(16) GrpEvent {
+  double kd[N + 2][4];         // incoming-convention momenta (+p initial, -p final), fp64
+  double d2[N + 2][N + 2];     // 2 k_i.k_j, i < j
+  double mh[1 << (N + 2)];     // |M_h|^2 (colour-summed, un-normalised) per helicity row
+  T Ksub[1 << N][4];           // sum of the gluon momenta of a subset (bit i = gluon i)
+  T qsub[1 << N][4];           // -(k_t + K_S): momentum of the quark line after the gluons of S
+  T gd[1 << N][2];             // 1 / (q^2 - m^2 + i m Gamma)
+  T ik[1 << N];                // 1 / K_S^2
+  T Q[4][8];                   // ubar(h_t) gamma^mu v(h_tbar), index 2 h_t + h_tbar
+  T ub[2][8], v[2][8];
+  T pol[N][6];
+  T mt;
+  TC wc[((1 << N) * 2 * N + 31) / 32 + 1][(N == 4) ? 24 : (N == 5 ? 120 : 6)];  // per-warp colour weights
+  unsigned char good[1 << (N + 2)];
+};
+
+template <typename T> struct GrpVec;
+template <> struct GrpVec<double> {
+  __device__ __forceinline__ static vec4<double> ld(const double* p, unsigned neg) {
+    vec4<double> r;
+    const double2* q = reinterpret_cast<const double2*>(p);
+    const int m = (int)(neg << 31);
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      const double2 x = q[i];
+      r.c[i].re = __hiloint2double(__double2hiint(x.x) ^ m, __double2loint(x.x));
+      r.c[i].im = __hiloint2double(__double2hiint(x.y) ^ m, __double2loint(x.y));
+    }
+    return r;
+  }
+  __device__ __forceinline__ static void st(double* p, const vec4<double>& a) {
+    double2* q = reinterpret_cast<double2*>(p);
+#pragma unroll
+    for (int i = 0; i < 4; i++) q[i] = make_double2(a.c[i].re, a.c[i].im);
+  }
+};
+template <> struct GrpVec<float> {
+  __device__ __forceinline__ static vec4<float> ld(const float* p, unsigned neg) {
+    vec4<float> r;
+    const float4* q = reinterpret_cast<const float4*>(p);
+    const int m = (int)(neg << 31);
+#pragma unroll
+    for (int i = 0; i < 2; i++) {
+      const float4 x = q[i];
+      r.c[2 * i].re = __int_as_float(__float_as_int(x.x) ^ m);
+      r.c[2 * i].im = __int_as_float(__float_as_int(x.y) ^ m);
+      r.c[2 * i + 1].re = __int_as_float(__float_as_int(x.z) ^ m);
+      r.c[2 * i + 1].im = __int_as_float(__float_as_int(x.w) ^ m);
+    }
+    return r;
+  }
+  __device__ __forceinline__ static void st(float* p, const vec4<float>& a) {
+    float4* q = reinterpret_cast<float4*>(p);
+#pragma unroll
+    for (int i = 0; i < 2; i++) q[i] = make_float4(a.c[2 * i].re, a.c[2 * i].im, a.c[2 * i + 1].re, a.c[2 * i + 1].im);
+  }
+};
+
+template <typename T> __device__ __forceinline__ spin4<T> ld_spin(const T* p) {
+  const vec4<T> x = GrpVec<T>::ld(p, 0u);
+  spin4<T> r;
+#pragma unroll
+  for (int i = 0; i < 4; i++) r.c[i] = x.c[i];
+  return r;
+}
+
+// acc += (A.B)(kA-kB) + ((kA+2kB).A) B - ((2kA+kB).B) A      (three-gluon vertex, propagator applied later)
+template <typename T>
+__device__ __forceinline__ void v3_acc(vec4<T>& acc, const vec4<T>& A, const vec4<T>& B, const T* kA, const T* kB) {
+  const cx<T> ab = mdot(A, B);
+  mom4<T> kab, k1, k2;
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    kab.c[i] = kA[i] - kB[i];
+    k1.c[i] = kA[i] + T(2) * kB[i];
+    k2.c[i] = -(T(2) * kA[i] + kB[i]);
+  }
+  const cx<T> ca = mdot(k1, A), cb = mdot(k2, B);
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    cx<T> t = fma(kab.c[i], ab, acc.c[i]);
+    t = fma(ca, B.c[i], t);
+    acc.c[i] = fma(cb, A.c[i], t);
+  }
+}
+// acc += 2 (A.C) B - (B.C) A - (A.B) C       (colour-ordered four-gluon vertex)
+template <typename T>
+__device__ __forceinline__ void v4_acc(vec4<T>& acc, const vec4<T>& A, const vec4<T>& B, const vec4<T>& C) {
+  const cx<T> ac = T(2) * mdot(A, C), bc = -mdot(B, C), ab = -mdot(A, B);
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    cx<T> t = fma(ac, B.c[i], acc.c[i]);
+    t = fma(bc, A.c[i], t);
+    acc.c[i] = fma(ab, C.c[i], t);
+  }
+}
+
+template <class G, typename T, typename TC, int L>
+__device__ __forceinline__ void grp_tree_level(const GrpEvent<T, TC, G::n>& ev, T* slots, T* J, int r, bool active) {
+  constexpr int LPG = 2 * G::n, NV3 = L - 1, NV4 = (L - 1) * (L - 2) / 2, W = 2 + NV3 + NV4;
+  constexpr bool TOP = (L == G::n);
+  const unsigned* tab = G::level(L);
+  const int nt = G::ntask(L);
+#pragma unroll 1
+  for (int t0 = 0; t0 < nt; t0 += LPG) {
+    const int t = t0 + r;
+    if (active && t < nt) {
+      const unsigned* tw = tab + t * W;
+      const unsigned h0 = __ldg(tw);
+      vec4<T> acc = zero_vec4<T>();
+#pragma unroll
+      for (int j = 0; j < NV3; j++) {
+        const unsigned w = __ldg(tw + 2 + j);
+        const vec4<T> A = GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31);
+        const vec4<T> B = GrpVec<T>::ld(slots + ((w >> 8) & 255u) * 8, 0u);
+        v3_acc(acc, A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
+      }
+#pragma unroll
+      for (int j = 0; j < NV4; j++) {
+        const unsigned w = __ldg(tw + 2 + NV3 + j);
+        const vec4<T> A = GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31);
+        const vec4<T> B = GrpVec<T>::ld(slots + ((w >> 8) & 255u) * 8, 0u);
+        const vec4<T> C = GrpVec<T>::ld(slots + ((w >> 16) & 255u) * 8, 0u);
+        v4_acc(acc, A, B, C);
+      }
+      const T s = ev.ik[(h0 >> 8) & 31u];
+#pragma unroll
+      for (int i = 0; i < 4; i++) acc.c[i] = s * acc.c[i];
+      if (!TOP) {
+        GrpVec<T>::st(slots + (h0 & 255u) * 8, acc);
+      } else {
+        const unsigned h1 = __ldg(tw + 1);
+        T* ja = J + (h1 & 127u) * 8;
+        T* jb = J + ((h1 >> 8) & 127u) * 8;
+        const T sb = (h1 >> 31) ? T(-1) : T(1);
+#pragma unroll
+        for (int v = 0; v < 4; v++) {
+          const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
+          const cx<T> a = mdot(q, acc);
+          ja[2 * v] = a.re; ja[2 * v + 1] = a.im;
+          jb[2 * v] = sb * a.re; jb[2 * v + 1] = sb * a.im;
+        }
+      }
+    }
+  }
+  __syncwarp();
+}
+
+template <class G, typename T, typename TC, int L>
+struct GrpTree {
+  __device__ __forceinline__ static void run(const GrpEvent<T, TC, G::n>& ev, T* slots, T* J, int r, bool active) {
+    GrpTree<G, T, TC, L - 1>::run(ev, slots, J, r, active);
+    grp_tree_level<G, T, TC, L>(ev, slots, J, r, active);
+  }
+};
+template <class G, typename T, typename TC>
+struct GrpTree<G, T, TC, 1> {
+  __device__ __forceinline__ static void run(const GrpEvent<T, TC, G::n>&, T*, T*, int, bool) {}
+};
+
+template <class G, typename T, typename TC>
+struct GrpWalkCtx {
+  const GrpEvent<T, TC, G::n>* ev;
+  const T* slots;
+  T* J;
+  const unsigned* role;
+  int ht;
+  __device__ __forceinline__ spin4<T> psi0() const { return ld_spin<T>(ev->ub[ht]); }
+  __device__ __forceinline__ vec4<T> cur(int id) const {
+    const unsigned w = __ldg(role + id);
+    return GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31);
+  }
+  __device__ __forceinline__ spin4<T> prop(const spin4<T>& X, int id) const {
+    const unsigned m = (__ldg(role + id) >> 8) & 31u;
+    mom4<T> q;
+#pragma unroll
+    for (int i = 0; i < 4; i++) q.c[i] = ev->qsub[m][i];
+    return row_prop(X, q, ev->mt, mk<T>(ev->gd[m][0], ev->gd[m][1]));
+  }
+  __device__ __forceinline__ void leaf(const spin4<T>& X, int id) const {
+    const unsigned f = (__ldg(role + id) >> 16) & 127u;
+    T* j = J + f * 8 + ht * 4;
+#pragma unroll
+    for (int b = 0; b < 2; b++) {
+      const cx<T> a = row_col(X, ld_spin<T>(ev->v[b]));
+      j[2 * b] += a.re;
+      j[2 * b + 1] += a.im;
+    }
+  }
+};
+
+// x^T C x for the real vector x_a = J[a*8 + off] (a < ncol), C = integer numerators CM::at (symmetric)
+template <int NCOL, typename T, typename TC, class CM>
+__device__ __forceinline__ TC grp_quadform(const T* J, int off, TC* x2 /*[NCOL] += x_a^2 or nullptr*/, TC keep) {
+  TC s = TC(0);
+  if (NCOL <= 24) {
+    TC x[NCOL];
+#pragma unroll
+    for (int a = 0; a < NCOL; a++) x[a] = TC(J[a * 8 + off]);
+#pragma unroll
+    for (int a = 0; a < NCOL; a++) {
+      TC y = TC(0.5) * CM::at(a * NCOL + a) * x[a];
+#pragma unroll
+      for (int b = a + 1; b < NCOL; b++) y += CM::at(a * NCOL + b) * x[b];
+      s += x[a] * y;
+      if (x2) x2[a] += keep * x[a] * x[a];
+    }
+  } else {
+    for (int a = 0; a < NCOL; a++) {
+      const TC xa = TC(J[a * 8 + off]);
+      TC y = TC(0.5) * CM::at(a * NCOL + a) * xa;
+#pragma unroll 8
+      for (int b = a + 1; b < NCOL; b++) y += CM::at(a * NCOL + b) * TC(J[b * 8 + off]);
+      s += xa * y;
+      if (x2) x2[a] += keep * xa * xa;
+    }
+  }
+  return TC(2) * s;
+}
+
+template <class G, typename T>
+struct GrpGeom {
+  static constexpr int N = G::n, LPG = 2 * N, GPW = 32 / LPG, NGRP = 1 << N, NW = (NGRP + GPW - 1) / GPW, NT = NW * 32;
+  // T units per group: current slots + J[ncol][4][2]; padded so that the byte stride is 32 mod 128
+  static constexpr int RAW = (G::nslot + G::ncol) * 8;
+  static constexpr int UNIT = 32 / (int)sizeof(T);  // T units in 32 bytes
+  static constexpr int GS = ((RAW + 4 * UNIT - 1) / (4 * UNIT)) * (4 * UNIT) + UNIT;
+};
+
+template <class G, typename T, typename TC, class CM, int MODE, int MINB>
+__global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const LaunchArgs a) {
+  typedef GrpGeom<G, T> GE;
+  constexpr int N = G::n, NPAR = N + 2, NCOMB = 1 << NPAR, LPG = GE::LPG, GPW = GE::GPW, NT = GE::NT;
+  typedef GrpEvent<T, TC, N> EV;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  EV& ev = *reinterpret_cast<EV*>(smem_raw);
+  T* gbase = reinterpret_cast<T*>(smem_raw + ((sizeof(EV) + 127) / 128) * 128);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int gi = lane / LPG, r = lane - gi * LPG;
+  const int grp = warp * GPW + gi;                       // gluon-helicity combination
+  const bool active = (gi < GPW) && (grp < GE::NGRP);
+  T* slots = gbase + (size_t)(active ? grp : 0) * GE::GS;
+  T* J = slots + G::nslot * 8;
+  const double mw = a.par.mt * a.par.wt;
+
+  for (long long e = blockIdx.x; e < a.nevt; e += gridDim.x) {
+    __syncthreads();
+    // ---- a1: load, incoming convention
+    for (int i = tid; i < NPAR * 4; i += NT) {
+      const double x = a.mom[e * (NPAR * 4) + i];
+      ev.kd[i >> 2][i & 3] = (i < 8) ? x : -x;
+    }
+    if (MODE == MODE_FILTER) {
+      for (int i = tid; i < NCOMB; i += NT) ev.good[i] = 1;
+    } else {
+      for (int i = tid; i < NCOMB; i += NT) ev.good[i] = 0;
+    }
+    if (tid == 0) ev.mt = T(a.par.mt);
+    __syncthreads();
+    if (MODE != MODE_FILTER)
+      for (int i = tid; i < a.good.n; i += NT) ev.good[a.good.h[i]] = 1;
+    // ---- per-event, helicity-independent data (a2 bases, invariants in fp64)
+    for (int task = tid; task < NPAR * NPAR + (1 << N) + N + 2; task += NT) {
+      if (task < NPAR * NPAR) {
+        const int i = task / NPAR, j = task - i * NPAR;
+        if (i < j)
+          ev.d2[i][j] = 2.0 * (ev.kd[i][0] * ev.kd[j][0] - ev.kd[i][1] * ev.kd[j][1] - ev.kd[i][2] * ev.kd[j][2] -
+                               ev.kd[i][3] * ev.kd[j][3]);
+      } else if (task < NPAR * NPAR + (1 << N)) {
+        const int m = task - NPAR * NPAR;
+        double k[4] = {0.0, 0.0, 0.0, 0.0};
+        for (int i = 0; i < N; i++)
+          if ((m >> i) & 1) {
+            const int p = (i < 2) ? i : i + 2;
+            for (int c = 0; c < 4; c++) k[c] += ev.kd[p][c];
+          }
+        for (int c = 0; c < 4; c++) {
+          ev.Ksub[m][c] = T(k[c]);
+          ev.qsub[m][c] = T(-(ev.kd[2][c] + k[c]));
+        }
+      } else if (task < NPAR * NPAR + (1 << N) + N) {
+        const int i = task - NPAR * NPAR - (1 << N), p = (i < 2) ? i : i + 2;
+        mom4<T> k;
+        for (int c = 0; c < 4; c++) k.c[c] = T(ev.kd[p][c]);
+        const polbasis<T> pb = make_polbasis<T>((p < 2) ? k : neg(k));
+        for (int c = 0; c < 3; c++) { ev.pol[i][c] = pb.e1[c]; ev.pol[i][3 + c] = pb.e2[c]; }
+      } else {
+        const int which = task - NPAR * NPAR - (1 << N) - N;  // 0: t, 1: tbar
+        mom4<T> k;
+        for (int c = 0; c < 4; c++) k.c[c] = T(-ev.kd[2 + which][c]);
+        const spinbasis<T> sb = make_spinbasis<T>(k, T(a.par.mt));
+        for (int l = 0; l < 2; l++) {
+          const spin4<T> s = which ? spinor_v(sb, l ? 1 : -1) : bar(spinor_u(sb, l ? 1 : -1));
+          T* o = which ? ev.v[l] : ev.ub[l];
+          for (int c = 0; c < 4; c++) { o[2 * c] = s.c[c].re; o[2 * c + 1] = s.c[c].im; }
+        }
+      }
+    }
+    __syncthreads();
+    for (int task = tid; task < (1 << N) + 4; task += NT) {
+      if (task < (1 << N)) {
+        const int m = task;
+        double pairs = 0.0, line = 0.0;
+        int cnt = 0;
+        for (int i = 0; i < N; i++)
+          if ((m >> i) & 1) {
+            const int pi = (i < 2) ? i : i + 2;
+            cnt++;
+            line += (pi < 2) ? ev.d2[pi][2] : ev.d2[2][pi];
+            for (int j = i + 1; j < N; j++)
+              if ((m >> j) & 1) pairs += ev.d2[pi][(j < 2) ? j : j + 2];
+          }
+        ev.ik[m] = (cnt >= 2) ? T(1.0 / pairs) : T(0);
+        const double den = line + pairs, nrm = 1.0 / (den * den + mw * mw);
+        ev.gd[m][0] = (cnt >= 1) ? T(den * nrm) : T(0);
+        ev.gd[m][1] = (cnt >= 1) ? T(-mw * nrm) : T(0);
+      } else {
+        const int v = task - (1 << N);
+        vec4<T> JR, JL;
+        chiral_currents(ld_spin<T>(ev.ub[v >> 1]), ld_spin<T>(ev.v[v & 1]), JR, JL);
+        for (int c = 0; c < 4; c++) { ev.Q[v][2 * c] = JR.c[c].re + JL.c[c].re; ev.Q[v][2 * c + 1] = JR.c[c].im + JL.c[c].im; }
+      }
+    }
+    __syncthreads();
+
+    // ---- a2: polarisation vectors of this group's gluon helicities
+    if (active && r < N) {
+      const int p = (r < 2) ? r : r + 2;
+      const int lam = ((grp >> (N - 1 - r)) & 1) ? 1 : -1;
+      polbasis<T> pb;
+      for (int c = 0; c < 3; c++) { pb.e1[c] = ev.pol[r][c]; pb.e2[c] = ev.pol[r][3 + c]; }
+      GrpVec<T>::st(slots + r * 8, polvec(pb, lam, p >= 2));
+    }
+    __syncwarp();
+    // ---- a3: colour-ordered gluon currents, level by level; the full-length ones initialise J
+    GrpTree<G, T, TC, N>::run(ev, slots, J, r, active);
+    // ---- a3-a5: quark line
+    if (active) {
+      GrpWalkCtx<G, T, TC> c;
+      c.ev = &ev; c.slots = slots; c.J = J; c.role = G::role(r >> 1); c.ht = r & 1;
+      G::template walk<T>(c);
+    }
+    __syncwarp();
+    // ---- a6: colour sums, lane = (variant, re/im)
+    TC wloc[(MODE == MODE_SELECT) ? G::ncol : 1];
+    if (MODE == MODE_SELECT) {
+#pragma unroll
+      for (int c = 0; c < G::ncol; c++) wloc[c] = TC(0);
+    }
+    {
+      TC q = TC(0);
+      int h = 0;
+      if (active && r < 8) {
+        const int v = r >> 1;
+        for (int i = 0; i < N; i++) {
+          const int p = (i < 2) ? i : i + 2;
+          h |= ((grp >> (N - 1 - i)) & 1) << (NPAR - 1 - p);
+        }
+        h |= (v >> 1) << (NPAR - 1 - 2);
+        h |= (v & 1) << (NPAR - 1 - 3);
+        const TC keep = ev.good[h] ? TC(1) : TC(0);
+        q = grp_quadform<G::ncol, T, TC, CM>(J, r, (MODE == MODE_SELECT) ? wloc : nullptr, keep);
+      }
+      q += __shfl_xor_sync(0xffffffffu, q, 1);
+      if (active && r < 8 && !(r & 1)) ev.mh[h] = (double)q;
+    }
+    if (MODE == MODE_SELECT) {
+#pragma unroll
+      for (int c = 0; c < G::ncol; c++) {
+        TC w = wloc[c];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
+        if (lane == 0) ev.wc[warp][c] = w;
+      }
+    }
+    __syncthreads();
+    // ---- a7-a9
+    if (MODE == MODE_FILTER) {
+      double total = 0.0;
+      for (int h = 0; h < NCOMB; h++) total += ev.mh[h];
+      for (int h = tid; h < NCOMB; h += NT) {
+        const double f = (total > 0.0) ? ev.mh[h] / total : 0.0;
+        atomicMax(a.fracmax + h, (unsigned long long)__double_as_longlong(f));
+      }
+    } else if (tid == 0) {
+      double total = 0.0;
+      for (int ih = 0; ih < a.good.n; ih++) total += ev.mh[a.good.h[ih]];
+      const double g = a.gs[e];
+      a.me[e] = total * ipow<2 * N>(g) * (1.0 / (double(G::denom) * double(G::cden)));
+      if (MODE == MODE_SELECT && a.selhel) {
+        const double target = a.rndhel[e] * total;
+        int sel = a.good.h[a.good.n - 1];
+        double run = 0.0;
+        for (int ih = 0; ih < a.good.n; ih++) {
+          run += ev.mh[a.good.h[ih]];
+          if (target < run) { sel = a.good.h[ih]; break; }
+        }
+        a.selhel[e] = sel;
+      }
+    } else if (tid == 32 && MODE == MODE_SELECT && a.selcol) {
+      double tot = 0.0;
+      for (int c = 0; c < G::ncol; c++) {
+        TC w = TC(0);
+        for (int k = 0; k < GE::NW; k++) w += ev.wc[k][c];
+        ev.wc[0][c] = w;
+        tot += (double)w;
+      }
+      const double target = a.rndcol[e] * tot;
+      int sel = G::ncol - 1;
+      double run = 0.0;
+      for (int c = 0; c < G::ncol; c++) {
+        run += (double)ev.wc[0][c];
+        if (target < run) { sel = c; break; }
+      }
+      a.selcol[e] = sel;
+    }
+  }
+}
+
+}  // namespace me

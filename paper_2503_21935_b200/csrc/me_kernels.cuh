@@ -37,6 +37,7 @@ struct LaunchArgs {
 
 struct LaunchInfo {
   int threads, blocks, regs, local_bytes;
+  long long cum_slots;  // MODE_SELECT scratch: doubles per good helicity (0: the kernel keeps them on chip)
 };
 
 enum { MODE_ME = 0, MODE_SELECT = 1, MODE_FILTER = 2 };

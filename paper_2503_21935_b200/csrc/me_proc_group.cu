@@ -1,24 +1,16 @@
-// me_proc.cu -- one translation unit per (process, precision): compiled with
-//   -DME_PROC=<name> -DME_PROC_UP=<NAME> -DME_PREC=<0|1|2> [-DME_NT=<threads>] [-DME_MINB=<min blocks/SM>]
-// and exports  me_launch_<name>_p<prec>  (C++ linkage, called from me_api.cu).
-// ME_PREC: 0 = fp64 (amplitudes and colour sum in double), 1 = fp32 (both float), 2 = mixed (amplitudes
-// double, colour quadratic form float: PAPER.md:108).
-#include "me_kernels.cuh"
+// me_proc_group.cu -- one translation unit per (process, precision) in the lane-group layout (me_group.cuh):
+//   -DME_PROC=<name> -DME_PROC_UP=<NAME> -DME_PREC=<0|1|2> [-DME_MINB=<min blocks/SM>]
+// exports  me_launch_<name>_p<prec>  (C++ linkage, called from me_api.cu), same contract as me_proc.cu.
+#include "me_group.cuh"
 
 #define ME_CAT_(a, b) a##b
 #define ME_CAT(a, b) ME_CAT_(a, b)
 #define ME_STR_(x) #x
 #define ME_STR(x) ME_STR_(x)
 
-#if defined(ME_IS_EE_MUMU)
-#include "proc_ee_mumu.cuh"
-#else
-#include ME_STR(ME_CAT(gen/proc_, ME_PROC).cuh)
-#endif
+#include ME_STR(ME_CAT(gen/grp_, ME_PROC).cuh)
+#include ME_STR(ME_CAT(gen/cmat_, ME_PROC).h)
 
-#ifndef ME_NT
-#define ME_NT 128
-#endif
 #ifndef ME_MINB
 #define ME_MINB 1
 #endif
@@ -34,45 +26,41 @@ typedef double T_amp;
 typedef float T_col;
 #endif
 
-typedef ME_CAT(Proc_, ME_PROC) Proc;
+typedef ME_CAT(Grp_, ME_PROC) Grp;
 
 // colour-matrix numerators: integers, exactly representable in fp32 (<= 4096), as T_col
-__constant__ T_col c_cmat[Proc::ncol * Proc::ncol] = ME_CAT(ME_CMAT_, ME_PROC_UP);
+__constant__ T_col c_cmat[Grp::ncol * Grp::ncol] = ME_CAT(ME_CMAT_, ME_PROC_UP);
 struct CMat {
   __device__ __forceinline__ static T_col at(int i) { return c_cmat[i]; }
 };
 
 template <int MODE, typename TA, typename TCo>
 static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo* info, bool dry) {
-  auto kern = me::event_kernel<Proc, TA, TCo, CMat, MODE, ME_NT, ME_MINB>;
-  int dev = 0, sms = 0, per_sm = 0;
-  cudaError_t err = cudaGetDevice(&dev);
-  if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, ME_NT, 0);
+  typedef me::GrpGeom<Grp, TA> GE;
+  auto kern = me::group_kernel<Grp, TA, TCo, CMat, MODE, ME_MINB>;
+  const size_t ev_bytes = ((sizeof(me::GrpEvent<TA, TCo, Grp::n>) + 127) / 128) * 128;
+  const size_t smem = ev_bytes + (size_t)GE::NGRP * GE::GS * sizeof(TA);
+  cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (err != cudaSuccess) return (int)err;
-  if (per_sm < 1) per_sm = 1;
-  long long ntiles = (a.nevt + ME_NT - 1) / ME_NT;
-  long long blocks = (long long)sms * per_sm;
+  long long blocks = a.nevt;
   if (a.blocks > 0) blocks = a.blocks;
-  if (blocks > ntiles) blocks = ntiles;
+  if (blocks > (1ll << 30)) blocks = 1ll << 30;
   if (blocks < 1) blocks = 1;
   if (info) {
     cudaFuncAttributes fa;
     err = cudaFuncGetAttributes(&fa, kern);
     if (err != cudaSuccess) return (int)err;
-    info->threads = ME_NT;
+    info->threads = GE::NT;
     info->blocks = (int)blocks;
     info->regs = fa.numRegs;
     info->local_bytes = (int)fa.localSizeBytes;
-    info->cum_slots = blocks * ME_NT;
+    info->cum_slots = 0;
   }
   if (dry || a.nevt == 0) return 0;
-  kern<<<(unsigned)blocks, ME_NT, 0, st>>>(a);
+  kern<<<(unsigned)blocks, GE::NT, smem, st>>>(a);
   return (int)cudaGetLastError();
 }
 
-// mode: me::MODE_*; dry = only report the launch geometry (blocks x threads) in *info.
-// The filter always runs in fp64 (reading R10).  Returns a cudaError_t value.
 int ME_CAT(ME_CAT(me_launch_, ME_PROC), ME_CAT(_p, ME_PREC))(const me::LaunchArgs& a, int mode, void* stream,
                                                               me::LaunchInfo* info, int dry) {
   cudaStream_t st = (cudaStream_t)stream;
