@@ -27,7 +27,7 @@ NVCC_BASE = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", 
 
 # launch configuration per (process, precision): threads per block, min blocks per SM (register cap)
 TUNE = {
-    ("gg_ttggg", 0): (64, 1), ("gg_ttggg", 1): (64, 1), ("gg_ttggg", 2): (64, 1),
+    ("gg_ttggg", 0): (128, 1), ("gg_ttggg", 1): (128, 2), ("gg_ttggg", 2): (128, 1),
     # lane-group layout: the block size is fixed by the layout, only min blocks/SM (the register cap) is tuned
     ("gg_ttgg", 0): (128, 3), ("gg_ttgg", 1): (128, 5), ("gg_ttgg", 2): (128, 3),
 }
@@ -41,6 +41,8 @@ def _units():
             defs = [f"-DME_PROC={p}", f"-DME_PROC_UP={p.upper()}", f"-DME_PREC={prec}", f"-DME_NT={nt}", f"-DME_MINB={minb}"]
             if p == "ee_mumu":
                 defs.append("-DME_IS_EE_MUMU")
+            if p == "gg_ttggg":
+                defs.append("-DME_CMAT_GLOBAL=1")
             src = "me_proc_group.cu" if p in GROUP_LAYOUT else "me_proc.cu"
             yield f"{p}_p{prec}", os.path.join(CSRC, src), defs
     yield "api", os.path.join(CSRC, "me_api.cu"), []

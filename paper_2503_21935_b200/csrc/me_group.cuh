@@ -25,15 +25,16 @@ struct alignas(16) GrpEvent {
   double kd[N + 2][4];         // incoming-convention momenta (+p initial, -p final), fp64
   double d2[N + 2][N + 2];     // 2 k_i.k_j, i < j
   double mh[1 << (N + 2)];     // |M_h|^2 (colour-summed, un-normalised) per helicity row
-  T Ksub[1 << N][4];           // sum of the gluon momenta of a subset (bit i = gluon i)
-  T qsub[1 << N][4];           // -(k_t + K_S): momentum of the quark line after the gluons of S
+  alignas(16) T Ksub[1 << N][4];           // sum of the gluon momenta of a subset (bit i = gluon i)
+  alignas(16) T qsub[1 << N][4];           // -(k_t + K_S): momentum of the quark line after the gluons of S
   T gd[1 << N][2];             // 1 / (q^2 - m^2 + i m Gamma)
   T ik[1 << N];                // 1 / K_S^2
-  T Q[4][8];                   // ubar(h_t) gamma^mu v(h_tbar), index 2 h_t + h_tbar
-  T ub[2][8], v[2][8];
+  alignas(16) T Q[4][8];                   // ubar(h_t) gamma^mu v(h_tbar), index 2 h_t + h_tbar
+  alignas(16) T ub[2][8];
+  alignas(16) T v[2][8];
   T pol[N][6];
   T mt;
-  TC wc[((1 << N) * 2 * N + 31) / 32 + 1][(N == 4) ? 24 : (N == 5 ? 120 : 6)];  // per-warp colour weights
+  TC wc[5][(N == 4) ? 24 : (N == 5 ? 120 : 6)];  // per-warp colour weights (at most 4 warps per block)
   unsigned char good[1 << (N + 2)];
 };
 
@@ -243,7 +244,11 @@ __device__ __forceinline__ TC grp_quadform(const T* J, int off, TC* x2 /*[NCOL] 
 
 template <class G, typename T>
 struct GrpGeom {
-  static constexpr int N = G::n, LPG = 2 * N, GPW = 32 / LPG, NGRP = 1 << N, NW = (NGRP + GPW - 1) / GPW, NT = NW * 32;
+  // NGRP combinations per event, processed NPASS groups at a time (n = 4: all 16 at once; n = 5: shared memory
+  // holds 12 of the 32)
+  static constexpr int N = G::n, LPG = 2 * N, GPW = 32 / LPG, NGRP = 1 << N;
+  static constexpr int NPASS = (N <= 4) ? NGRP : 4 * GPW;
+  static constexpr int NW = (NPASS + GPW - 1) / GPW, NT = NW * 32;
   // T units per group: current slots + J[ncol][4][2]; padded so that the byte stride is 32 mod 128
   static constexpr int RAW = (G::nslot + G::ncol) * 8;
   static constexpr int UNIT = 32 / (int)sizeof(T);  // T units in 32 bytes
@@ -260,9 +265,8 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
   T* gbase = reinterpret_cast<T*>(smem_raw + ((sizeof(EV) + 127) / 128) * 128);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int gi = lane / LPG, r = lane - gi * LPG;
-  const int grp = warp * GPW + gi;                       // gluon-helicity combination
-  const bool active = (gi < GPW) && (grp < GE::NGRP);
-  T* slots = gbase + (size_t)(active ? grp : 0) * GE::GS;
+  const int lgrp = warp * GPW + gi;                      // group slot of this lane within a pass
+  T* slots = gbase + (size_t)((gi < GPW && lgrp < GE::NPASS) ? lgrp : 0) * GE::GS;
   T* J = slots + G::nslot * 8;
   const double mw = a.par.mt * a.par.wt;
 
@@ -346,6 +350,15 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
     }
     __syncthreads();
 
+    TC wloc[(MODE == MODE_SELECT) ? G::ncol : 1];
+    if (MODE == MODE_SELECT) {
+#pragma unroll
+      for (int c = 0; c < G::ncol; c++) wloc[c] = TC(0);
+    }
+#pragma unroll 1
+    for (int pass0 = 0; pass0 < GE::NGRP; pass0 += GE::NPASS) {
+    const int grp = pass0 + lgrp;                        // gluon-helicity combination
+    const bool active = (gi < GPW) && (lgrp < GE::NPASS) && (grp < GE::NGRP);
     // ---- a2: polarisation vectors of this group's gluon helicities
     if (active && r < N) {
       const int p = (r < 2) ? r : r + 2;
@@ -365,11 +378,6 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
     }
     __syncwarp();
     // ---- a6: colour sums, lane = (variant, re/im)
-    TC wloc[(MODE == MODE_SELECT) ? G::ncol : 1];
-    if (MODE == MODE_SELECT) {
-#pragma unroll
-      for (int c = 0; c < G::ncol; c++) wloc[c] = TC(0);
-    }
     {
       TC q = TC(0);
       int h = 0;
@@ -387,6 +395,8 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
       q += __shfl_xor_sync(0xffffffffu, q, 1);
       if (active && r < 8 && !(r & 1)) ev.mh[h] = (double)q;
     }
+    __syncwarp();
+    }  // passes
     if (MODE == MODE_SELECT) {
 #pragma unroll
       for (int c = 0; c < G::ncol; c++) {

@@ -14,6 +14,9 @@
 #ifndef ME_MINB
 #define ME_MINB 1
 #endif
+#ifndef ME_CMAT_GLOBAL
+#define ME_CMAT_GLOBAL 0
+#endif
 
 #if ME_PREC == 0
 typedef double T_amp;
@@ -29,17 +32,25 @@ typedef float T_col;
 typedef ME_CAT(Grp_, ME_PROC) Grp;
 
 // colour-matrix numerators: integers, exactly representable in fp32 (<= 4096), as T_col
+// (constant memory up to 24 flows; the 120 x 120 matrix exceeds the 64 KB bank and is read through L1)
+#if ME_CMAT_GLOBAL
+__device__ const T_col c_cmat[Grp::ncol * Grp::ncol] = ME_CAT(ME_CMAT_, ME_PROC_UP);
+struct CMat {
+  __device__ __forceinline__ static T_col at(int i) { return __ldg(c_cmat + i); }
+};
+#else
 __constant__ T_col c_cmat[Grp::ncol * Grp::ncol] = ME_CAT(ME_CMAT_, ME_PROC_UP);
 struct CMat {
   __device__ __forceinline__ static T_col at(int i) { return c_cmat[i]; }
 };
+#endif
 
 template <int MODE, typename TA, typename TCo>
 static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo* info, bool dry) {
   typedef me::GrpGeom<Grp, TA> GE;
   auto kern = me::group_kernel<Grp, TA, TCo, CMat, MODE, ME_MINB>;
   const size_t ev_bytes = ((sizeof(me::GrpEvent<TA, TCo, Grp::n>) + 127) / 128) * 128;
-  const size_t smem = ev_bytes + (size_t)GE::NGRP * GE::GS * sizeof(TA);
+  const size_t smem = ev_bytes + (size_t)GE::NPASS * GE::GS * sizeof(TA);
   cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (err != cudaSuccess) return (int)err;
   long long blocks = a.nevt;
