@@ -83,88 +83,42 @@ class Group:
         return words
 
     # ------------------------------------------------------------------ quark-line walk, relative labels
-    def rel_ids(self):
-        """ids of the relative sequences the walk refers to: paths (0, p1..pk) and suffixes over 1..n-1."""
-        n = self.n
-        ids = {}
-        rest = tuple(range(1, n))
-        for k in range(0, n):
-            for p in itertools.permutations(rest, k):
-                ids[(0,) + p] = len(ids)
-        for k in range(1, n):
-            for p in itertools.permutations(rest, k):
-                ids[p] = len(ids)
-        return ids
+    def role_stream(self, s1):
+        """Words consumed, in execution order, by the lanes whose first gluon is s1 (me_group.cuh GrpWalk).
 
-    def role_table(self, s1, ids):
-        """word per relative sequence for the lanes whose first gluon is s1:
-        bits 0-7 slot, 8-12 subset mask, 16-22 flow (full-length paths), 31 sign."""
+        The walk is a depth-first loop nest over the gluons that follow s1 (relative labels 1.. = the other
+        gluons in increasing order); a node with path (s1, p1..pk) consumes
+          inner node: [path word: slot+sign of Jord(path), subset mask], then Jord(path[j:]) for j = 1..k
+          leaf      : Jord(path[j:]) for j = 1..n-1 (the j = 0 block was contracted in the tree phase),
+                      then [flow word: flow index << 16]
+        word bits: 0-7 slot, 8-12 subset mask, 16-22 flow, 31 sign."""
         n = self.n
         others = [i for i in range(n) if i != s1]
-        amap = {0: s1}
-        for k, o in enumerate(others):
-            amap[k + 1] = o
-        out = [0] * len(ids)
-        for rel, i in ids.items():
-            act = tuple(amap[r] for r in rel)
-            w = mask_of(act) << 8
-            if len(act) == n:
-                w |= self.flow_index[act] << 16
-            else:
-                slot, sgn = self.ref(act)
-                w |= slot | ((1 << 31) if sgn < 0 else 0)
-            out[i] = w
-        return out
+        out = []
 
-    def emit_walk(self, ids):
-        """Straight-line depth-first walk in relative labels (one lane = one (s1, h_t))."""
-        n = self.n
-        L = []
-        ind = [1]
-
-        def w(s):
-            L.append("  " * ind[0] + s)
-
-        w("template <typename T, class CTX> __device__ __forceinline__ static void walk(CTX& c) {")
-        ind[0] += 1
-        w("const me::spin4<T> psi_ext = c.psi0();")
+        def cur_word(seq):
+            slot, sgn = self.ref(seq)
+            return slot | (mask_of(seq) << 8) | ((1 << 31) if sgn < 0 else 0)
 
         def node(path):
-            k = len(path)  # number of gluons attached so far, including this node's last one
-            w("{")
-            ind[0] += 1
-            leaf = k == n
-            first = True
-            for j in range(0, k):
-                if leaf and j == 0:
-                    continue  # the all-gluon block was contracted with the t-tbar current in the tree phase
-                seq = path[j:]
-                stack = "psi_ext" if j == 0 else "psi_" + "_".join(str(x) for x in path[:j])
-                if first:
-                    w(f"me::spin4<T> X = me::row_slash({stack}, c.cur({ids[seq]}));")
-                    first = False
-                else:
-                    w(f"me::row_slash_add(X, {stack}, c.cur({ids[seq]}));")
-            if leaf:
-                w(f"c.leaf(X, {ids[path]});")
-            else:
-                name = "psi_" + "_".join(str(x) for x in path)
-                w(f"const me::spin4<T> {name} = c.prop(X, {ids[path]});")
-                for g in range(1, n):
-                    if g not in path:
-                        node(path + (g,))
-            ind[0] -= 1
-            w("}")
+            if len(path) == n:
+                for j in range(1, n):
+                    out.append(cur_word(path[j:]))
+                out.append((self.flow_index[path] << 16) | (mask_of(path) << 8))
+                return
+            out.append(cur_word(path))
+            for j in range(1, len(path)):
+                out.append(cur_word(path[j:]))
+            for g in others:
+                if g not in path:
+                    node(path + (g,))
 
-        node((0,))
-        ind[0] -= 1
-        w("}")
-        return L
+        node((s1,))
+        return out
 
     # ------------------------------------------------------------------ whole file
     def emit(self, cmat_num, cmat_den, ndiag, denom):
         n = self.n
-        ids = self.rel_ids()
         out = []
         o = out.append
         o(f"// GENERATED by paper_2503_21935_b200/codegen (emit_group.py) -- do not edit.  Process {self.name}:")
@@ -176,11 +130,13 @@ class Group:
             o(f"__device__ const unsigned int kGrpLevel{L}_{self.name}[] = {{{', '.join(str(x) for x in tab)}}};")
         roles = []
         for s1 in range(n):
-            roles += self.role_table(s1, ids)
+            st = self.role_stream(s1)
+            nstream = len(st)
+            roles += st
         o(f"__device__ const unsigned int kGrpRole_{self.name}[] = {{{', '.join(str(x) for x in roles)}}};")
         o(f"struct Grp_{self.name} {{")
         o(f"  static constexpr int n = {n}, npar = {n + 2}, ncomb = {1 << (n + 2)}, ncol = {len(self.flows)}, "
-          f"ndiag = {ndiag}, denom = {denom}, cden = {cmat_den}, nslot = {self.nslot}, nrel = {len(ids)};")
+          f"ndiag = {ndiag}, denom = {denom}, cden = {cmat_den}, nslot = {self.nslot}, nstream = {nstream};")
         o("  __device__ __forceinline__ static const unsigned int* level(int L) {")
         o("    switch (L) {")
         for L in range(2, n + 1):
@@ -195,8 +151,7 @@ class Group:
         o("    }")
         o("    return 0;")
         o("  }")
-        o(f"  __device__ __forceinline__ static const unsigned int* role(int s1) {{ return kGrpRole_{self.name} + s1 * {len(ids)}; }}")
-        out += self.emit_walk(ids)
+        o(f"  __device__ __forceinline__ static const unsigned int* role(int s1) {{ return kGrpRole_{self.name} + s1 * {nstream}; }}")
         o("};")
         return "\n".join(out) + "\n"
 
@@ -204,12 +159,14 @@ class Group:
     def flops(self):
         """Algorithmic FLOPs of this layout per gluon-helicity combination (4 helicities) and per event."""
         n = self.n
-        V3, V4, SL, SLA, PROP, COL, DOT = 110, 84, 64, 72, 82, 30, 30
+        # per-op counts derived line by line from me_group.cuh (v3_acc, v4_acc) and me_ops.cuh (row_slash, row_slash_add,
+        # row_prop, row_col, mdot): complex multiply 6, complex fma 8, real*complex fma 4
+        V3, V4, SL, SLA, PROP, COL, DOT = 162, 188, 64, 72, 82, 30, 30
         tree = 0
         for L in range(2, n + 1):
             nt = len(self.level_seqs[L])
-            tree += nt * ((L - 1) * V3 + (L - 1) * (L - 2) // 2 * V4 + 8 * (L - 1 + (L - 1) * (L - 2) // 2) + 8)
-        tree += len(self.level_seqs[n]) * 4 * DOT
+            tree += nt * ((L - 1) * V3 + (L - 1) * (L - 2) // 2 * V4 + 8)
+        tree += len(self.level_seqs[n]) * (4 * DOT + 8)
         walk = 0
         rest = n - 1
         for k in range(1, n + 1):

@@ -182,34 +182,55 @@ struct GrpTree<G, T, TC, 1> {
   __device__ __forceinline__ static void run(const GrpEvent<T, TC, G::n>&, T*, T*, int, bool) {}
 };
 
+// Quark-line walk of lane (s1, h_t): depth-first loop nest over the gluons that follow s1.  The words are read
+// in execution order from the role's stream (emit_group.py role_stream); psi[j] = Psi(path[:j]) stays in registers.
 template <class G, typename T, typename TC>
 struct GrpWalkCtx {
   const GrpEvent<T, TC, G::n>* ev;
   const T* slots;
   T* J;
-  const unsigned* role;
+  const unsigned* stream;
   int ht;
-  __device__ __forceinline__ spin4<T> psi0() const { return ld_spin<T>(ev->ub[ht]); }
-  __device__ __forceinline__ vec4<T> cur(int id) const {
-    const unsigned w = __ldg(role + id);
-    return GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31);
-  }
-  __device__ __forceinline__ spin4<T> prop(const spin4<T>& X, int id) const {
-    const unsigned m = (__ldg(role + id) >> 8) & 31u;
+  __device__ __forceinline__ unsigned next() { return __ldg(stream++); }
+  __device__ __forceinline__ vec4<T> cur(unsigned w) const { return GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31); }
+  __device__ __forceinline__ spin4<T> prop(const spin4<T>& X, unsigned w) const {
+    const unsigned m = (w >> 8) & 31u;
     mom4<T> q;
 #pragma unroll
     for (int i = 0; i < 4; i++) q.c[i] = ev->qsub[m][i];
     return row_prop(X, q, ev->mt, mk<T>(ev->gd[m][0], ev->gd[m][1]));
   }
-  __device__ __forceinline__ void leaf(const spin4<T>& X, int id) const {
-    const unsigned f = (__ldg(role + id) >> 16) & 127u;
-    T* j = J + f * 8 + ht * 4;
+  __device__ __forceinline__ void leaf(const spin4<T>& X, unsigned w) const {
+    T* j = J + ((w >> 16) & 127u) * 8 + ht * 4;
 #pragma unroll
     for (int b = 0; b < 2; b++) {
       const cx<T> a = row_col(X, ld_spin<T>(ev->v[b]));
       j[2 * b] += a.re;
       j[2 * b + 1] += a.im;
     }
+  }
+};
+
+// node whose path holds D gluons; psi[0..D-1] are valid on entry
+template <class G, typename T, typename TC, int D>
+struct GrpWalk {
+  __device__ __forceinline__ static void node(GrpWalkCtx<G, T, TC>& c, spin4<T> (&psi)[G::n]) {
+    const unsigned w0 = c.next();
+    spin4<T> X = row_slash(psi[0], c.cur(w0));
+#pragma unroll
+    for (int j = 1; j < D; j++) row_slash_add(X, psi[j], c.cur(c.next()));
+    psi[D] = c.prop(X, w0);
+#pragma unroll 1
+    for (int child = 0; child < G::n - D; child++) GrpWalk<G, T, TC, D + 1>::node(c, psi);
+  }
+};
+template <class G, typename T, typename TC>
+struct GrpWalk<G, T, TC, G::n> {
+  __device__ __forceinline__ static void node(GrpWalkCtx<G, T, TC>& c, spin4<T> (&psi)[G::n]) {
+    spin4<T> X = row_slash(psi[1], c.cur(c.next()));
+#pragma unroll
+    for (int j = 2; j < G::n; j++) row_slash_add(X, psi[j], c.cur(c.next()));
+    c.leaf(X, c.next());
   }
 };
 
@@ -373,8 +394,10 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
     // ---- a3-a5: quark line
     if (active) {
       GrpWalkCtx<G, T, TC> c;
-      c.ev = &ev; c.slots = slots; c.J = J; c.role = G::role(r >> 1); c.ht = r & 1;
-      G::template walk<T>(c);
+      c.ev = &ev; c.slots = slots; c.J = J; c.stream = G::role(r >> 1); c.ht = r & 1;
+      spin4<T> psi[G::n];
+      psi[0] = ld_spin<T>(ev.ub[c.ht]);
+      GrpWalk<G, T, TC, 1>::node(c, psi);
     }
     __syncwarp();
     // ---- a6: colour sums, lane = (variant, re/im)
