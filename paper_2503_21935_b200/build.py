@@ -29,7 +29,7 @@ NVCC_BASE = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", 
 TUNE = {
     ("gg_ttggg", 0): (128, 1), ("gg_ttggg", 1): (128, 2), ("gg_ttggg", 2): (128, 1),
     # lane-group layout: the block size is fixed by the layout, only min blocks/SM (the register cap) is tuned
-    ("gg_ttgg", 0): (128, 3), ("gg_ttgg", 1): (128, 5), ("gg_ttgg", 2): (128, 3),
+    ("gg_ttgg", 0): (64, 4), ("gg_ttgg", 1): (64, 8), ("gg_ttgg", 2): (64, 4),
 }
 DEFAULT_TUNE = (128, 1)
 

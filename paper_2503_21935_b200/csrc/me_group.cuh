@@ -1,6 +1,7 @@
 // me_group.cuh -- the "lane-group" event kernel (layout B2) for g g -> t tbar + (n-2) g, n >= 4.
 //
-// One CUDA block per event.  A GROUP of LPG = 2n lanes of one warp owns one combination of the n gluon
+// One CUDA block per event.  A GROUP of LPG lanes of one warp (n lanes, or 2n when the t helicities are split over
+// lanes) owns one combination of the n gluon
 // helicities; the four (h_t, h_tbar) combinations are handled inside the group, so the gluon currents
 // are computed once per gluon-helicity combination instead of once per helicity.
 // Phases of a group (warp-synchronous, no block barrier until the final reduction):
@@ -119,9 +120,25 @@ __device__ __forceinline__ void v4_acc(vec4<T>& acc, const vec4<T>& A, const vec
   }
 }
 
+template <class G, typename T>
+struct GrpGeom {
+  // NGRP combinations per event, processed NPASS groups at a time (n = 4: all 16 at once; n = 5: shared memory
+  // holds 12 of the 32)
+  // HTL: both t helicities are walked by the same lane (every current loaded from shared memory feeds two
+  // quark-line products); otherwise lanes are (s1, h_t) pairs
+  static constexpr bool HTL = (G::n <= 4);
+  static constexpr int N = G::n, NHT = HTL ? 2 : 1, LPG = HTL ? N : 2 * N, GPW = 32 / LPG, NGRP = 1 << N;
+  static constexpr int NPASS = (N <= 4) ? NGRP : 4 * GPW;
+  static constexpr int NW = (NPASS + GPW - 1) / GPW, NT = NW * 32;
+  // T units per group: current slots + J[ncol][4][2]; padded so that the byte stride is 32 mod 128
+  static constexpr int RAW = (G::nslot + G::ncol) * 8;
+  static constexpr int UNIT = 32 / (int)sizeof(T);  // T units in 32 bytes
+  static constexpr int GS = ((RAW + 4 * UNIT - 1) / (4 * UNIT)) * (4 * UNIT) + UNIT;
+};
+
 template <class G, typename T, typename TC, int L>
 __device__ __forceinline__ void grp_tree_level(const GrpEvent<T, TC, G::n>& ev, T* slots, T* J, int r, bool active) {
-  constexpr int LPG = 2 * G::n, NV3 = L - 1, NV4 = (L - 1) * (L - 2) / 2, W = 2 + NV3 + NV4;
+  constexpr int LPG = GrpGeom<G, T>::LPG, NV3 = L - 1, NV4 = (L - 1) * (L - 2) / 2, W = 2 + NV3 + NV4;
   constexpr bool TOP = (L == G::n);
   const unsigned* tab = G::level(L);
   const int nt = G::ntask(L);
@@ -193,15 +210,15 @@ struct GrpWalkCtx {
   int ht;
   __device__ __forceinline__ unsigned next() { return __ldg(stream++); }
   __device__ __forceinline__ vec4<T> cur(unsigned w) const { return GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31); }
-  __device__ __forceinline__ spin4<T> prop(const spin4<T>& X, unsigned w) const {
+  // q and the denominator of the propagator after the gluons of word w (shared by both t helicities)
+  __device__ __forceinline__ void prop_data(unsigned w, mom4<T>& q, cx<T>& gd) const {
     const unsigned m = (w >> 8) & 31u;
-    mom4<T> q;
 #pragma unroll
     for (int i = 0; i < 4; i++) q.c[i] = ev->qsub[m][i];
-    return row_prop(X, q, ev->mt, mk<T>(ev->gd[m][0], ev->gd[m][1]));
+    gd = mk<T>(ev->gd[m][0], ev->gd[m][1]);
   }
-  __device__ __forceinline__ void leaf(const spin4<T>& X, unsigned w) const {
-    T* j = J + ((w >> 16) & 127u) * 8 + ht * 4;
+  __device__ __forceinline__ void leaf(const spin4<T>& X, unsigned w, int h) const {
+    T* j = J + ((w >> 16) & 127u) * 8 + h * 4;
 #pragma unroll
     for (int b = 0; b < 2; b++) {
       const cx<T> a = row_col(X, ld_spin<T>(ev->v[b]));
@@ -211,26 +228,52 @@ struct GrpWalkCtx {
   }
 };
 
-// node whose path holds D gluons; psi[0..D-1] are valid on entry
-template <class G, typename T, typename TC, int D>
+// node whose path holds D gluons; psi[h][0..D-1] are valid on entry (h runs over the NHT t helicities of the lane)
+template <class G, typename T, typename TC, int NHT, int D>
 struct GrpWalk {
-  __device__ __forceinline__ static void node(GrpWalkCtx<G, T, TC>& c, spin4<T> (&psi)[G::n]) {
+  __device__ __forceinline__ static void node(GrpWalkCtx<G, T, TC>& c, spin4<T> (&psi)[NHT][G::n]) {
     const unsigned w0 = c.next();
-    spin4<T> X = row_slash(psi[0], c.cur(w0));
+    spin4<T> X[NHT];
+    {
+      const vec4<T> J0 = c.cur(w0);
 #pragma unroll
-    for (int j = 1; j < D; j++) row_slash_add(X, psi[j], c.cur(c.next()));
-    psi[D] = c.prop(X, w0);
+      for (int h = 0; h < NHT; h++) X[h] = row_slash(psi[h][0], J0);
+    }
+#pragma unroll
+    for (int j = 1; j < D; j++) {
+      const vec4<T> Jj = c.cur(c.next());
+#pragma unroll
+      for (int h = 0; h < NHT; h++) row_slash_add(X[h], psi[h][j], Jj);
+    }
+    {
+      mom4<T> q;
+      cx<T> gd;
+      c.prop_data(w0, q, gd);
+#pragma unroll
+      for (int h = 0; h < NHT; h++) psi[h][D] = row_prop(X[h], q, c.ev->mt, gd);
+    }
 #pragma unroll 1
-    for (int child = 0; child < G::n - D; child++) GrpWalk<G, T, TC, D + 1>::node(c, psi);
+    for (int child = 0; child < G::n - D; child++) GrpWalk<G, T, TC, NHT, D + 1>::node(c, psi);
   }
 };
-template <class G, typename T, typename TC>
-struct GrpWalk<G, T, TC, G::n> {
-  __device__ __forceinline__ static void node(GrpWalkCtx<G, T, TC>& c, spin4<T> (&psi)[G::n]) {
-    spin4<T> X = row_slash(psi[1], c.cur(c.next()));
+template <class G, typename T, typename TC, int NHT>
+struct GrpWalk<G, T, TC, NHT, G::n> {
+  __device__ __forceinline__ static void node(GrpWalkCtx<G, T, TC>& c, spin4<T> (&psi)[NHT][G::n]) {
+    spin4<T> X[NHT];
+    {
+      const vec4<T> J1 = c.cur(c.next());
 #pragma unroll
-    for (int j = 2; j < G::n; j++) row_slash_add(X, psi[j], c.cur(c.next()));
-    c.leaf(X, c.next());
+      for (int h = 0; h < NHT; h++) X[h] = row_slash(psi[h][1], J1);
+    }
+#pragma unroll
+    for (int j = 2; j < G::n; j++) {
+      const vec4<T> Jj = c.cur(c.next());
+#pragma unroll
+      for (int h = 0; h < NHT; h++) row_slash_add(X[h], psi[h][j], Jj);
+    }
+    const unsigned w = c.next();
+#pragma unroll
+    for (int h = 0; h < NHT; h++) c.leaf(X[h], w, (NHT == 2) ? h : c.ht);
   }
 };
 
@@ -262,19 +305,6 @@ __device__ __forceinline__ TC grp_quadform(const T* J, int off, TC* x2 /*[NCOL] 
   }
   return TC(2) * s;
 }
-
-template <class G, typename T>
-struct GrpGeom {
-  // NGRP combinations per event, processed NPASS groups at a time (n = 4: all 16 at once; n = 5: shared memory
-  // holds 12 of the 32)
-  static constexpr int N = G::n, LPG = 2 * N, GPW = 32 / LPG, NGRP = 1 << N;
-  static constexpr int NPASS = (N <= 4) ? NGRP : 4 * GPW;
-  static constexpr int NW = (NPASS + GPW - 1) / GPW, NT = NW * 32;
-  // T units per group: current slots + J[ncol][4][2]; padded so that the byte stride is 32 mod 128
-  static constexpr int RAW = (G::nslot + G::ncol) * 8;
-  static constexpr int UNIT = 32 / (int)sizeof(T);  // T units in 32 bytes
-  static constexpr int GS = ((RAW + 4 * UNIT - 1) / (4 * UNIT)) * (4 * UNIT) + UNIT;
-};
 
 template <class G, typename T, typename TC, class CM, int MODE, int MINB>
 __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const LaunchArgs a) {
@@ -394,18 +424,24 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
     // ---- a3-a5: quark line
     if (active) {
       GrpWalkCtx<G, T, TC> c;
-      c.ev = &ev; c.slots = slots; c.J = J; c.stream = G::role(r >> 1); c.ht = r & 1;
-      spin4<T> psi[G::n];
-      psi[0] = ld_spin<T>(ev.ub[c.ht]);
-      GrpWalk<G, T, TC, 1>::node(c, psi);
+      c.ev = &ev; c.slots = slots; c.J = J;
+      c.stream = G::role(GE::HTL ? r : (r >> 1));
+      c.ht = GE::HTL ? 0 : (r & 1);
+      spin4<T> psi[GE::NHT][G::n];
+#pragma unroll
+      for (int h = 0; h < GE::NHT; h++) psi[h][0] = ld_spin<T>(ev.ub[GE::HTL ? h : c.ht]);
+      GrpWalk<G, T, TC, GE::NHT, 1>::node(c, psi);
     }
     __syncwarp();
-    // ---- a6: colour sums, lane = (variant, re/im)
-    {
+    // ---- a6: colour sums, task = (variant, re/im): 8 per group, lane r takes tasks r, r + LPG, ...
+#pragma unroll 1
+    for (int k0 = 0; k0 < 8; k0 += LPG) {
+      const int k = k0 + r;
       TC q = TC(0);
       int h = 0;
-      if (active && r < 8) {
-        const int v = r >> 1;
+      const bool on = active && k < 8;
+      if (on) {
+        const int v = k >> 1;
         for (int i = 0; i < N; i++) {
           const int p = (i < 2) ? i : i + 2;
           h |= ((grp >> (N - 1 - i)) & 1) << (NPAR - 1 - p);
@@ -413,10 +449,10 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
         h |= (v >> 1) << (NPAR - 1 - 2);
         h |= (v & 1) << (NPAR - 1 - 3);
         const TC keep = ev.good[h] ? TC(1) : TC(0);
-        q = grp_quadform<G::ncol, T, TC, CM>(J, r, (MODE == MODE_SELECT) ? wloc : nullptr, keep);
+        q = grp_quadform<G::ncol, T, TC, CM>(J, k, (MODE == MODE_SELECT) ? wloc : nullptr, keep);
       }
       q += __shfl_xor_sync(0xffffffffu, q, 1);
-      if (active && r < 8 && !(r & 1)) ev.mh[h] = (double)q;
+      if (on && !(k & 1)) ev.mh[h] = (double)q;
     }
     __syncwarp();
     }  // passes
