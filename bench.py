@@ -27,8 +27,16 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 from paper_2503_21935_b200 import inputs as I  # noqa: E402
+from paper_2503_21935_b200.shard import max_over_ranks, rank_range  # noqa: E402
 
-METRIC = "matrix elements/sec (MEs/s) for gg->ttbar gg on 1 B200"
+# DRAM traffic per event of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full
+# capture, profiles/r1_ttgg_fp64_group_v2_ncu_full.txt: 14.24 MB for 65536 events); algorithmic bytes are
+# 6*4*8 + 8 + 16 + 16 = 232 B per event
+TRAFFIC_BYTES_PER_EVENT = {"gg_ttgg": 14.24256e6 / 65536}
+# SURVEY.md 8(d) accounting ("each distinct current once per helicity"): FLOPs of the one-event-per-thread code
+PER_HELICITY_ACCOUNTING = {"gg_ttgg": 30331 * 64 + 672}
+
+METRIC = "matrix elements/sec (MEs/s) for gg->ttbar gg fp64 & fp32 on 1 B200; % of FMA peak"
 UNIT = "MEs/s"
 ALPHAS = {"ee_mumu": 0.118, "gg_tt": 0.118, "gg_ttg": 0.118, "gg_ttgg": None, "gg_ttggg": 0.118}
 DTYPE = {"fp64": "f64", "fp32": "f32", "mixed": "f64+f32"}
@@ -43,7 +51,7 @@ def parse():
     ap.add_argument("--process", default="gg_ttgg")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--sweep", action="store_true", help="add the events-per-launch sweep 2^14..2^22")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the events-per-launch sweep 2^14..2^22")
     ap.add_argument("--no-extras", action="store_true", help="skip fp32/mixed lines, cpu_baseline and e2e")
     return ap.parse_args()
 
@@ -192,8 +200,13 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    # seeded inputs: rank r takes events [r*nevt, (r+1)*nevt) of the stream (disjoint shards, no exchange)
-    mom_h, gs_h, rh_h, rc_h = make_inputs(process, nevt, seed=1, start=rank * nevt)
+    # seeded inputs: rank r takes events [r*nevt, (r+1)*nevt) of the stream (disjoint shards, no exchange);
+    # rank 0 generates up to 2^22 events when it also runs the events-per-launch sweep
+    sweep = rank == 0 and not a.no_extras and not a.no_sweep and process == "gg_ttgg"
+    start, stop = rank_range(nevt, rank, world)
+    nmax = max(nevt, 1 << 22) if sweep else nevt
+    mom_all, gs_all, rh_all, rc_all = make_inputs(process, nmax, seed=1, start=start)
+    mom_h, gs_h, rh_h, rc_h = mom_all[:nevt], gs_all[:nevt], rh_all[:nevt], rc_all[:nevt]
     t = lambda x: torch.from_numpy(x).to(dev)
     bufs = (t(mom_h), t(gs_h), t(rh_h), t(rc_h), torch.empty(nevt, dtype=torch.float64, device=dev),
             torch.empty(nevt, dtype=torch.int32, device=dev), torch.empty(nevt, dtype=torch.int32, device=dev))
@@ -210,10 +223,7 @@ def main():
         return m, mask, total_ms, per, cs.summary(), info
 
     m, mask, total_ms, per, clocks, info = bench_precision(a.precision, a.steps, a.warmup)
-    tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    total_ms = float(tmax.item())
+    total_ms = max_over_ranks(total_ms, dist if world > 1 else None, dev)
     ms_per_step = total_ms / a.steps
     value = world * nevt / (ms_per_step * 1e-3)
     ngood = int(mask.sum())
@@ -235,9 +245,13 @@ def main():
         kernel_ms = float(np.mean(per))
         achieved = fl * nevt / (kernel_ms * 1e-3) * 1e-12
         line["roofline"] = {
-            "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
-            "flops_per_me": fl, "flops_source": "generator count of the emitted straight-line code (FMA = 2): "
-            f"{fl_detail['per_helicity']} per helicity x {ngood} good helicities + {fl_detail['per_event']} per event",
+            "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+            "traffic": (TRAFFIC_BYTES_PER_EVENT[process] * nevt if process in TRAFFIC_BYTES_PER_EVENT else None),
+            "traffic_note": "DRAM bytes per launch scaled from one ncu capture (profiles/); the path is FMA-bound, not HBM-bound",
+            "frac_per_helicity_accounting": (PER_HELICITY_ACCOUNTING[process] * nevt / (kernel_ms * 1e-3) * 1e-12 / peak
+                                             if process in PER_HELICITY_ACCOUNTING else None),
+            "flops_per_me": fl, "flops_source": "generator count of the operations this kernel executes (FMA = 2, "
+            f"DESIGN.md section 5): {fl_detail['per_helicity']} per helicity x {ngood} good helicities + {fl_detail['per_event']} per event",
             "peak_source": f"me_fma_peak({prec_peak}): register-resident FMA chain measured on this GPU in this run",
             "nominal_peak": 148 * (64 if prec_peak == "fp64" else 128) * 2 * 1.965e-3,
             "kernel_ms": kernel_ms,
@@ -274,17 +288,23 @@ def main():
                             "roofline_frac": ach / pk, "peak_tflops": pk, "clocks": clk2}
             m2.close()
         line["other_precisions"] = others
-        if a.sweep:
+        if sweep:
+            big = tuple(torch.from_numpy(x).to(dev) for x in (mom_all, gs_all, rh_all, rc_all)) + (
+                torch.empty(nmax, dtype=torch.float64, device=dev), torch.empty(nmax, dtype=torch.int32, device=dev),
+                torch.empty(nmax, dtype=torch.int32, device=dev))
             sw = {}
-            for prec in ("fp64", "fp32"):
+            for prec in ("fp64", "fp32", "mixed"):
+                m3 = MatrixElement(process, prec, device=local)
+                m3.set_good_helicities(mask)
                 for lg in range(14, 23):
                     n = 1 << lg
-                    if n > nevt:
-                        break
-                    m3, _, tot3, _, _, _ = bench_precision(prec, 3, 3, n)
-                    sw[f"{prec}:{n}"] = n / (tot3 / 3 * 1e-3)
-                    m3.close()
+                    b3 = tuple(x[:n] for x in big)
+                    tot3, per3 = time_device(torch, m3, b3, 5, 3)
+                    sw[f"{prec}:{n}"] = n / (float(np.median(per3)) * 1e-3)
+                m3.close()
             line["sweep_mes_per_s"] = sw
+            best = max((v, k) for k, v in sw.items() if k.startswith("fp64"))
+            line["sweep_best"] = {"fp64": best[1], "fp32": max((v, k) for k, v in sw.items() if k.startswith("fp32"))[1]}
         line["cpu_baseline"] = cpu_baseline(process)
     if rank == 0:
         print(json.dumps(line))
