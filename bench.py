@@ -156,7 +156,7 @@ def run_reference(a):
         return
     from oracle import oracle as O
     process = a.process
-    n0 = {"ee_mumu": 16384, "gg_tt": 16384, "gg_ttg": 4096, "gg_ttgg": 512, "gg_ttggg": 16}[process]
+    n0 = {"ee_mumu": 16384, "gg_tt": 16384, "gg_ttg": 16384, "gg_ttgg": 8192, "gg_ttggg": 64}[process]
     mom, gs, _, _ = make_inputs(process, n0, seed=1)
     mask = O.good_helicities(process, mom[: min(n0, 256)], gs[: min(n0, 256)])
     for _ in range(a.warmup):
@@ -171,7 +171,8 @@ def run_reference(a):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
         "warmup": a.warmup, "ms_per_step": 1e3 * dt / a.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": process, "events_per_step": n0, "precision": "fp64"},
+        "config": {"workload": process, "events_per_step_per_gpu": a.nevt, "precision": "fp64",
+                   "inputs": "seeded RAMBO sqrt(s)=1500 GeV, alpha_s~U[0.10,0.13]", "reference_events_per_step": n0},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
