@@ -136,68 +136,65 @@ struct GrpGeom {
   static constexpr int GS = ((RAW + 4 * UNIT - 1) / (4 * UNIT)) * (4 * UNIT) + UNIT;
 };
 
-template <class G, typename T, typename TC, int L>
-__device__ __forceinline__ void grp_tree_level(const GrpEvent<T, TC, G::n>& ev, T* slots, T* J, int r, bool active) {
-  constexpr int LPG = GrpGeom<G, T>::LPG, NV3 = L - 1, NV4 = (L - 1) * (L - 2) / 2, W = 2 + NV3 + NV4;
-  constexpr bool TOP = (L == G::n);
-  const unsigned* tab = G::level(L);
-  const int nt = G::ntask(L);
+// Colour-ordered gluon currents of one group, level by level (|seq| = 2 .. n).  One copy of the vertex code: the
+// levels, the tasks of a level and the terms of a task are run-time loops over the generated tables (keeps the
+// kernel small enough for the instruction cache; the loop bodies are ~100 FMA-pipe instructions each).
+template <class G, typename T, typename TC>
+__device__ __forceinline__ void grp_tree(const GrpEvent<T, TC, G::n>& ev, T* slots, T* J, int r, bool active) {
+  constexpr int LPG = GrpGeom<G, T>::LPG;
 #pragma unroll 1
-  for (int t0 = 0; t0 < nt; t0 += LPG) {
-    const int t = t0 + r;
-    if (active && t < nt) {
-      const unsigned* tw = tab + t * W;
-      const unsigned h0 = __ldg(tw);
-      vec4<T> acc = zero_vec4<T>();
+  for (int L = 2; L <= G::n; L++) {
+    const int NV3 = L - 1, NV4 = (L - 1) * (L - 2) / 2, W = 2 + NV3 + NV4;
+    const bool TOP = (L == G::n);
+    const unsigned* tab = G::level(L);
+    const int nt = G::ntask(L);
+#pragma unroll 1
+    for (int t0 = 0; t0 < nt; t0 += LPG) {
+      const int t = t0 + r;
+      if (active && t < nt) {
+        const unsigned* tw = tab + t * W;
+        const unsigned h0 = __ldg(tw);
+        vec4<T> acc = zero_vec4<T>();
+#pragma unroll 1
+        for (int j = 0; j < NV3; j++) {
+          const unsigned w = __ldg(tw + 2 + j);
+          const vec4<T> A = GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31);
+          const vec4<T> B = GrpVec<T>::ld(slots + ((w >> 8) & 255u) * 8, 0u);
+          v3_acc(acc, A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
+        }
+#pragma unroll 1
+        for (int j = 0; j < NV4; j++) {
+          const unsigned w = __ldg(tw + 2 + NV3 + j);
+          const vec4<T> A = GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31);
+          const vec4<T> B = GrpVec<T>::ld(slots + ((w >> 8) & 255u) * 8, 0u);
+          const vec4<T> C = GrpVec<T>::ld(slots + ((w >> 16) & 255u) * 8, 0u);
+          v4_acc(acc, A, B, C);
+        }
+        const T s = ev.ik[(h0 >> 8) & 31u];
 #pragma unroll
-      for (int j = 0; j < NV3; j++) {
-        const unsigned w = __ldg(tw + 2 + j);
-        const vec4<T> A = GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31);
-        const vec4<T> B = GrpVec<T>::ld(slots + ((w >> 8) & 255u) * 8, 0u);
-        v3_acc(acc, A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
-      }
+        for (int i = 0; i < 4; i++) acc.c[i] = s * acc.c[i];
+        if (!TOP) {
+          GrpVec<T>::st(slots + (h0 & 255u) * 8, acc);
+        } else {
+          // the full-length current is contracted at once with the four t-tbar currents: initial J of the flow
+          // and of its reverse
+          const unsigned h1 = __ldg(tw + 1);
+          T* ja = J + (h1 & 127u) * 8;
+          T* jb = J + ((h1 >> 8) & 127u) * 8;
+          const T sb = (h1 >> 31) ? T(-1) : T(1);
 #pragma unroll
-      for (int j = 0; j < NV4; j++) {
-        const unsigned w = __ldg(tw + 2 + NV3 + j);
-        const vec4<T> A = GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31);
-        const vec4<T> B = GrpVec<T>::ld(slots + ((w >> 8) & 255u) * 8, 0u);
-        const vec4<T> C = GrpVec<T>::ld(slots + ((w >> 16) & 255u) * 8, 0u);
-        v4_acc(acc, A, B, C);
-      }
-      const T s = ev.ik[(h0 >> 8) & 31u];
-#pragma unroll
-      for (int i = 0; i < 4; i++) acc.c[i] = s * acc.c[i];
-      if (!TOP) {
-        GrpVec<T>::st(slots + (h0 & 255u) * 8, acc);
-      } else {
-        const unsigned h1 = __ldg(tw + 1);
-        T* ja = J + (h1 & 127u) * 8;
-        T* jb = J + ((h1 >> 8) & 127u) * 8;
-        const T sb = (h1 >> 31) ? T(-1) : T(1);
-#pragma unroll
-        for (int v = 0; v < 4; v++) {
-          const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
-          const cx<T> a = mdot(q, acc);
-          ja[2 * v] = a.re; ja[2 * v + 1] = a.im;
-          jb[2 * v] = sb * a.re; jb[2 * v + 1] = sb * a.im;
+          for (int v = 0; v < 4; v++) {
+            const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
+            const cx<T> a = mdot(q, acc);
+            ja[2 * v] = a.re; ja[2 * v + 1] = a.im;
+            jb[2 * v] = sb * a.re; jb[2 * v + 1] = sb * a.im;
+          }
         }
       }
     }
+    __syncwarp();
   }
-  __syncwarp();
 }
-
-template <class G, typename T, typename TC, int L>
-struct GrpTree {
-  __device__ __forceinline__ static void run(const GrpEvent<T, TC, G::n>& ev, T* slots, T* J, int r, bool active) {
-    GrpTree<G, T, TC, L - 1>::run(ev, slots, J, r, active);
-    grp_tree_level<G, T, TC, L>(ev, slots, J, r, active);
-  }
-};
-template <class G, typename T, typename TC>
-struct GrpTree<G, T, TC, 1> {
-  __device__ __forceinline__ static void run(const GrpEvent<T, TC, G::n>&, T*, T*, int, bool) {}
-};
 
 // Quark-line walk of lane (s1, h_t): depth-first loop nest over the gluons that follow s1.  The words are read
 // in execution order from the role's stream (emit_group.py role_stream); psi[j] = Psi(path[:j]) stays in registers.
@@ -420,7 +417,7 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
     }
     __syncwarp();
     // ---- a3: colour-ordered gluon currents, level by level; the full-length ones initialise J
-    GrpTree<G, T, TC, N>::run(ev, slots, J, r, active);
+    grp_tree<G, T, TC>(ev, slots, J, r, active);
     // ---- a3-a5: quark line
     if (active) {
       GrpWalkCtx<G, T, TC> c;
