@@ -21,6 +21,31 @@
 
 namespace me {
 
+// Packed pair of floats: lane-local SIMD over the two t helicities of the quark-line walk in the fp32 build
+// (sm_100a FFMA2 / FMUL2 / FADD2: two fp32 operations per issued instruction; negation and the broadcast of a
+// scalar are operand modifiers, so make_float2(-x,-y) and make_float2(x,x) cost nothing).
+struct f2 {
+  float2 v;
+};
+__device__ __forceinline__ f2 mkf2(float x, float y) { f2 r; r.v = make_float2(x, y); return r; }
+__device__ __forceinline__ f2 operator+(f2 a, f2 b) { f2 r; r.v = __fadd2_rn(a.v, b.v); return r; }
+__device__ __forceinline__ f2 operator-(f2 a, f2 b) { f2 r; r.v = __fadd2_rn(a.v, make_float2(-b.v.x, -b.v.y)); return r; }
+__device__ __forceinline__ f2 operator-(f2 a) { return mkf2(-a.v.x, -a.v.y); }
+__device__ __forceinline__ f2 operator*(f2 a, f2 b) { f2 r; r.v = __fmul2_rn(a.v, b.v); return r; }
+__device__ __forceinline__ f2 fmad(f2 a, f2 b, f2 c) { f2 r; r.v = __ffma2_rn(a.v, b.v, c.v); return r; }
+
+// How the walk keeps the t helicities of a lane: NCH register chains of scalar type PS
+template <typename T, bool HTL> struct WalkPack {
+  typedef T PS;
+  static constexpr int NCH = HTL ? 2 : 1;
+  __device__ __forceinline__ static PS widen(T x) { return x; }
+};
+template <> struct WalkPack<float, true> {
+  typedef f2 PS;
+  static constexpr int NCH = 1;
+  __device__ __forceinline__ static PS widen(float x) { return mkf2(x, x); }
+};
+
 template <typename T, typename TC, int N>
 struct alignas(16) GrpEvent {
   double kd[N + 2][4];         // incoming-convention momenta (+p initial, -p final), fp64
@@ -207,70 +232,109 @@ struct GrpWalkCtx {
   int ht;
   __device__ __forceinline__ unsigned next() { return __ldg(stream++); }
   __device__ __forceinline__ vec4<T> cur(unsigned w) const { return GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31); }
-  // q and the denominator of the propagator after the gluons of word w (shared by both t helicities)
-  __device__ __forceinline__ void prop_data(unsigned w, mom4<T>& q, cx<T>& gd) const {
-    const unsigned m = (w >> 8) & 31u;
+  typedef WalkPack<T, GrpGeom<G, T>::HTL> WP;
+  typedef typename WP::PS PS;
+  __device__ __forceinline__ vec4<PS> curw(unsigned w) const {
+    const vec4<T> x = cur(w);
+    vec4<PS> r;
 #pragma unroll
-    for (int i = 0; i < 4; i++) q.c[i] = ev->qsub[m][i];
-    gd = mk<T>(ev->gd[m][0], ev->gd[m][1]);
+    for (int i = 0; i < 4; i++) r.c[i] = mk<PS>(WP::widen(x.c[i].re), WP::widen(x.c[i].im));
+    return r;
   }
-  __device__ __forceinline__ void leaf(const spin4<T>& X, unsigned w, int h) const {
-    T* j = J + ((w >> 16) & 127u) * 8 + h * 4;
+  // external spinor(s) ubar(t) of chain c
+  __device__ __forceinline__ spin4<PS> psi0(int c) const {
+    spin4<PS> r;
+    if constexpr (WP::NCH == 1 && GrpGeom<G, T>::HTL) {  // packed pair: (h_t = 0, h_t = 1)
+      const spin4<T> a = ld_spin<T>(ev->ub[0]), b = ld_spin<T>(ev->ub[1]);
+#pragma unroll
+      for (int i = 0; i < 4; i++) r.c[i] = mk<PS>(pack(a.c[i].re, b.c[i].re), pack(a.c[i].im, b.c[i].im));
+    } else {
+      const spin4<T> a = ld_spin<T>(ev->ub[GrpGeom<G, T>::HTL ? c : ht]);
+#pragma unroll
+      for (int i = 0; i < 4; i++) r.c[i] = mk<PS>(WP::widen(a.c[i].re), WP::widen(a.c[i].im));
+    }
+    return r;
+  }
+  __device__ __forceinline__ static f2 pack(float x, float y) { return mkf2(x, y); }
+  __device__ __forceinline__ static double pack(double x, double) { return x; }
+  // Psi = X (qslash + m) / (q^2 - m^2 + i m Gamma) after the gluons of word w; q, the denominator and m are shared
+  __device__ __forceinline__ static void addto(T* j, int h, int b, f2 re, f2 im) {
+    j[0 * 4 + 2 * b] += re.v.x; j[0 * 4 + 2 * b + 1] += im.v.x;
+    j[1 * 4 + 2 * b] += re.v.y; j[1 * 4 + 2 * b + 1] += im.v.y;
+  }
+  template <typename S> __device__ __forceinline__ static void addto(T* j, int h, int b, S re, S im) {
+    j[h * 4 + 2 * b] += re; j[h * 4 + 2 * b + 1] += im;
+  }
+  __device__ __forceinline__ void leaf(const spin4<PS> (&X)[WP::NCH], unsigned w) const {
+    T* j = J + ((w >> 16) & 127u) * 8;
 #pragma unroll
     for (int b = 0; b < 2; b++) {
-      const cx<T> a = row_col(X, ld_spin<T>(ev->v[b]));
-      j[2 * b] += a.re;
-      j[2 * b + 1] += a.im;
+      const spin4<T> vb = ld_spin<T>(ev->v[b]);
+      spin4<PS> vw;
+#pragma unroll
+      for (int i = 0; i < 4; i++) vw.c[i] = mk<PS>(WP::widen(vb.c[i].re), WP::widen(vb.c[i].im));
+#pragma unroll
+      for (int c = 0; c < WP::NCH; c++) {
+        const cx<PS> a = row_col(X[c], vw);
+        addto(j, GrpGeom<G, T>::HTL ? c : ht, b, a.re, a.im);
+      }
     }
   }
 };
 
-// node whose path holds D gluons; psi[h][0..D-1] are valid on entry (h runs over the NHT t helicities of the lane)
-template <class G, typename T, typename TC, int NHT, int D>
+// node whose path holds D gluons; psi[c][0..D-1] are valid on entry (c runs over the register chains of the lane)
+template <class G, typename T, typename TC, int D>
 struct GrpWalk {
-  __device__ __forceinline__ static void node(GrpWalkCtx<G, T, TC>& c, spin4<T> (&psi)[NHT][G::n]) {
+  typedef GrpWalkCtx<G, T, TC> Ctx;
+  typedef typename Ctx::PS PS;
+  static constexpr int NCH = Ctx::WP::NCH;
+  __device__ __forceinline__ static void node(Ctx& c, spin4<PS> (&psi)[NCH][G::n]) {
     const unsigned w0 = c.next();
-    spin4<T> X[NHT];
+    spin4<PS> X[NCH];
     {
-      const vec4<T> J0 = c.cur(w0);
+      const vec4<PS> J0 = c.curw(w0);
 #pragma unroll
-      for (int h = 0; h < NHT; h++) X[h] = row_slash(psi[h][0], J0);
+      for (int h = 0; h < NCH; h++) X[h] = row_slash(psi[h][0], J0);
     }
 #pragma unroll
     for (int j = 1; j < D; j++) {
-      const vec4<T> Jj = c.cur(c.next());
+      const vec4<PS> Jj = c.curw(c.next());
 #pragma unroll
-      for (int h = 0; h < NHT; h++) row_slash_add(X[h], psi[h][j], Jj);
+      for (int h = 0; h < NCH; h++) row_slash_add(X[h], psi[h][j], Jj);
     }
     {
-      mom4<T> q;
-      cx<T> gd;
-      c.prop_data(w0, q, gd);
+      const unsigned m = (w0 >> 8) & 31u;
+      mom4<PS> q;
 #pragma unroll
-      for (int h = 0; h < NHT; h++) psi[h][D] = row_prop(X[h], q, c.ev->mt, gd);
+      for (int i = 0; i < 4; i++) q.c[i] = Ctx::WP::widen(c.ev->qsub[m][i]);
+      const cx<PS> gd = mk<PS>(Ctx::WP::widen(c.ev->gd[m][0]), Ctx::WP::widen(c.ev->gd[m][1]));
+      const PS mt = Ctx::WP::widen(c.ev->mt);
+#pragma unroll
+      for (int h = 0; h < NCH; h++) psi[h][D] = row_prop(X[h], q, mt, gd);
     }
 #pragma unroll 1
-    for (int child = 0; child < G::n - D; child++) GrpWalk<G, T, TC, NHT, D + 1>::node(c, psi);
+    for (int child = 0; child < G::n - D; child++) GrpWalk<G, T, TC, D + 1>::node(c, psi);
   }
 };
-template <class G, typename T, typename TC, int NHT>
-struct GrpWalk<G, T, TC, NHT, G::n> {
-  __device__ __forceinline__ static void node(GrpWalkCtx<G, T, TC>& c, spin4<T> (&psi)[NHT][G::n]) {
-    spin4<T> X[NHT];
+template <class G, typename T, typename TC>
+struct GrpWalk<G, T, TC, G::n> {
+  typedef GrpWalkCtx<G, T, TC> Ctx;
+  typedef typename Ctx::PS PS;
+  static constexpr int NCH = Ctx::WP::NCH;
+  __device__ __forceinline__ static void node(Ctx& c, spin4<PS> (&psi)[NCH][G::n]) {
+    spin4<PS> X[NCH];
     {
-      const vec4<T> J1 = c.cur(c.next());
+      const vec4<PS> J1 = c.curw(c.next());
 #pragma unroll
-      for (int h = 0; h < NHT; h++) X[h] = row_slash(psi[h][1], J1);
+      for (int h = 0; h < NCH; h++) X[h] = row_slash(psi[h][1], J1);
     }
 #pragma unroll
     for (int j = 2; j < G::n; j++) {
-      const vec4<T> Jj = c.cur(c.next());
+      const vec4<PS> Jj = c.curw(c.next());
 #pragma unroll
-      for (int h = 0; h < NHT; h++) row_slash_add(X[h], psi[h][j], Jj);
+      for (int h = 0; h < NCH; h++) row_slash_add(X[h], psi[h][j], Jj);
     }
-    const unsigned w = c.next();
-#pragma unroll
-    for (int h = 0; h < NHT; h++) c.leaf(X[h], w, (NHT == 2) ? h : c.ht);
+    c.leaf(X, c.next());
   }
 };
 
@@ -424,10 +488,11 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
       c.ev = &ev; c.slots = slots; c.J = J;
       c.stream = G::role(GE::HTL ? r : (r >> 1));
       c.ht = GE::HTL ? 0 : (r & 1);
-      spin4<T> psi[GE::NHT][G::n];
+      typedef GrpWalkCtx<G, T, TC> Ctx;
+      spin4<typename Ctx::PS> psi[Ctx::WP::NCH][G::n];
 #pragma unroll
-      for (int h = 0; h < GE::NHT; h++) psi[h][0] = ld_spin<T>(ev.ub[GE::HTL ? h : c.ht]);
-      GrpWalk<G, T, TC, GE::NHT, 1>::node(c, psi);
+      for (int h = 0; h < Ctx::WP::NCH; h++) psi[h][0] = c.psi0(h);
+      GrpWalk<G, T, TC, 1>::node(c, psi);
     }
     __syncwarp();
     // ---- a6: colour sums, task = (variant, re/im): 8 per group, lane r takes tasks r, r + LPG, ...

@@ -44,15 +44,21 @@ template <typename T> ME_HD cx<T> mk(T re, T im) { cx<T> r; r.re = re; r.im = im
 template <typename T> ME_HD cx<T> operator+(cx<T> a, cx<T> b) { return mk<T>(a.re + b.re, a.im + b.im); }
 template <typename T> ME_HD cx<T> operator-(cx<T> a, cx<T> b) { return mk<T>(a.re - b.re, a.im - b.im); }
 template <typename T> ME_HD cx<T> operator-(cx<T> a) { return mk<T>(-a.re, -a.im); }
+// a*b + c as one operation of the scalar type (overloaded for the packed float pair of me_group.cuh)
+template <typename T> ME_HD T fmad(T a, T b, T c) { return a * b + c; }
 template <typename T> ME_HD cx<T> operator*(cx<T> a, cx<T> b) {
-  return mk<T>(a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re);
+  return mk<T>(fmad(a.re, b.re, (-a.im) * b.im), fmad(a.re, b.im, a.im * b.re));
 }
 template <typename T> ME_HD cx<T> operator*(T s, cx<T> a) { return mk<T>(s * a.re, s * a.im); }
 // a + b*c
 template <typename T> ME_HD cx<T> fma(cx<T> b, cx<T> c, cx<T> a) {
-  return mk<T>(a.re + b.re * c.re - b.im * c.im, a.im + b.re * c.im + b.im * c.re);
+  return mk<T>(fmad(-b.im, c.im, fmad(b.re, c.re, a.re)), fmad(b.im, c.re, fmad(b.re, c.im, a.im)));
 }
-template <typename T> ME_HD cx<T> fma(T s, cx<T> c, cx<T> a) { return mk<T>(a.re + s * c.re, a.im + s * c.im); }
+// a - b*c
+template <typename T> ME_HD cx<T> fnma(cx<T> b, cx<T> c, cx<T> a) {
+  return mk<T>(fmad(b.im, c.im, fmad(-b.re, c.re, a.re)), fmad(-b.im, c.re, fmad(-b.re, c.im, a.im)));
+}
+template <typename T> ME_HD cx<T> fma(T s, cx<T> c, cx<T> a) { return mk<T>(fmad(s, c.re, a.re), fmad(s, c.im, a.im)); }
 template <typename T> ME_HD cx<T> conj(cx<T> a) { return mk<T>(a.re, -a.im); }
 template <typename T> ME_HD T norm2(cx<T> a) { return a.re * a.re + a.im * a.im; }
 // i * a
@@ -264,8 +270,8 @@ template <typename T> ME_HD spin4<T> row_slash(const spin4<T>& R, const vec4<T>&
   spin4<T> o;
   o.c[0] = fma(R.c[3], jt, R.c[2] * jp);
   o.c[1] = fma(R.c[3], jm, R.c[2] * jtb);
-  o.c[2] = R.c[0] * jm - R.c[1] * jt;
-  o.c[3] = R.c[1] * jp - R.c[0] * jtb;
+  o.c[2] = fnma(R.c[1], jt, R.c[0] * jm);
+  o.c[3] = fnma(R.c[0], jtb, R.c[1] * jp);
   return o;
 }
 template <typename T> ME_HD spin4<T> row_slash_neg(const spin4<T>& R, const vec4<T>& J) {
@@ -281,8 +287,8 @@ template <typename T> ME_HD void row_slash_add(spin4<T>& X, const spin4<T>& R, c
   const cx<T> jtb = J.c[1] - times_i(J.c[2]);
   X.c[0] = fma(R.c[3], jt, fma(R.c[2], jp, X.c[0]));
   X.c[1] = fma(R.c[3], jm, fma(R.c[2], jtb, X.c[1]));
-  X.c[2] = fma(R.c[0], jm, X.c[2]) - R.c[1] * jt;
-  X.c[3] = fma(R.c[1], jp, X.c[3]) - R.c[0] * jtb;
+  X.c[2] = fnma(R.c[1], jt, fma(R.c[0], jm, X.c[2]));
+  X.c[3] = fnma(R.c[0], jtb, fma(R.c[1], jp, X.c[3]));
 }
 // X -= R * Jslash
 template <typename T> ME_HD void row_slash_sub(spin4<T>& X, const spin4<T>& R, const vec4<T>& J) {
@@ -301,8 +307,8 @@ template <typename T> ME_HD spin4<T> row_prop(const spin4<T>& X, mom4<T> q, T m,
   spin4<T> o;
   o.c[0] = fma(X.c[3], qt, fma(qp, X.c[2], m * X.c[0]));
   o.c[1] = fma(qm, X.c[3], fma(X.c[2], qtb, m * X.c[1]));
-  o.c[2] = fma(qm, X.c[0], m * X.c[2]) - X.c[1] * qt;
-  o.c[3] = fma(qp, X.c[1], m * X.c[3]) - X.c[0] * qtb;
+  o.c[2] = fnma(X.c[1], qt, fma(qm, X.c[0], m * X.c[2]));
+  o.c[3] = fnma(X.c[0], qtb, fma(qp, X.c[1], m * X.c[3]));
 #pragma unroll
   for (int i = 0; i < 4; i++) o.c[i] = o.c[i] * gd;
   return o;
