@@ -138,3 +138,47 @@ def test_product_does_not_import_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(root, f)).read()
                 assert "import oracle" not in txt and "from oracle" not in txt and "me_oracle" not in txt, f
+
+
+def test_group_layout_tables_are_consistent():
+    """Lane-group layout (codegen/emit_group.py): slots, level tables and per-role word streams."""
+    import itertools
+    from paper_2503_21935_b200.codegen import emit_group as EG
+    for n, nslot in ((4, 22), (5, 105)):
+        g = EG.Group("t", n)
+        assert g.nslot == nslot == sum(len(g.level_seqs[L]) for L in range(1, n))
+        # canonical sequences: one of each {seq, reversed seq}; the reflection sign is (-1)^(len+1)
+        for L in range(1, n + 1):
+            allseq = [s for c in itertools.combinations(range(n), L) for s in itertools.permutations(c)]
+            assert len(g.level_seqs[L]) * (1 if L == 1 else 2) == len(allseq)
+            for s in allseq:
+                can, sgn = EG.canonical(s)
+                assert can in g.level_seqs[L] and sgn == (1 if can == s else (-1) ** (L + 1))
+        # level tables: every operand slot was produced by a lower level; masks partition the task's set
+        for L in range(2, n + 1):
+            tab, nv3, nv4 = g.level_table(L), L - 1, (L - 1) * (L - 2) // 2
+            W = 2 + nv3 + nv4
+            assert len(tab) == W * len(g.level_seqs[L])
+            lower = {g.slot[s] for k in range(1, L) for s in g.level_seqs[k]}
+            for t, seq in enumerate(g.level_seqs[L]):
+                w = tab[t * W:(t + 1) * W]
+                assert (w[0] >> 8) & 31 == EG.mask_of(seq)
+                for x in w[2:2 + nv3]:
+                    assert (x & 255) in lower and ((x >> 8) & 255) in lower
+                    assert ((x >> 16) & 31) | ((x >> 21) & 31) == EG.mask_of(seq) and ((x >> 16) & 31) & ((x >> 21) & 31) == 0
+                for x in w[2 + nv3:]:
+                    assert {x & 255, (x >> 8) & 255, (x >> 16) & 255} <= lower
+        # top level: every flow is initialised exactly once (as a canonical sequence or as its reverse)
+        W = 2 + (n - 1) + (n - 1) * (n - 2) // 2
+        top = g.level_table(n)
+        flows = [f for t in range(len(g.level_seqs[n])) for f in (top[t * W + 1] & 127, (top[t * W + 1] >> 8) & 127)]
+        assert sorted(flows) == list(range(len(g.flows)))
+        # role streams: same length for every first gluon, every flow is a leaf of exactly one role
+        leaves = []
+        for s1 in range(n):
+            st = g.role_stream(s1)
+            assert len(st) == len(g.role_stream(0))
+            leaves += [(w >> 16) & 127 for w in st if (w >> 8) & 31 == (1 << n) - 1]
+        assert sorted(leaves) == list(range(len(g.flows)))
+        fl = g.flops()
+        assert fl["per_gluon_combination"] == fl["tree"] + fl["walk"] + fl["colour"]
