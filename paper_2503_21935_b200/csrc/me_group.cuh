@@ -495,26 +495,82 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
       GrpWalk<G, T, TC, 1>::node(c, psi);
     }
     __syncwarp();
-    // ---- a6: colour sums, task = (variant, re/im): 8 per group, lane r takes tasks r, r + LPG, ...
-#pragma unroll 1
-    for (int k0 = 0; k0 < 8; k0 += LPG) {
-      const int k = k0 + r;
-      TC q = TC(0);
+    // ---- a6: colour sums.  Helicity row of variant v = 2 h_t + h_tbar of this group:
+    auto hel_row = [&](int v) {
       int h = 0;
-      const bool on = active && k < 8;
-      if (on) {
-        const int v = k >> 1;
-        for (int i = 0; i < N; i++) {
-          const int p = (i < 2) ? i : i + 2;
-          h |= ((grp >> (N - 1 - i)) & 1) << (NPAR - 1 - p);
-        }
-        h |= (v >> 1) << (NPAR - 1 - 2);
-        h |= (v & 1) << (NPAR - 1 - 3);
-        const TC keep = ev.good[h] ? TC(1) : TC(0);
-        q = grp_quadform<G::ncol, T, TC, CM>(J, k, (MODE == MODE_SELECT) ? wloc : nullptr, keep);
+      for (int i = 0; i < N; i++) {
+        const int p = (i < 2) ? i : i + 2;
+        h |= ((grp >> (N - 1 - i)) & 1) << (NPAR - 1 - p);
       }
-      q += __shfl_xor_sync(0xffffffffu, q, 1);
-      if (on && !(k & 1)) ev.mh[h] = (double)q;
+      h |= (v >> 1) << (NPAR - 1 - 2);
+      h |= (v & 1) << (NPAR - 1 - 3);
+      return h;
+    };
+    if constexpr (G::ncol > 24) {
+      // rows of C split over the lanes of the group; every C_ab read once feeds the 8 real vectors
+      // (4 variants x re/im) of the group; partial sums meet in the (now free) current slots
+      TC part[8];
+#pragma unroll
+      for (int k = 0; k < 8; k++) part[k] = TC(0);
+      if (active) {
+        TC keep[4];
+#pragma unroll
+        for (int v = 0; v < 4; v++) keep[v] = ev.good[hel_row(v)] ? TC(1) : TC(0);
+#pragma unroll 1
+        for (int a = r; a < G::ncol; a += LPG) {
+          const vec4<T> ja = GrpVec<T>::ld(J + a * 8, 0u);
+          TC xa[8], y[8];
+#pragma unroll
+          for (int k = 0; k < 4; k++) { xa[2 * k] = TC(ja.c[k].re); xa[2 * k + 1] = TC(ja.c[k].im); }
+          const TC caa = TC(0.5) * CM::at(a * G::ncol + a);
+#pragma unroll
+          for (int k = 0; k < 8; k++) y[k] = caa * xa[k];
+#pragma unroll 4
+          for (int b = a + 1; b < G::ncol; b++) {
+            const TC c = CM::at(a * G::ncol + b);
+            const vec4<T> jb = GrpVec<T>::ld(J + b * 8, 0u);
+#pragma unroll
+            for (int k = 0; k < 4; k++) { y[2 * k] += c * TC(jb.c[k].re); y[2 * k + 1] += c * TC(jb.c[k].im); }
+          }
+#pragma unroll
+          for (int k = 0; k < 8; k++) part[k] += xa[k] * y[k];
+          if (MODE == MODE_SELECT) {
+            TC w = TC(0);
+#pragma unroll
+            for (int v = 0; v < 4; v++) w += keep[v] * (xa[2 * v] * xa[2 * v] + xa[2 * v + 1] * xa[2 * v + 1]);
+            wloc[a] += w;
+          }
+        }
+      }
+      __syncwarp();  // every lane of the group is done with the current slots
+      if (active) {
+        vec4<T> pv;
+#pragma unroll
+        for (int k = 0; k < 4; k++) pv.c[k] = mk<T>(T(part[2 * k]), T(part[2 * k + 1]));
+        GrpVec<T>::st(slots + r * 8, pv);
+      }
+      __syncwarp();
+      if (active && r < 4) {
+        double q = 0.0;
+        for (int l = 0; l < LPG; l++) q += (double)slots[l * 8 + 2 * r] + (double)slots[l * 8 + 2 * r + 1];
+        ev.mh[hel_row(r)] = 2.0 * q;
+      }
+    } else {
+      // task = (variant, re/im): 8 per group, lane r takes tasks r, r + LPG, ...; pairs are added by one shuffle
+#pragma unroll 1
+      for (int k0 = 0; k0 < 8; k0 += LPG) {
+        const int k = k0 + r;
+        TC q = TC(0);
+        int h = 0;
+        const bool on = active && k < 8;
+        if (on) {
+          h = hel_row(k >> 1);
+          const TC keep = ev.good[h] ? TC(1) : TC(0);
+          q = grp_quadform<G::ncol, T, TC, CM>(J, k, (MODE == MODE_SELECT) ? wloc : nullptr, keep);
+        }
+        q += __shfl_xor_sync(0xffffffffu, q, 1);
+        if (on && !(k & 1)) ev.mh[h] = (double)q;
+      }
     }
     __syncwarp();
     }  // passes
