@@ -114,6 +114,56 @@ template <typename T> __device__ __forceinline__ spin4<T> ld_spin(const T* p) {
   return r;
 }
 
+// Current slots (8 T = 64 or 32 bytes each) are stored with their 16-byte chunks permuted by the slot index
+// (chunk i of slot s sits at position i ^ x(s)), so that the slots the lanes of a quarter-warp read together fall
+// into different bank groups: without it a 64-byte slot stride reaches only half of the banks for a given chunk.
+template <typename T> struct GrpSlot;
+template <> struct GrpSlot<double> {
+  __device__ __forceinline__ static vec4<double> ld(const double* slots, unsigned s, unsigned neg) {
+    const char* base = reinterpret_cast<const char*>(slots + s * 8);
+    const unsigned x = (s >> 1) & 3u;
+    const int m = (int)(neg << 31);
+    vec4<double> r;
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      const double2 v = *reinterpret_cast<const double2*>(base + ((i ^ x) << 4));
+      r.c[i].re = __hiloint2double(__double2hiint(v.x) ^ m, __double2loint(v.x));
+      r.c[i].im = __hiloint2double(__double2hiint(v.y) ^ m, __double2loint(v.y));
+    }
+    return r;
+  }
+  __device__ __forceinline__ static void st(double* slots, unsigned s, const vec4<double>& a) {
+    char* base = reinterpret_cast<char*>(slots + s * 8);
+    const unsigned x = (s >> 1) & 3u;
+#pragma unroll
+    for (int i = 0; i < 4; i++) *reinterpret_cast<double2*>(base + ((i ^ x) << 4)) = make_double2(a.c[i].re, a.c[i].im);
+  }
+};
+template <> struct GrpSlot<float> {
+  __device__ __forceinline__ static vec4<float> ld(const float* slots, unsigned s, unsigned neg) {
+    const char* base = reinterpret_cast<const char*>(slots + s * 8);
+    const unsigned x = 0u;  // fp32: the extra address arithmetic costs more issue slots than the conflicts (measured)
+    const int m = (int)(neg << 31);
+    vec4<float> r;
+#pragma unroll
+    for (int i = 0; i < 2; i++) {
+      const float4 v = *reinterpret_cast<const float4*>(base + ((i ^ x) << 4));
+      r.c[2 * i].re = __int_as_float(__float_as_int(v.x) ^ m);
+      r.c[2 * i].im = __int_as_float(__float_as_int(v.y) ^ m);
+      r.c[2 * i + 1].re = __int_as_float(__float_as_int(v.z) ^ m);
+      r.c[2 * i + 1].im = __int_as_float(__float_as_int(v.w) ^ m);
+    }
+    return r;
+  }
+  __device__ __forceinline__ static void st(float* slots, unsigned s, const vec4<float>& a) {
+    char* base = reinterpret_cast<char*>(slots + s * 8);
+    const unsigned x = 0u;
+#pragma unroll
+    for (int i = 0; i < 2; i++)
+      *reinterpret_cast<float4*>(base + ((i ^ x) << 4)) = make_float4(a.c[2 * i].re, a.c[2 * i].im, a.c[2 * i + 1].re, a.c[2 * i + 1].im);
+  }
+};
+
 // acc += (A.B)(kA-kB) + ((kA+2kB).A) B - ((2kA+kB).B) A      (three-gluon vertex, propagator applied later)
 template <typename T>
 __device__ __forceinline__ void v3_acc(vec4<T>& acc, const vec4<T>& A, const vec4<T>& B, const T* kA, const T* kB) {
@@ -183,23 +233,23 @@ __device__ __forceinline__ void grp_tree(const GrpEvent<T, TC, G::n>& ev, T* slo
 #pragma unroll 1
         for (int j = 0; j < NV3; j++) {
           const unsigned w = __ldg(tw + 2 + j);
-          const vec4<T> A = GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31);
-          const vec4<T> B = GrpVec<T>::ld(slots + ((w >> 8) & 255u) * 8, 0u);
+          const vec4<T> A = GrpSlot<T>::ld(slots, w & 255u, w >> 31);
+          const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
           v3_acc(acc, A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
         }
 #pragma unroll 1
         for (int j = 0; j < NV4; j++) {
           const unsigned w = __ldg(tw + 2 + NV3 + j);
-          const vec4<T> A = GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31);
-          const vec4<T> B = GrpVec<T>::ld(slots + ((w >> 8) & 255u) * 8, 0u);
-          const vec4<T> C = GrpVec<T>::ld(slots + ((w >> 16) & 255u) * 8, 0u);
+          const vec4<T> A = GrpSlot<T>::ld(slots, w & 255u, w >> 31);
+          const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
+          const vec4<T> C = GrpSlot<T>::ld(slots, (w >> 16) & 255u, 0u);
           v4_acc(acc, A, B, C);
         }
         const T s = ev.ik[(h0 >> 8) & 31u];
 #pragma unroll
         for (int i = 0; i < 4; i++) acc.c[i] = s * acc.c[i];
         if (!TOP) {
-          GrpVec<T>::st(slots + (h0 & 255u) * 8, acc);
+          GrpSlot<T>::st(slots, h0 & 255u, acc);
         } else {
           // the full-length current is contracted at once with the four t-tbar currents: initial J of the flow
           // and of its reverse
@@ -231,7 +281,7 @@ struct GrpWalkCtx {
   const unsigned* stream;
   int ht;
   __device__ __forceinline__ unsigned next() { return __ldg(stream++); }
-  __device__ __forceinline__ vec4<T> cur(unsigned w) const { return GrpVec<T>::ld(slots + (w & 255u) * 8, w >> 31); }
+  __device__ __forceinline__ vec4<T> cur(unsigned w) const { return GrpSlot<T>::ld(slots, w & 255u, w >> 31); }
   typedef WalkPack<T, GrpGeom<G, T>::HTL> WP;
   typedef typename WP::PS PS;
   __device__ __forceinline__ vec4<PS> curw(unsigned w) const {
@@ -477,7 +527,7 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
       const int lam = ((grp >> (N - 1 - r)) & 1) ? 1 : -1;
       polbasis<T> pb;
       for (int c = 0; c < 3; c++) { pb.e1[c] = ev.pol[r][c]; pb.e2[c] = ev.pol[r][3 + c]; }
-      GrpVec<T>::st(slots + r * 8, polvec(pb, lam, p >= 2));
+      GrpSlot<T>::st(slots, r, polvec(pb, lam, p >= 2));
     }
     __syncwarp();
     // ---- a3: colour-ordered gluon currents, level by level; the full-length ones initialise J
