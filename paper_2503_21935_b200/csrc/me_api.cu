@@ -293,6 +293,8 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
   memset(&a, 0, sizeof(a));
   a.mom = d_momenta; a.gs = d_gs; a.rndhel = d_rndhel; a.rndcol = d_rndcol; a.nevt = nevt;
   a.me = d_me; a.selhel = d_selhel; a.selcol = d_selcol; a.par = h->par; a.good = h->good;
+  a.good.mask[0] = a.good.mask[1] = 0ull;
+  for (int i = 0; i < a.good.n; i++) a.good.mask[a.good.h[i] >> 6] |= 1ull << (a.good.h[i] & 63);
   const int mode = (d_selhel || d_selcol) ? me::MODE_SELECT : me::MODE_ME;
   launch_fn fn = h->proc->fn[h->precision];
   me::LaunchInfo info;

@@ -48,8 +48,6 @@ template <> struct WalkPack<float, true> {
 
 template <typename T, typename TC, int N>
 struct alignas(16) GrpEvent {
-  double kd[N + 2][4];         // incoming-convention momenta (+p initial, -p final), fp64
-  double d2[N + 2][N + 2];     // 2 k_i.k_j, i < j
   double mh[1 << (N + 2)];     // |M_h|^2 (colour-summed, un-normalised) per helicity row
   alignas(16) T Ksub[1 << N][4];           // sum of the gluon momenta of a subset (bit i = gluon i)
   alignas(16) T qsub[1 << N][4];           // -(k_t + K_S): momentum of the quark line after the gluons of S
@@ -61,7 +59,6 @@ struct alignas(16) GrpEvent {
   T pol[N][6];
   T mt;
   TC wc[5][(N == 4) ? 24 : (N == 5 ? 120 : 6)];  // per-warp colour weights (at most 4 warps per block)
-  unsigned char good[1 << (N + 2)];
 };
 
 template <typename T> struct GrpVec;
@@ -417,6 +414,35 @@ __device__ __forceinline__ TC grp_quadform(const T* J, int off, TC* x2 /*[NCOL] 
   return TC(2) * s;
 }
 
+// One warp: in-order cumulative sums of PER consecutive values per lane (index = lane * PER + i; val = 0 where
+// !ok), their total, and the selection of reading R11: first index with rnd * total < cumulative sum, else the last
+// ok index.  Every lane returns the same total and sel.
+template <int PER>
+__device__ __forceinline__ void grp_warp_select(const double (&val)[PER], const bool (&ok)[PER], double rnd, int lane,
+                                                double& total, int& sel) {
+  double pre[PER], run = 0.0;
+#pragma unroll
+  for (int i = 0; i < PER; i++) { run += val[i]; pre[i] = run; }
+  double inc = run;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const double t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  const double off = inc - run;
+  total = __shfl_sync(0xffffffffu, inc, 31);
+  const double target = rnd * total;
+  int hit = -1, lastok = -1;
+#pragma unroll
+  for (int i = 0; i < PER; i++) {
+    if (hit < 0 && ok[i] && target < off + pre[i]) hit = lane * PER + i;
+    if (ok[i]) lastok = lane * PER + i;
+  }
+  const unsigned bh = __ballot_sync(0xffffffffu, hit >= 0), bo = __ballot_sync(0xffffffffu, lastok >= 0);
+  if (bh) sel = __shfl_sync(0xffffffffu, hit, __ffs(bh) - 1);
+  else sel = bo ? __shfl_sync(0xffffffffu, lastok, 31 - __clz(bo)) : 0;
+}
+
 template <class G, typename T, typename TC, class CM, int MODE, int MINB>
 __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const LaunchArgs a) {
   typedef GrpGeom<G, T> GE;
@@ -434,83 +460,73 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
 
   for (long long e = blockIdx.x; e < a.nevt; e += gridDim.x) {
     __syncthreads();
-    // ---- a1: load, incoming convention
-    for (int i = tid; i < NPAR * 4; i += NT) {
-      const double x = a.mom[e * (NPAR * 4) + i];
-      ev.kd[i >> 2][i & 3] = (i < 8) ? x : -x;
-    }
-    if (MODE == MODE_FILTER) {
-      for (int i = tid; i < NCOMB; i += NT) ev.good[i] = 1;
-    } else {
-      for (int i = tid; i < NCOMB; i += NT) ev.good[i] = 0;
-    }
+    // ---- a1 + per-event, helicity-independent data (a2 bases, invariants in fp64) in ONE phase: every task reads
+    // the momenta it needs from global memory (L1-resident after the first touch; incoming convention: +p for the
+    // initial, -p for the final state), so no task waits for another and one block barrier ends the setup
+    const double* pm = a.mom + e * (NPAR * 4);
+    auto kd = [&](int p, int c) { const double x = __ldg(pm + 4 * p + c); return (p < 2) ? x : -x; };
+    auto dot2 = [&](int p, int q) {  // 2 k_p . k_q
+      return 2.0 * (kd(p, 0) * kd(q, 0) - kd(p, 1) * kd(q, 1) - kd(p, 2) * kd(q, 2) - kd(p, 3) * kd(q, 3));
+    };
     if (tid == 0) ev.mt = T(a.par.mt);
-    __syncthreads();
-    if (MODE != MODE_FILTER)
-      for (int i = tid; i < a.good.n; i += NT) ev.good[a.good.h[i]] = 1;
-    // ---- per-event, helicity-independent data (a2 bases, invariants in fp64)
-    for (int task = tid; task < NPAR * NPAR + (1 << N) + N + 2; task += NT) {
-      if (task < NPAR * NPAR) {
-        const int i = task / NPAR, j = task - i * NPAR;
-        if (i < j)
-          ev.d2[i][j] = 2.0 * (ev.kd[i][0] * ev.kd[j][0] - ev.kd[i][1] * ev.kd[j][1] - ev.kd[i][2] * ev.kd[j][2] -
-                               ev.kd[i][3] * ev.kd[j][3]);
-      } else if (task < NPAR * NPAR + (1 << N)) {
-        const int m = task - NPAR * NPAR;
-        double k[4] = {0.0, 0.0, 0.0, 0.0};
-        for (int i = 0; i < N; i++)
-          if ((m >> i) & 1) {
-            const int p = (i < 2) ? i : i + 2;
-            for (int c = 0; c < 4; c++) k[c] += ev.kd[p][c];
-          }
-        for (int c = 0; c < 4; c++) {
-          ev.Ksub[m][c] = T(k[c]);
-          ev.qsub[m][c] = T(-(ev.kd[2][c] + k[c]));
-        }
-      } else if (task < NPAR * NPAR + (1 << N) + N) {
-        const int i = task - NPAR * NPAR - (1 << N), p = (i < 2) ? i : i + 2;
-        mom4<T> k;
-        for (int c = 0; c < 4; c++) k.c[c] = T(ev.kd[p][c]);
-        const polbasis<T> pb = make_polbasis<T>((p < 2) ? k : neg(k));
-        for (int c = 0; c < 3; c++) { ev.pol[i][c] = pb.e1[c]; ev.pol[i][3 + c] = pb.e2[c]; }
-      } else {
-        const int which = task - NPAR * NPAR - (1 << N) - N;  // 0: t, 1: tbar
-        mom4<T> k;
-        for (int c = 0; c < 4; c++) k.c[c] = T(-ev.kd[2 + which][c]);
-        const spinbasis<T> sb = make_spinbasis<T>(k, T(a.par.mt));
-        for (int l = 0; l < 2; l++) {
-          const spin4<T> s = which ? spinor_v(sb, l ? 1 : -1) : bar(spinor_u(sb, l ? 1 : -1));
-          T* o = which ? ev.v[l] : ev.ub[l];
-          for (int c = 0; c < 4; c++) { o[2 * c] = s.c[c].re; o[2 * c + 1] = s.c[c].im; }
-        }
-      }
-    }
-    __syncthreads();
-    for (int task = tid; task < (1 << N) + 4; task += NT) {
+    for (int task = tid; task < (1 << N) + N + 2 + 4; task += NT) {
       if (task < (1 << N)) {
+        // gluon subset m: momentum sum, quark-line momentum after it, 1/K^2, quark-line denominator
         const int m = task;
-        double pairs = 0.0, line = 0.0;
+        double k[4] = {0.0, 0.0, 0.0, 0.0}, pairs = 0.0, line = 0.0;
         int cnt = 0;
         for (int i = 0; i < N; i++)
           if ((m >> i) & 1) {
             const int pi = (i < 2) ? i : i + 2;
             cnt++;
-            line += (pi < 2) ? ev.d2[pi][2] : ev.d2[2][pi];
+            for (int c = 0; c < 4; c++) k[c] += kd(pi, c);
+            line += dot2(2, pi);
             for (int j = i + 1; j < N; j++)
-              if ((m >> j) & 1) pairs += ev.d2[pi][(j < 2) ? j : j + 2];
+              if ((m >> j) & 1) pairs += dot2(pi, (j < 2) ? j : j + 2);
           }
+        for (int c = 0; c < 4; c++) {
+          ev.Ksub[m][c] = T(k[c]);
+          ev.qsub[m][c] = T(-(kd(2, c) + k[c]));
+        }
         ev.ik[m] = (cnt >= 2) ? T(1.0 / pairs) : T(0);
         const double den = line + pairs, nrm = 1.0 / (den * den + mw * mw);
         ev.gd[m][0] = (cnt >= 1) ? T(den * nrm) : T(0);
         ev.gd[m][1] = (cnt >= 1) ? T(-mw * nrm) : T(0);
+      } else if (task < (1 << N) + N) {
+        const int i = task - (1 << N), p = (i < 2) ? i : i + 2;
+        mom4<T> k;
+        for (int c = 0; c < 4; c++) k.c[c] = T(kd(p, c));
+        const polbasis<T> pb = make_polbasis<T>((p < 2) ? k : neg(k));
+        for (int c = 0; c < 3; c++) { ev.pol[i][c] = pb.e1[c]; ev.pol[i][3 + c] = pb.e2[c]; }
       } else {
-        const int v = task - (1 << N);
-        vec4<T> JR, JL;
-        chiral_currents(ld_spin<T>(ev.ub[v >> 1]), ld_spin<T>(ev.v[v & 1]), JR, JL);
-        for (int c = 0; c < 4; c++) { ev.Q[v][2 * c] = JR.c[c].re + JL.c[c].re; ev.Q[v][2 * c + 1] = JR.c[c].im + JL.c[c].im; }
+        // tasks 0,1: ubar(t), v(tbar) for both helicities; tasks 2..5: Q(h_t, h_tbar) = ubar gamma^mu v
+        const int w = task - (1 << N) - N;
+        spin4<T> ub[2], vv[2];
+        for (int which = 0; which < 2; which++) {
+          mom4<T> k;
+          for (int c = 0; c < 4; c++) k.c[c] = T(-kd(2 + which, c));
+          const spinbasis<T> sb = make_spinbasis<T>(k, T(a.par.mt));
+          for (int l = 0; l < 2; l++) {
+            if (which) vv[l] = spinor_v(sb, l ? 1 : -1);
+            else ub[l] = bar(spinor_u(sb, l ? 1 : -1));
+          }
+        }
+        if (w < 2) {
+          for (int l = 0; l < 2; l++) {
+            const spin4<T>& sp = w ? vv[l] : ub[l];
+            T* o = w ? ev.v[l] : ev.ub[l];
+            for (int c = 0; c < 4; c++) { o[2 * c] = sp.c[c].re; o[2 * c + 1] = sp.c[c].im; }
+          }
+        } else {
+          const int v = w - 2;
+          vec4<T> JR, JL;
+          chiral_currents((v >> 1) ? ub[1] : ub[0], (v & 1) ? vv[1] : vv[0], JR, JL);
+          for (int c = 0; c < 4; c++) { ev.Q[v][2 * c] = JR.c[c].re + JL.c[c].re; ev.Q[v][2 * c + 1] = JR.c[c].im + JL.c[c].im; }
+        }
       }
     }
     __syncthreads();
+    auto is_good = [&](int h) { return MODE == MODE_FILTER || ((a.good.mask[h >> 6] >> (h & 63)) & 1ull) != 0ull; };
 
     TC wloc[(MODE == MODE_SELECT) ? G::ncol : 1];
     if (MODE == MODE_SELECT) {
@@ -565,7 +581,7 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
       if (active) {
         TC keep[4];
 #pragma unroll
-        for (int v = 0; v < 4; v++) keep[v] = ev.good[hel_row(v)] ? TC(1) : TC(0);
+        for (int v = 0; v < 4; v++) keep[v] = is_good(hel_row(v)) ? TC(1) : TC(0);
 #pragma unroll 1
         for (int a = r; a < G::ncol; a += LPG) {
           const vec4<T> ja = GrpVec<T>::ld(J + a * 8, 0u);
@@ -615,7 +631,7 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
         const bool on = active && k < 8;
         if (on) {
           h = hel_row(k >> 1);
-          const TC keep = ev.good[h] ? TC(1) : TC(0);
+          const TC keep = is_good(h) ? TC(1) : TC(0);
           q = grp_quadform<G::ncol, T, TC, CM>(J, k, (MODE == MODE_SELECT) ? wloc : nullptr, keep);
         }
         q += __shfl_xor_sync(0xffffffffu, q, 1);
@@ -642,37 +658,42 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
         const double f = (total > 0.0) ? ev.mh[h] / total : 0.0;
         atomicMax(a.fracmax + h, (unsigned long long)__double_as_longlong(f));
       }
-    } else if (tid == 0) {
-      double total = 0.0;
-      for (int ih = 0; ih < a.good.n; ih++) total += ev.mh[a.good.h[ih]];
-      const double g = a.gs[e];
-      a.me[e] = total * ipow<2 * N>(g) * (1.0 / (double(G::denom) * double(G::cden)));
-      if (MODE == MODE_SELECT && a.selhel) {
-        const double target = a.rndhel[e] * total;
-        int sel = a.good.h[a.good.n - 1];
-        double run = 0.0;
-        for (int ih = 0; ih < a.good.n; ih++) {
-          run += ev.mh[a.good.h[ih]];
-          if (target < run) { sel = a.good.h[ih]; break; }
-        }
-        a.selhel[e] = sel;
+    } else if (warp == 0) {
+      // helicity sum in table order (a7), ME (a9) and helicity selection (a8): one warp, in-order scan
+      constexpr int PER = NCOMB / 32;
+      double val[PER];
+      bool ok[PER];
+#pragma unroll
+      for (int i = 0; i < PER; i++) {
+        const int h = lane * PER + i;
+        ok[i] = is_good(h);
+        val[i] = ok[i] ? ev.mh[h] : 0.0;
       }
-    } else if (tid == 32 && MODE == MODE_SELECT && a.selcol) {
-      double tot = 0.0;
-      for (int c = 0; c < G::ncol; c++) {
+      double total;
+      int sel;
+      grp_warp_select<PER>(val, ok, (MODE == MODE_SELECT && a.selhel) ? a.rndhel[e] : 0.0, lane, total, sel);
+      if (lane == 0) {
+        const double g = a.gs[e];
+        a.me[e] = total * ipow<2 * N>(g) * (1.0 / (double(G::denom) * double(G::cden)));
+        if (MODE == MODE_SELECT && a.selhel) a.selhel[e] = sel;
+      }
+    } else if (warp == 1 && MODE == MODE_SELECT && a.selcol) {
+      constexpr int PER = (G::ncol + 31) / 32;
+      double val[PER];
+      bool ok[PER];
+#pragma unroll
+      for (int i = 0; i < PER; i++) {
+        const int c = lane * PER + i;
+        ok[i] = c < G::ncol;
         TC w = TC(0);
-        for (int k = 0; k < GE::NW; k++) w += ev.wc[k][c];
-        ev.wc[0][c] = w;
-        tot += (double)w;
+        if (ok[i])
+          for (int k = 0; k < GE::NW; k++) w += ev.wc[k][c];
+        val[i] = (double)w;
       }
-      const double target = a.rndcol[e] * tot;
-      int sel = G::ncol - 1;
-      double run = 0.0;
-      for (int c = 0; c < G::ncol; c++) {
-        run += (double)ev.wc[0][c];
-        if (target < run) { sel = c; break; }
-      }
-      a.selcol[e] = sel;
+      double total;
+      int sel;
+      grp_warp_select<PER>(val, ok, a.rndcol[e], lane, total, sel);
+      if (lane == 0) a.selcol[e] = sel;
     }
   }
 }

@@ -16,7 +16,8 @@ namespace me {
 
 struct GoodList {
   int n;
-  uint8_t h[128];
+  uint8_t h[128];               // good helicity rows in increasing order
+  unsigned long long mask[2];   // the same as a bit mask (bit h of mask[h >> 6])
 };
 
 struct LaunchArgs {
