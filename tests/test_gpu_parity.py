@@ -187,3 +187,51 @@ def test_physics_invariants_on_gpu(torch_cuda):
             c = m.compute(torch.from_numpy(sw).cuda(), g1)[0].cpu().numpy()
             assert np.max(np.abs(c - a) / a) < 1e-10
         m.close()
+
+
+@pytest.mark.parametrize("process", ["gg_ttg", "gg_ttgg", "gg_ttggg"])
+def test_partial_helicity_mask_matches_oracle(torch_cuda, process):
+    """An imported good-helicity mask that drops helicities (me_set_good_helicities): ME, helicity and colour
+    selections are those of the oracle with the same mask (both kernel layouts)."""
+    torch = torch_cuda
+    from oracle import oracle as O
+    from paper_2503_21935_b200.me import MatrixElement
+    case = oracle_case(process)
+    n = {"gg_ttg": 1000, "gg_ttgg": 333, "gg_ttggg": 45}[process]
+    mom, gs, rh, rc = case["mom"][:n], case["gs"][:n], case["rh"][:n], case["rc"][:n]
+    ncomb = len(case["mask"])
+    mask = (np.arange(ncomb) % 3 != 1).astype(np.uint8)  # drops a third of the rows, keeps the last one or not
+    mask[-1] = 0
+    ref = O.select(process, mom, gs, rh, rc, mask=mask)
+    m = MatrixElement(process, "fp64")
+    m.set_good_helicities(mask)
+    me, sh, sc = m.compute(torch.from_numpy(mom).cuda(), torch.from_numpy(gs).cuda(), torch.from_numpy(rh).cuda(),
+                           torch.from_numpy(rc).cuda())
+    torch.cuda.synchronize()
+    me, sh, sc = me.cpu().numpy(), sh.cpu().numpy(), sc.cpu().numpy()
+    assert np.max(np.abs(me - ref["me"]) / ref["me"]) <= 1e-10
+    assert np.all(mask[sh] == 1)
+    _check_selection(sh, ref["selhel"], ref["cumhel"], rh, 1e-9)
+    _check_selection(sc, ref["selcol"], ref["cumcol"], rc, 1e-9)
+    m.close()
+
+
+def test_group_kernel_edge_batches(torch_cuda):
+    """gg_ttgg (lane-group kernel): empty, single-event and ragged batches, host-buffer path."""
+    torch = torch_cuda
+    from paper_2503_21935_b200.me import MatrixElement
+    case = oracle_case("gg_ttgg")
+    m = MatrixElement("gg_ttgg", "fp64")
+    mom = torch.from_numpy(case["mom"]).cuda()
+    gs = torch.from_numpy(case["gs"]).cuda()
+    m.filter_helicities(mom, gs)
+    me, _, _ = m.compute(mom[:0], gs[:0])
+    assert me.shape == (0,)
+    for n in (1, 2, 65):
+        me, _, _ = m.compute(mom[:n].contiguous(), gs[:n].contiguous())
+        torch.cuda.synchronize()
+        assert np.allclose(me.cpu().numpy(), case["sel"]["me"][:n], rtol=1e-10, atol=0)
+    me_h, sh, sc = m.compute_host(case["mom"], case["gs"], case["rh"], case["rc"])
+    assert np.allclose(me_h, case["sel"]["me"], rtol=1e-10, atol=0)
+    assert np.mean(sh == case["sel"]["selhel"]) > 0.999 and np.mean(sc == case["sel"]["selcol"]) > 0.999
+    m.close()
