@@ -192,15 +192,91 @@ __device__ __forceinline__ void v4_acc(vec4<T>& acc, const vec4<T>& A, const vec
   }
 }
 
+// fp32 build: the same two vertices with every complex number as one packed f32x2 register pair (re, im): a complex
+// multiply-add is two FFMA2 (the second with the operand halves swapped and one sign flipped, both operand
+// modifiers on sm_100a) instead of four FFMA.
+__device__ __forceinline__ float2 pk(const cx<float>& a) { return make_float2(a.re, a.im); }
+__device__ __forceinline__ float2 cmul2(float2 a, float2 b) {  // a * b
+  const float2 t = __fmul2_rn(make_float2(a.x, a.x), b);
+  return __ffma2_rn(make_float2(-a.y, a.y), make_float2(b.y, b.x), t);
+}
+__device__ __forceinline__ float2 cmac2(float2 acc, float2 a, float2 b) {  // acc + a * b
+  acc = __ffma2_rn(make_float2(a.x, a.x), b, acc);
+  return __ffma2_rn(make_float2(-a.y, a.y), make_float2(b.y, b.x), acc);
+}
+__device__ __forceinline__ float2 cmsc2(float2 acc, float2 a, float2 b) {  // acc - a * b
+  acc = __ffma2_rn(make_float2(-a.x, -a.x), b, acc);
+  return __ffma2_rn(make_float2(a.y, -a.y), make_float2(b.y, b.x), acc);
+}
+__device__ __forceinline__ float2 rmac2(float2 acc, float s, float2 b) { return __ffma2_rn(make_float2(s, s), b, acc); }
+// Minkowski product of two complex vectors / of a real and a complex vector.  Both factors vary from term to term
+// here, so the second FFMA2 takes the broadcast of a.im (free) against (-b.im, b.re) (one sign flip) rather than a
+// materialised (-a.im, a.im) pair (two moves).
+__device__ __forceinline__ float2 mdot2(const float2 (&A)[4], const float2 (&B)[4]) {
+  float2 r = __fmul2_rn(make_float2(A[0].x, A[0].x), B[0]);
+  r = __ffma2_rn(make_float2(A[0].y, A[0].y), make_float2(-B[0].y, B[0].x), r);
+#pragma unroll
+  for (int i = 1; i < 4; i++) {
+    r = __ffma2_rn(make_float2(-A[i].x, -A[i].x), B[i], r);
+    r = __ffma2_rn(make_float2(A[i].y, A[i].y), make_float2(B[i].y, -B[i].x), r);
+  }
+  return r;
+}
+__device__ __forceinline__ float2 mdot2(const float (&k)[4], const float2 (&A)[4]) {
+  float2 r = __fmul2_rn(make_float2(k[0], k[0]), A[0]);
+  r = rmac2(r, -k[1], A[1]);
+  r = rmac2(r, -k[2], A[2]);
+  return rmac2(r, -k[3], A[3]);
+}
+__device__ __forceinline__ void v3_acc(vec4<float>& acc, const vec4<float>& A, const vec4<float>& B, const float* kA,
+                                       const float* kB) {
+  float2 a[4], b[4];
+  float kab[4], k1[4], k2[4];
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    a[i] = pk(A.c[i]); b[i] = pk(B.c[i]);
+    kab[i] = kA[i] - kB[i];
+    k1[i] = kA[i] + 2.f * kB[i];
+    k2[i] = -(2.f * kA[i] + kB[i]);
+  }
+  const float2 ab = mdot2(a, b), ca = mdot2(k1, a), cb = mdot2(k2, b);
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    float2 t = rmac2(pk(acc.c[i]), kab[i], ab);
+    t = cmac2(t, ca, b[i]);
+    t = cmac2(t, cb, a[i]);
+    acc.c[i].re = t.x; acc.c[i].im = t.y;
+  }
+}
+__device__ __forceinline__ void v4_acc(vec4<float>& acc, const vec4<float>& A, const vec4<float>& B, const vec4<float>& C) {
+  float2 a[4], b[4], c[4];
+#pragma unroll
+  for (int i = 0; i < 4; i++) { a[i] = pk(A.c[i]); b[i] = pk(B.c[i]); c[i] = pk(C.c[i]); }
+  float2 ac = mdot2(a, c);
+  ac = __fadd2_rn(ac, ac);
+  const float2 bc = mdot2(b, c), ab = mdot2(a, b);
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    float2 t = cmac2(pk(acc.c[i]), ac, b[i]);
+    t = cmsc2(t, bc, a[i]);
+    t = cmsc2(t, ab, c[i]);
+    acc.c[i].re = t.x; acc.c[i].im = t.y;
+  }
+}
+
 template <class G, typename T>
 struct GrpGeom {
   // NGRP combinations per event, processed NPASS groups at a time (n = 4: all 16 at once; n = 5: shared memory
   // holds 12 of the 32)
   // HTL: both t helicities are walked by the same lane (every current loaded from shared memory feeds two
   // quark-line products); otherwise lanes are (s1, h_t) pairs
+#ifdef ME_HTL
+  static constexpr bool HTL = (ME_HTL != 0);
+#else
   static constexpr bool HTL = (G::n <= 4);
+#endif
   static constexpr int N = G::n, NHT = HTL ? 2 : 1, LPG = HTL ? N : 2 * N, GPW = 32 / LPG, NGRP = 1 << N;
-  static constexpr int NPASS = (N <= 4) ? NGRP : 4 * GPW;
+  static constexpr int NPASS = (N <= 4) ? NGRP : 12;
   static constexpr int NW = (NPASS + GPW - 1) / GPW, NT = NW * 32;
   // T units per group: current slots + J[ncol][4][2]; padded so that the byte stride is 32 mod 128
   static constexpr int RAW = (G::nslot + G::ncol) * 8;
