@@ -547,22 +547,34 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
     if (tid == 0) ev.mt = T(a.par.mt);
     for (int task = tid; task < (1 << N) + N + 2 + 4; task += NT) {
       if (task < (1 << N)) {
-        // gluon subset m: momentum sum, quark-line momentum after it, 1/K^2, quark-line denominator
+        // gluon subset m: momentum sum, quark-line momentum after it, 1/K^2, quark-line denominator.
+        // Branch-free: every lane loads all gluon momenta and forms every 2 k_i.k_j, members are picked with
+        // 0/1 factors (exact), so the latency of this serial section is one round of loads + ~150 FP64 operations
         const int m = task;
-        double k[4] = {0.0, 0.0, 0.0, 0.0}, pairs = 0.0, line = 0.0;
-        int cnt = 0;
+        double kg[N][4], kt[4];
+#pragma unroll
         for (int i = 0; i < N; i++)
-          if ((m >> i) & 1) {
-            const int pi = (i < 2) ? i : i + 2;
-            cnt++;
-            for (int c = 0; c < 4; c++) k[c] += kd(pi, c);
-            line += dot2(2, pi);
-            for (int j = i + 1; j < N; j++)
-              if ((m >> j) & 1) pairs += dot2(pi, (j < 2) ? j : j + 2);
+#pragma unroll
+          for (int c = 0; c < 4; c++) kg[i][c] = kd((i < 2) ? i : i + 2, c);
+#pragma unroll
+        for (int c = 0; c < 4; c++) kt[c] = kd(2, c);
+        double k[4] = {0.0, 0.0, 0.0, 0.0}, pairs = 0.0, line = 0.0;
+#pragma unroll
+        for (int i = 0; i < N; i++) {
+          const double bi = ((m >> i) & 1) ? 1.0 : 0.0;
+#pragma unroll
+          for (int c = 0; c < 4; c++) k[c] += bi * kg[i][c];
+          line += bi * 2.0 * (kt[0] * kg[i][0] - kt[1] * kg[i][1] - kt[2] * kg[i][2] - kt[3] * kg[i][3]);
+#pragma unroll
+          for (int j = i + 1; j < N; j++) {
+            const double bj = ((m >> j) & 1) ? bi : 0.0;
+            pairs += bj * 2.0 * (kg[i][0] * kg[j][0] - kg[i][1] * kg[j][1] - kg[i][2] * kg[j][2] - kg[i][3] * kg[j][3]);
           }
+        }
+        const int cnt = __popc(m);
         for (int c = 0; c < 4; c++) {
           ev.Ksub[m][c] = T(k[c]);
-          ev.qsub[m][c] = T(-(kd(2, c) + k[c]));
+          ev.qsub[m][c] = T(-(kt[c] + k[c]));
         }
         ev.ik[m] = (cnt >= 2) ? T(1.0 / pairs) : T(0);
         const double den = line + pairs, nrm = 1.0 / (den * den + mw * mw);
@@ -578,25 +590,32 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
         // tasks 0,1: ubar(t), v(tbar) for both helicities; tasks 2..5: Q(h_t, h_tbar) = ubar gamma^mu v
         const int w = task - (1 << N) - N;
         spin4<T> ub[2], vv[2];
+#pragma unroll
         for (int which = 0; which < 2; which++) {
           mom4<T> k;
+#pragma unroll
           for (int c = 0; c < 4; c++) k.c[c] = T(-kd(2 + which, c));
           const spinbasis<T> sb = make_spinbasis<T>(k, T(a.par.mt));
+#pragma unroll
           for (int l = 0; l < 2; l++) {
             if (which) vv[l] = spinor_v(sb, l ? 1 : -1);
             else ub[l] = bar(spinor_u(sb, l ? 1 : -1));
           }
         }
         if (w < 2) {
+#pragma unroll
           for (int l = 0; l < 2; l++) {
-            const spin4<T>& sp = w ? vv[l] : ub[l];
             T* o = w ? ev.v[l] : ev.ub[l];
-            for (int c = 0; c < 4; c++) { o[2 * c] = sp.c[c].re; o[2 * c + 1] = sp.c[c].im; }
+#pragma unroll
+            for (int c = 0; c < 4; c++) {
+              o[2 * c] = w ? vv[l].c[c].re : ub[l].c[c].re;
+              o[2 * c + 1] = w ? vv[l].c[c].im : ub[l].c[c].im;
+            }
           }
         } else {
           const int v = w - 2;
           vec4<T> JR, JL;
-          chiral_currents((v >> 1) ? ub[1] : ub[0], (v & 1) ? vv[1] : vv[0], JR, JL);
+          chiral_currents(select((v >> 1) != 0, ub[1], ub[0]), select((v & 1) != 0, vv[1], vv[0]), JR, JL);
           for (int c = 0; c < 4; c++) { ev.Q[v][2 * c] = JR.c[c].re + JL.c[c].re; ev.Q[v][2 * c + 1] = JR.c[c].im + JL.c[c].im; }
         }
       }
