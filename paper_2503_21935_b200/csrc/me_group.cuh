@@ -519,6 +519,54 @@ __device__ __forceinline__ void grp_warp_select(const double (&val)[PER], const 
   else sel = bo ? __shfl_sync(0xffffffffu, lastok, 31 - __clz(bo)) : 0;
 }
 
+// float colour sum of one variant (h_t, h_tbar) with the real and imaginary parts of J as one packed f32x2 pair
+// (inline PTX on 64-bit registers: arrays of them unroll like scalars, arrays of float2 through the builtins did
+// not): returns Re(J^dagger C J) = x^T C x + y^T C y for J = x + i y, J_a at J[a*8 + 2*v .. +1]
+__device__ __forceinline__ unsigned long long pk2(float x, float y) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y));
+  return r;
+}
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+  unsigned long long r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ unsigned long long mul2(unsigned long long a, unsigned long long b) {
+  unsigned long long r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+template <int NCOL, typename T, class CM>
+__device__ __forceinline__ float grp_quadform_pk(const T* J, int v, float* x2 /*[NCOL] += |J_a|^2 or nullptr*/, float keep) {
+  static_assert(NCOL <= 24, "register-resident form");
+  unsigned long long x[NCOL];
+  float xr[NCOL], xi[NCOL];
+#pragma unroll
+  for (int a = 0; a < NCOL; a++) {
+    xr[a] = float(J[a * 8 + 2 * v]); xi[a] = float(J[a * 8 + 2 * v + 1]);
+    x[a] = pk2(xr[a], xi[a]);
+  }
+  unsigned long long s = pk2(0.f, 0.f);
+#pragma unroll
+  for (int a = 0; a < NCOL; a++) {
+    const float caa = 0.5f * CM::at(a * NCOL + a);
+    unsigned long long y = mul2(pk2(caa, caa), x[a]);
+#pragma unroll
+    for (int b = a + 1; b < NCOL; b++) {
+      const float c = CM::at(a * NCOL + b);
+      y = fma2(pk2(c, c), x[b], y);
+    }
+    s = fma2(x[a], y, s);
+    if (x2) x2[a] += keep * (xr[a] * xr[a] + xi[a] * xi[a]);
+  }
+  float sx, sy;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(sx), "=f"(sy) : "l"(s));
+  return 2.f * (sx + sy);
+}
+template <typename TC> struct GrpIsFloat { static constexpr bool value = false; };
+template <> struct GrpIsFloat<float> { static constexpr bool value = true; };
+
 template <class G, typename T, typename TC, class CM, int MODE, int MINB>
 __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const LaunchArgs a) {
   typedef GrpGeom<G, T> GE;
@@ -715,6 +763,17 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
         double q = 0.0;
         for (int l = 0; l < LPG; l++) q += (double)slots[l * 8 + 2 * r] + (double)slots[l * 8 + 2 * r + 1];
         ev.mh[hel_row(r)] = 2.0 * q;
+      }
+    } else if constexpr (GrpIsFloat<TC>::value) {
+      // float colour sum: task = variant (4 per group), re and im of J as one packed f32x2 pair
+#pragma unroll 1
+      for (int k0 = 0; k0 < 4; k0 += LPG) {
+        const int v = k0 + r;
+        if (active && v < 4) {
+          const int h = hel_row(v);
+          const float keep = is_good(h) ? 1.f : 0.f;
+          ev.mh[h] = (double)grp_quadform_pk<G::ncol, T, CM>(J, v, (MODE == MODE_SELECT) ? wloc : nullptr, keep);
+        }
       }
     } else {
       // task = (variant, re/im): 8 per group, lane r takes tasks r, r + LPG, ...; pairs are added by one shuffle
