@@ -593,8 +593,13 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
       return 2.0 * (kd(p, 0) * kd(q, 0) - kd(p, 1) * kd(q, 1) - kd(p, 2) * kd(q, 2) - kd(p, 3) * kd(q, 3));
     };
     if (tid == 0) ev.mt = T(a.par.mt);
-    for (int task = tid; task < (1 << N) + N + 2 + 4; task += NT) {
-      if (task < (1 << N)) {
+    // the subset tasks run on warp 0, the wavefunction tasks on warp 1: different task types in one warp would
+    // diverge and run one after the other, and this section is pure latency for the whole block
+    static_assert((1 << N) <= 32 && NT >= 32 + N + 6, "setup task layout");
+    {
+      const int task = (tid < (1 << N)) ? tid : ((tid >= 32 && tid < 32 + N + 6) ? (1 << N) + tid - 32 : -1);
+      if (task < 0) {
+      } else if (task < (1 << N)) {
         // gluon subset m: momentum sum, quark-line momentum after it, 1/K^2, quark-line denominator.
         // Branch-free: every lane loads all gluon momenta and forms every 2 k_i.k_j, members are picked with
         // 0/1 factors (exact), so the latency of this serial section is one round of loads + ~150 FP64 operations
