@@ -50,3 +50,25 @@ def test_fullsize_sampled_against_oracle(process, precision, nevt, nsample, tol)
     if precision == "fp32":
         assert np.median(rel) <= 1e-5
     m.close()
+
+
+@pytest.mark.parametrize("process,nevt", [("gg_ttg", 65536), ("gg_ttgg", 65536), ("gg_ttggg", 2048)])
+def test_accuracy_tail_every_event(process, nevt):
+    """Every event of a larger batch against the oracle (flat RAMBO has a soft/collinear tail, no cuts): the
+    BASELINE tolerances hold for the worst event, not only for sampled ones (accuracy)."""
+    import torch
+    from oracle import oracle as O
+    from paper_2503_21935_b200.me import MatrixElement
+    mom = I.make_momenta(process, nevt, seed=1)
+    gs = I.make_gs(nevt, seed=1, alphas=ALPHAS[process])
+    ref = O.me(process, mom, gs)
+    d_mom, d_gs = torch.from_numpy(mom).cuda(), torch.from_numpy(gs).cuda()
+    for precision, tol in (("fp64", 1e-10), ("mixed", 1e-5), ("fp32", 1e-3)):
+        m = MatrixElement(process, precision)
+        m.filter_helicities(d_mom, d_gs)
+        me = m.compute(d_mom, d_gs)[0].cpu().numpy()
+        rel = np.abs(me - ref) / ref
+        assert rel.max() <= tol, f"{precision}: max rel diff {rel.max():.3e} at event {rel.argmax()}"
+        if precision == "fp32":
+            assert np.median(rel) <= 1e-5
+        m.close()
