@@ -1,18 +1,21 @@
 // me_group.cuh -- the "lane-group" event kernel (layout B2) for g g -> t tbar + (n-2) g, n >= 4.
 //
-// One CUDA block per event.  A GROUP of LPG lanes of one warp (n lanes, or 2n when the t helicities are split over
-// lanes) owns one combination of the n gluon
-// helicities; the four (h_t, h_tbar) combinations are handled inside the group, so the gluon currents
+// One CUDA block per event.  A GROUP of LPG lanes of one warp owns one combination of the n gluon helicities
+// (n = 4: 4 lanes, one per first gluon s1 of the colour flow, both t helicities walked by the same lane; n = 5:
+// 10 lanes (s1, h_t)); the four (h_t, h_tbar) combinations are handled inside the group, so the gluon currents
 // are computed once per gluon-helicity combination instead of once per helicity.
-// Phases of a group (warp-synchronous, no block barrier until the final reduction):
+// Per event the block first forms the helicity-independent data in shared memory (one branch-free phase, one
+// block barrier); then every group runs, warp-synchronously:
 //   leaves  lane i < n      : polarisation vector of gluon i (a2)                       -> shared memory slot
 //   tree    lane = sequence : colour-ordered currents Jord(seq), |seq| = 2..n-1 (a3)    -> shared memory slot
 //           |seq| = n       : contracted at once with the four t-tbar currents Q(h_t,h_tbar) -> J init (a4, a5)
-//   walk    lane = (s1,h_t) : quark line for the flows that start with gluon s1 (a3-a5) -> J[flow][h_t][h_tbar]
-//   colour  lane = (h_t,h_tbar,re/im): x^T C x over the n! flows (a6)                   -> |M_h|^2
-// then the block sums the good helicities (a7), selects helicity / colour (a8) and stores (a9).
-// Operands of the walk are read from shared memory with 16-byte loads that are broadcast to the lanes of
-// a group, so one LDS.128 wavefront feeds 8 lanes; the running spinors stay in registers.
+//   walk    lane = s1       : quark line for the flows that start with gluon s1 (a3-a5) -> J[flow][h_t][h_tbar]
+//   colour  task = (h_t,h_tbar[,re/im]): x^T C x over the n! flows (a6)                 -> |M_h|^2
+// and one warp sums the good helicities in table order (a7), selects helicity / colour (a8) and stores (a9).
+// Current operands of the walk are read from shared memory with 16-byte loads (the lanes of a quarter-warp read
+// different slots: chunk-swizzled in the fp64 build) and feed both t helicities; the running spinors stay in
+// registers.  fp32 build: the two t-helicity chains, the complex arithmetic of the tree vertices and the colour
+// sum are packed f32x2 operations (FFMA2).  DESIGN.md section 5 has the measured history of these choices.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -464,8 +467,9 @@ struct GrpWalk<G, T, TC, G::n> {
 // x^T C x for the real vector x_a = J[a*8 + off] (a < ncol), C = integer numerators CM::at (symmetric)
 template <int NCOL, typename T, typename TC, class CM>
 __device__ __forceinline__ TC grp_quadform(const T* J, int off, TC* x2 /*[NCOL] += x_a^2 or nullptr*/, TC keep) {
+  static_assert(NCOL <= 24, "register-resident form (120 flows: the row-split loop of the kernel)");
   TC s = TC(0);
-  if (NCOL <= 24) {
+  {
     TC x[NCOL];
 #pragma unroll
     for (int a = 0; a < NCOL; a++) x[a] = TC(J[a * 8 + off]);
@@ -476,15 +480,6 @@ __device__ __forceinline__ TC grp_quadform(const T* J, int off, TC* x2 /*[NCOL] 
       for (int b = a + 1; b < NCOL; b++) y += CM::at(a * NCOL + b) * x[b];
       s += x[a] * y;
       if (x2) x2[a] += keep * x[a] * x[a];
-    }
-  } else {
-    for (int a = 0; a < NCOL; a++) {
-      const TC xa = TC(J[a * 8 + off]);
-      TC y = TC(0.5) * CM::at(a * NCOL + a) * xa;
-#pragma unroll 8
-      for (int b = a + 1; b < NCOL; b++) y += CM::at(a * NCOL + b) * TC(J[b * 8 + off]);
-      s += xa * y;
-      if (x2) x2[a] += keep * xa * xa;
     }
   }
   return TC(2) * s;
