@@ -306,6 +306,29 @@ def main():
             line["sweep_mes_per_s"] = sw
             best = max((v, k) for k, v in sw.items() if k.startswith("fp64"))
             line["sweep_best"] = {"fp64": best[1], "fp32": max((v, k) for k, v in sw.items() if k.startswith("fp32"))[1]}
+        # self-contained step: inputs made on the device by me_generate, then me_compute
+        m4 = MatrixElement(process, a.precision, device=local)
+        m4.set_good_helicities(mask)
+        stream = torch.cuda.current_stream()
+        alphas_dev = 0.0 if ALPHAS[process] is None else ALPHAS[process]
+        for _ in range(a.warmup):
+            g = m4.generate(nevt, seed=1, alphas=alphas_dev)
+            m4.compute(*g, out=bufs[4], selhel=bufs[5], selcol=bufs[6])
+        torch.cuda.synchronize()
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record(stream)
+        for _ in range(a.steps):
+            g = m4.generate(nevt, seed=1, alphas=alphas_dev)
+        e1.record(stream)
+        for _ in range(a.steps):
+            g = m4.generate(nevt, seed=1, alphas=alphas_dev)
+            m4.compute(*g, out=bufs[4], selhel=bufs[5], selcol=bufs[6])
+        e2.record(stream)
+        torch.cuda.synchronize()
+        line["device_inputs"] = {"generate_events_per_s": a.steps * nevt / (e0.elapsed_time(e1) * 1e-3),
+                                 "generate_plus_compute_mes_per_s": a.steps * nevt / (e1.elapsed_time(e2) * 1e-3),
+                                 "api": "me_generate (seeded RAMBO on the device) + me_compute"}
+        m4.close()
         line["cpu_baseline"] = cpu_baseline(process)
     if rank == 0:
         print(json.dumps(line))

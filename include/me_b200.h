@@ -97,6 +97,17 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
 int me_compute_host(me_handle* h, const double* momenta, const double* gs, const double* rndhel,
                     const double* rndcol, int64_t nevt, double* me, int32_t* selhel, int32_t* selcol);
 
+/* Device-side seeded inputs (the paper's standalone application draws random numbers and
+ * maps them to momenta with a phase-space sampling algorithm).  Writes, for the events
+ * start .. start+nevt-1 of the seeded stream, d_momenta[nevt][npar][4] (incoming p0 = (E,0,0,E), p1 = (E,0,0,-E),
+ * E = sqrts/2; final state from RAMBO flat phase space with the process' masses) and, where the pointer is not
+ * NULL, d_gs[nevt] (alphas > 0: g_s = sqrt(4 pi alphas) fixed; alphas <= 0: alpha_s ~ U[0.10, 0.13] per event),
+ * d_rndhel[nevt], d_rndcol[nevt] (uniforms in (0,1)) and d_weight[nevt] (the RAMBO phase-space weight).  The
+ * numbers are those of paper_2503_21935_b200/inputs.py (same counter-based generator, fp64) up to the rounding of
+ * the device math library.  Enqueues on `stream`, does not synchronise. */
+int me_generate(me_handle* h, uint64_t seed, int64_t start, int64_t nevt, double sqrts, double alphas,
+                double* d_momenta, double* d_gs, double* d_rndhel, double* d_rndcol, double* d_weight, void* stream);
+
 /* launch geometry of the last me_compute (for reports): threads per block, blocks, registers per thread,
  * bytes of local (spill) memory per thread of the kernel used */
 int me_launch_info(const me_handle* h, int* threads, int* blocks, int* regs, int* local_bytes);

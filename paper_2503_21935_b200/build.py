@@ -47,6 +47,7 @@ def _units():
             yield f"{p}_p{prec}", os.path.join(CSRC, src), defs
     yield "api", os.path.join(CSRC, "me_api.cu"), []
     yield "peak", os.path.join(CSRC, "me_peak.cu"), []
+    yield "rambo", os.path.join(CSRC, "me_rambo.cu"), []
 
 
 def _deps_hash(defs):

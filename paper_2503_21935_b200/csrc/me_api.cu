@@ -10,6 +10,7 @@
 
 #include "../../include/me_b200.h"
 #include "me_kernels.cuh"
+#include "me_rambo.h"
 
 typedef int (*launch_fn)(const me::LaunchArgs&, int mode, void* stream, me::LaunchInfo* info, int dry);
 
@@ -352,6 +353,29 @@ int me_compute_host(me_handle* h, const double* momenta, const double* gs, const
   if (sh && (e = cudaMemcpyAsync(selhel, d_sh, b4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(h, e, "D2H selhel");
   if (sc && (e = cudaMemcpyAsync(selcol, d_sc, b4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(h, e, "D2H selcol");
   if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: synchronize");
+  return ME_OK;
+}
+
+int me_generate(me_handle* h, uint64_t seed, int64_t start, int64_t nevt, double sqrts, double alphas,
+                double* d_momenta, double* d_gs, double* d_rndhel, double* d_rndcol, double* d_weight, void* stream) {
+  if (!h) return ME_ERR_ARG;
+  if (nevt < 0 || start < 0) return fail(h, ME_ERR_ARG, "me_generate: negative nevt or start");
+  if (!(sqrts > 0.0)) return fail(h, ME_ERR_ARG, "me_generate: sqrts must be positive");
+  if (nevt > 0 && !d_momenta) return fail(h, ME_ERR_ARG, "me_generate: null momenta pointer");
+  if (misaligned(d_momenta, 8) || misaligned(d_gs, 8) || misaligned(d_rndhel, 8) || misaligned(d_rndcol, 8) || misaligned(d_weight, 8))
+    return fail(h, ME_ERR_ARG, "me_generate: misaligned pointer");
+  const int nfin = h->npar - 2;
+  me::RamboArgs a;
+  memset(&a, 0, sizeof(a));
+  a.mom = d_momenta; a.gs = d_gs; a.rndhel = d_rndhel; a.rndcol = d_rndcol; a.weight = d_weight;
+  a.nevt = nevt; a.start = start; a.sqrts = sqrts; a.alphas = alphas;
+  double msum = 0.0;
+  for (int i = 0; i < nfin; i++) { a.mass[i] = (h->proc->ngl && i < 2) ? h->par.mt : 0.0; msum += a.mass[i]; }
+  if (!(msum < sqrts)) return fail(h, ME_ERR_ARG, "me_generate: sqrts below the mass threshold");
+  cudaError_t e = cudaSetDevice(h->device);
+  if (e != cudaSuccess) return cuda_fail(h, e, "me_generate");
+  int ce = me::launch_rambo(a, nfin, (unsigned long long)seed, stream);
+  if (ce) return cuda_fail(h, (cudaError_t)ce, "me_generate: launch");
   return ME_OK;
 }
 

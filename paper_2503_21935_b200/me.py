@@ -19,7 +19,7 @@ PROCESSES = ("ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg")
 
 EXPORTS = ("me_create", "me_destroy", "me_last_error", "me_info", "me_helicity_table", "me_color_table",
            "me_color_matrix", "me_filter_helicities", "me_get_good_helicities", "me_set_good_helicities",
-           "me_compute", "me_compute_host", "me_launch_info", "me_fma_peak")
+           "me_compute", "me_compute_host", "me_generate", "me_launch_info", "me_fma_peak")
 
 
 class MEError(RuntimeError):
@@ -55,6 +55,7 @@ def load_library(path: str = LIB_PATH):
     L.me_set_good_helicities.argtypes = [vp, vp]
     L.me_compute.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, vp, vp]
     L.me_compute_host.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, vp]
+    L.me_generate.argtypes = [vp, ctypes.c_uint64, i64, i64, ctypes.c_double, ctypes.c_double, vp, vp, vp, vp, vp, vp]
     L.me_launch_info.argtypes = [vp, ip, ip, ip, ip]
     L.me_fma_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
     for n in EXPORTS:
@@ -194,6 +195,20 @@ class MatrixElement:
         self._check(self._L.me_compute_host(self._h, _hptr(mom), _hptr(gs), _hptr(rndhel), _hptr(rndcol), nevt,
                                             _hptr(out), _hptr(selhel), _hptr(selcol)))
         return out, selhel, selcol
+
+    def generate(self, nevt, seed=1, start=0, sqrts=1500.0, alphas=0.0, device=None, want_weight=False, stream=None):
+        """Seeded RAMBO inputs made on the device (me_generate): returns (momenta, gs, rndhel, rndcol[, weight])
+        as cuda float64 tensors for events start..start+nevt-1 of the stream; alphas <= 0 draws alpha_s ~ U[0.10, 0.13]."""
+        import torch
+        dev = torch.device("cuda", self.device) if device is None else device
+        f64 = torch.float64
+        mom = torch.empty((nevt, self.npar, 4), dtype=f64, device=dev)
+        gs, rh, rc = (torch.empty(nevt, dtype=f64, device=dev) for _ in range(3))
+        wt = torch.empty(nevt, dtype=f64, device=dev) if want_weight else None
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        self._check(self._L.me_generate(self._h, int(seed), int(start), int(nevt), float(sqrts), float(alphas), _ptr(mom, f64),
+                                        _ptr(gs, f64), _ptr(rh, f64), _ptr(rc, f64), _ptr(wt, f64), ctypes.c_void_p(s.cuda_stream)))
+        return (mom, gs, rh, rc, wt) if want_weight else (mom, gs, rh, rc)
 
     def launch_info(self) -> dict:
         v = [ctypes.c_int() for _ in range(4)]
