@@ -671,11 +671,8 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
     __syncthreads();
     auto is_good = [&](int h) { return MODE == MODE_FILTER || ((a.good.mask[h >> 6] >> (h & 63)) & 1ull) != 0ull; };
 
-    TC wloc[(MODE == MODE_SELECT) ? G::ncol : 1];
-    if (MODE == MODE_SELECT) {
-#pragma unroll
-      for (int c = 0; c < G::ncol; c++) wloc[c] = TC(0);
-    }
+    if (MODE == MODE_SELECT)  // colour weights of this warp's groups (a8), accumulated over the passes
+      for (int c = lane; c < G::ncol; c += 32) ev.wc[warp][c] = TC(0);
 #pragma unroll 1
     for (int pass0 = 0; pass0 < GE::NGRP; pass0 += GE::NPASS) {
     const int grp = pass0 + lgrp;                        // gluon-helicity combination
@@ -705,16 +702,17 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
     }
     __syncwarp();
     // ---- a6: colour sums.  Helicity row of variant v = 2 h_t + h_tbar of this group:
-    auto hel_row = [&](int v) {
+    auto hel_of = [&](int gg, int v) {
       int h = 0;
       for (int i = 0; i < N; i++) {
         const int p = (i < 2) ? i : i + 2;
-        h |= ((grp >> (N - 1 - i)) & 1) << (NPAR - 1 - p);
+        h |= ((gg >> (N - 1 - i)) & 1) << (NPAR - 1 - p);
       }
       h |= (v >> 1) << (NPAR - 1 - 2);
       h |= (v & 1) << (NPAR - 1 - 3);
       return h;
     };
+    auto hel_row = [&](int v) { return hel_of(grp, v); };
     if constexpr (G::ncol > 24) {
       // rows of C split over the lanes of the group; every C_ab read once feeds the 8 real vectors
       // (4 variants x re/im) of the group; partial sums meet in the (now free) current slots
@@ -743,12 +741,6 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
           }
 #pragma unroll
           for (int k = 0; k < 8; k++) part[k] += xa[k] * y[k];
-          if (MODE == MODE_SELECT) {
-            TC w = TC(0);
-#pragma unroll
-            for (int v = 0; v < 4; v++) w += keep[v] * (xa[2 * v] * xa[2 * v] + xa[2 * v + 1] * xa[2 * v + 1]);
-            wloc[a] += w;
-          }
         }
       }
       __syncwarp();  // every lane of the group is done with the current slots
@@ -772,7 +764,7 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
         if (active && v < 4) {
           const int h = hel_row(v);
           const float keep = is_good(h) ? 1.f : 0.f;
-          ev.mh[h] = (double)grp_quadform_pk<G::ncol, T, CM>(J, v, (MODE == MODE_SELECT) ? wloc : nullptr, keep);
+          ev.mh[h] = (double)grp_quadform_pk<G::ncol, T, CM>(J, v, nullptr, keep);
         }
       }
     } else {
@@ -786,23 +778,33 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
         if (on) {
           h = hel_row(k >> 1);
           const TC keep = is_good(h) ? TC(1) : TC(0);
-          q = grp_quadform<G::ncol, T, TC, CM>(J, k, (MODE == MODE_SELECT) ? wloc : nullptr, keep);
+          q = grp_quadform<G::ncol, T, TC, CM>(J, k, nullptr, keep);
         }
         q += __shfl_xor_sync(0xffffffffu, q, 1);
         if (on && !(k & 1)) ev.mh[h] = (double)q;
       }
     }
     __syncwarp();
-    }  // passes
     if (MODE == MODE_SELECT) {
+      // a8 colour weights w_c += sum over this warp's groups and the good (h_t, h_tbar) of |J_c|^2: lane = flow,
+      // read back from the J areas (cheaper than per-lane partial sums and a shuffle reduction per flow)
+      for (int c = lane; c < G::ncol; c += 32) {
+        TC w = TC(0);
+#pragma unroll 1
+        for (int g = 0; g < GPW; g++) {
+          const int lg = warp * GPW + g, gg = pass0 + lg;
+          if (lg < GE::NPASS && gg < GE::NGRP) {
+            const vec4<T> j = GrpVec<T>::ld(gbase + (size_t)lg * GE::GS + G::nslot * 8 + c * 8, 0u);
 #pragma unroll
-      for (int c = 0; c < G::ncol; c++) {
-        TC w = wloc[c];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
-        if (lane == 0) ev.wc[warp][c] = w;
+            for (int v = 0; v < 4; v++)
+              if (is_good(hel_of(gg, v))) w += TC(j.c[v].re) * TC(j.c[v].re) + TC(j.c[v].im) * TC(j.c[v].im);
+          }
+        }
+        ev.wc[warp][c] += w;
       }
+      __syncwarp();
     }
+    }  // passes
     __syncthreads();
     // ---- a7-a9
     if (MODE == MODE_FILTER) {
