@@ -570,6 +570,13 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
   extern __shared__ __align__(16) unsigned char smem_raw[];
   EV& ev = *reinterpret_cast<EV*>(smem_raw);
   T* gbase = reinterpret_cast<T*>(smem_raw + ((sizeof(EV) + 127) / 128) * 128);
+  // optional shared-memory copy of the colour matrix as 16-bit integers (behind the group areas), made once
+  const short* cm16 = reinterpret_cast<const short*>(gbase + (size_t)GrpGeom<G, T>::NPASS * GrpGeom<G, T>::GS);
+  if constexpr (CM::smem16) {
+    const int4* src = reinterpret_cast<const int4*>(CM::table16());
+    int4* dst = reinterpret_cast<int4*>(const_cast<short*>(cm16));
+    for (int i = threadIdx.x; i < (G::ncol * G::ncol * 2 + 15) / 16; i += GrpGeom<G, T>::NT) dst[i] = __ldg(src + i);
+  }
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int gi = lane / LPG, r = lane - gi * LPG;
   const int lgrp = warp * GPW + gi;                      // group slot of this lane within a pass
@@ -729,12 +736,12 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
           TC xa[8], y[8];
 #pragma unroll
           for (int k = 0; k < 4; k++) { xa[2 * k] = TC(ja.c[k].re); xa[2 * k + 1] = TC(ja.c[k].im); }
-          const TC caa = TC(0.5) * CM::at(a * G::ncol + a);
+          const TC caa = TC(0.5) * (CM::smem16 ? TC(cm16[a * G::ncol + a]) : CM::at(a * G::ncol + a));
 #pragma unroll
           for (int k = 0; k < 8; k++) y[k] = caa * xa[k];
 #pragma unroll 4
           for (int b = a + 1; b < G::ncol; b++) {
-            const TC c = CM::at(a * G::ncol + b);
+            const TC c = CM::smem16 ? TC(cm16[a * G::ncol + b]) : CM::at(a * G::ncol + b);
             const vec4<T> jb = GrpVec<T>::ld(J + b * 8, 0u);
 #pragma unroll
             for (int k = 0; k < 4; k++) { y[2 * k] += c * TC(jb.c[k].re); y[2 * k + 1] += c * TC(jb.c[k].im); }

@@ -35,13 +35,20 @@ typedef ME_CAT(Grp_, ME_PROC) Grp;
 // (constant memory up to 24 flows; the 120 x 120 matrix exceeds the 64 KB bank and is read through L1)
 #if ME_CMAT_GLOBAL
 __device__ const T_col c_cmat[Grp::ncol * Grp::ncol] = ME_CAT(ME_CMAT_, ME_PROC_UP);
+// the same numerators as 16-bit integers (|C| <= 4096): 28.8 KB, copied into shared memory by builds whose
+// amplitudes are fp64 (one block per SM anyway); the fp32 build keeps two blocks per SM and reads C through L1
+__device__ const short c_cmat16[Grp::ncol * Grp::ncol] = ME_CAT(ME_CMAT_, ME_PROC_UP);
 struct CMat {
+  static constexpr bool smem16 = (ME_PREC != 1);
   __device__ __forceinline__ static T_col at(int i) { return __ldg(c_cmat + i); }
+  __device__ __forceinline__ static const short* table16() { return c_cmat16; }
 };
 #else
 __constant__ T_col c_cmat[Grp::ncol * Grp::ncol] = ME_CAT(ME_CMAT_, ME_PROC_UP);
 struct CMat {
+  static constexpr bool smem16 = false;
   __device__ __forceinline__ static T_col at(int i) { return c_cmat[i]; }
+  __device__ __forceinline__ static const short* table16() { return nullptr; }
 };
 #endif
 
@@ -50,7 +57,7 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
   typedef me::GrpGeom<Grp, TA> GE;
   auto kern = me::group_kernel<Grp, TA, TCo, CMat, MODE, ME_MINB>;
   const size_t ev_bytes = ((sizeof(me::GrpEvent<TA, TCo, Grp::n>) + 127) / 128) * 128;
-  const size_t smem = ev_bytes + (size_t)GE::NPASS * GE::GS * sizeof(TA);
+  const size_t smem = ev_bytes + (size_t)GE::NPASS * GE::GS * sizeof(TA) + (CMat::smem16 ? (size_t)Grp::ncol * Grp::ncol * 2 + 16 : 0);
   cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (err != cudaSuccess) return (int)err;
   long long blocks = a.nevt;
