@@ -727,27 +727,41 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
 #pragma unroll
       for (int k = 0; k < 8; k++) part[k] = TC(0);
       if (active) {
-        TC keep[4];
-#pragma unroll
-        for (int v = 0; v < 4; v++) keep[v] = is_good(hel_row(v)) ? TC(1) : TC(0);
+        // RB rows of the lane at a time: every x_b fetched from shared memory feeds RB rows (the loop is bound by
+        // shared-memory wavefronts: the lanes are at different b, nothing is broadcast)
+        constexpr int RB = 3;
+        auto cmat = [&](int i) { return CM::smem16 ? TC(cm16[i]) : CM::at(i); };
 #pragma unroll 1
-        for (int a = r; a < G::ncol; a += LPG) {
-          const vec4<T> ja = GrpVec<T>::ld(J + a * 8, 0u);
-          TC xa[8], y[8];
+        for (int a0 = r; a0 < G::ncol; a0 += RB * LPG) {
+          TC xa[RB][8], y[RB][8];
+          int row[RB];
 #pragma unroll
-          for (int k = 0; k < 4; k++) { xa[2 * k] = TC(ja.c[k].re); xa[2 * k + 1] = TC(ja.c[k].im); }
-          const TC caa = TC(0.5) * (CM::smem16 ? TC(cm16[a * G::ncol + a]) : CM::at(a * G::ncol + a));
+          for (int j = 0; j < RB; j++) {
+            const int aj = a0 + j * LPG;
+            const bool on = aj < G::ncol;
+            row[j] = on ? aj : G::ncol - 1;
+            const vec4<T> ja = GrpVec<T>::ld(J + row[j] * 8, 0u);
 #pragma unroll
-          for (int k = 0; k < 8; k++) y[k] = caa * xa[k];
-#pragma unroll 4
-          for (int b = a + 1; b < G::ncol; b++) {
-            const TC c = CM::smem16 ? TC(cm16[a * G::ncol + b]) : CM::at(a * G::ncol + b);
+            for (int k = 0; k < 4; k++) { xa[j][2 * k] = on ? TC(ja.c[k].re) : TC(0); xa[j][2 * k + 1] = on ? TC(ja.c[k].im) : TC(0); }
+            const TC caa = TC(0.5) * cmat(row[j] * G::ncol + row[j]);
+#pragma unroll
+            for (int k = 0; k < 8; k++) y[j][k] = caa * xa[j][k];
+            if (!on) row[j] = G::ncol;  // no column b > row: contributes nothing
+          }
+#pragma unroll 2
+          for (int b = a0 + 1; b < G::ncol; b++) {
             const vec4<T> jb = GrpVec<T>::ld(J + b * 8, 0u);
 #pragma unroll
-            for (int k = 0; k < 4; k++) { y[2 * k] += c * TC(jb.c[k].re); y[2 * k + 1] += c * TC(jb.c[k].im); }
+            for (int j = 0; j < RB; j++) {
+              const TC c = (b > row[j]) ? cmat(row[j] * G::ncol + b) : TC(0);
+#pragma unroll
+              for (int k = 0; k < 4; k++) { y[j][2 * k] += c * TC(jb.c[k].re); y[j][2 * k + 1] += c * TC(jb.c[k].im); }
+            }
           }
 #pragma unroll
-          for (int k = 0; k < 8; k++) part[k] += xa[k] * y[k];
+          for (int j = 0; j < RB; j++)
+#pragma unroll
+            for (int k = 0; k < 8; k++) part[k] += xa[j][k] * y[j][k];
         }
       }
       __syncwarp();  // every lane of the group is done with the current slots
