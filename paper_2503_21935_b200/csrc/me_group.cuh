@@ -729,7 +729,7 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
       if (active) {
         // RB rows of the lane at a time: every x_b fetched from shared memory feeds RB rows (the loop is bound by
         // shared-memory wavefronts: the lanes are at different b, nothing is broadcast)
-        constexpr int RB = 3;
+        constexpr int RB = 4;
         auto cmat = [&](int i) { return CM::smem16 ? TC(cm16[i]) : CM::at(i); };
 #pragma unroll 1
         for (int a0 = r; a0 < G::ncol; a0 += RB * LPG) {
