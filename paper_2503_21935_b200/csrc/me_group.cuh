@@ -62,6 +62,7 @@ struct alignas(16) GrpEvent {
   T pol[N][6];
   T mt;
   TC wc[5][(N == 4) ? 24 : (N == 5 ? 120 : 6)];  // per-warp colour weights (at most 4 warps per block)
+  unsigned char gmask[1 << N];  // per gluon-helicity combination: bit v set iff helicity row (combination, v) is good
 };
 
 template <typename T> struct GrpVec;
@@ -595,6 +596,23 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
       return 2.0 * (kd(p, 0) * kd(q, 0) - kd(p, 1) * kd(q, 1) - kd(p, 2) * kd(q, 2) - kd(p, 3) * kd(q, 3));
     };
     if (tid == 0) ev.mt = T(a.par.mt);
+    auto is_good = [&](int h) { return MODE == MODE_FILTER || ((a.good.mask[h >> 6] >> (h & 63)) & 1ull) != 0ull; };
+    auto hel_of = [&](int gg, int v) {  // helicity row of gluon-helicity combination gg and variant v = 2 h_t + h_tbar
+      int h = 0;
+      for (int i = 0; i < N; i++) {
+        const int p = (i < 2) ? i : i + 2;
+        h |= ((gg >> (N - 1 - i)) & 1) << (NPAR - 1 - p);
+      }
+      h |= (v >> 1) << (NPAR - 1 - 2);
+      h |= (v & 1) << (NPAR - 1 - 3);
+      return h;
+    };
+    if (MODE == MODE_SELECT && tid >= NT - GE::NGRP) {  // the last NGRP threads: good-helicity bits per combination
+      const int gg = tid - (NT - GE::NGRP);
+      int m = 0;
+      for (int v = 0; v < 4; v++) m |= is_good(hel_of(gg, v)) ? (1 << v) : 0;
+      ev.gmask[gg] = (unsigned char)m;
+    }
     // the subset tasks run on warp 0, the wavefunction tasks on warp 1: different task types in one warp would
     // diverge and run one after the other, and this section is pure latency for the whole block
     static_assert((1 << N) <= 32 && NT >= 32 + N + 6, "setup task layout");
@@ -676,8 +694,6 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
       }
     }
     __syncthreads();
-    auto is_good = [&](int h) { return MODE == MODE_FILTER || ((a.good.mask[h >> 6] >> (h & 63)) & 1ull) != 0ull; };
-
     if (MODE == MODE_SELECT)  // colour weights of this warp's groups (a8), accumulated over the passes
       for (int c = lane; c < G::ncol; c += 32) ev.wc[warp][c] = TC(0);
 #pragma unroll 1
@@ -709,16 +725,6 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
     }
     __syncwarp();
     // ---- a6: colour sums.  Helicity row of variant v = 2 h_t + h_tbar of this group:
-    auto hel_of = [&](int gg, int v) {
-      int h = 0;
-      for (int i = 0; i < N; i++) {
-        const int p = (i < 2) ? i : i + 2;
-        h |= ((gg >> (N - 1 - i)) & 1) << (NPAR - 1 - p);
-      }
-      h |= (v >> 1) << (NPAR - 1 - 2);
-      h |= (v & 1) << (NPAR - 1 - 3);
-      return h;
-    };
     auto hel_row = [&](int v) { return hel_of(grp, v); };
     if constexpr (G::ncol > 24) {
       // rows of C split over the lanes of the group; every C_ab read once feeds the 8 real vectors
@@ -816,9 +822,12 @@ __global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const La
           const int lg = warp * GPW + g, gg = pass0 + lg;
           if (lg < GE::NPASS && gg < GE::NGRP) {
             const vec4<T> j = GrpVec<T>::ld(gbase + (size_t)lg * GE::GS + G::nslot * 8 + c * 8, 0u);
+            const int gm = ev.gmask[gg];
 #pragma unroll
-            for (int v = 0; v < 4; v++)
-              if (is_good(hel_of(gg, v))) w += TC(j.c[v].re) * TC(j.c[v].re) + TC(j.c[v].im) * TC(j.c[v].im);
+            for (int v = 0; v < 4; v++) {
+              const TC keep = ((gm >> v) & 1) ? TC(1) : TC(0);
+              w += keep * (TC(j.c[v].re) * TC(j.c[v].re) + TC(j.c[v].im) * TC(j.c[v].im));
+            }
           }
         }
         ev.wc[warp][c] += w;
