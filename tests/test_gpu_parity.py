@@ -16,7 +16,7 @@ NEVT = {"ee_mumu": 16384, "gg_tt": 8192 + 77, "gg_ttg": 4096 + 77, "gg_ttgg": 10
 ALPHAS = {"ee_mumu": 0.118, "gg_tt": 0.118, "gg_ttg": 0.118, "gg_ttgg": None, "gg_ttggg": 0.118}
 BUILDS = [("ee_mumu", "fp64"), ("gg_tt", "fp64"), ("gg_tt", "fp32"), ("gg_ttg", "fp64"), ("gg_ttg", "fp32"),
           ("gg_ttg", "mixed"), ("gg_ttgg", "fp64"), ("gg_ttgg", "fp32"), ("gg_ttgg", "mixed"),
-          ("gg_ttggg", "fp64"), ("gg_ttggg", "fp32")]
+          ("gg_ttggg", "fp64"), ("gg_ttggg", "fp32"), ("gg_ttggg", "mixed")]
 
 
 @pytest.fixture(scope="module")
@@ -91,13 +91,15 @@ def _check_selection(sel_gpu, sel_ref, cum, rnd, tol):
 def test_selection_matches_oracle(torch_cuda, process, precision):
     case = oracle_case(process)
     got = run_gpu(torch_cuda, process, precision, case)
-    tol = TOL[precision] * 10
+    tol = TOL[precision]        # north_star: mismatches only where the cumulative weight is within tolerance of r
     sel = case["sel"]
     nbad_h = _check_selection(got["selhel"], sel["selhel"], sel["cumhel"], case["rh"], tol)
     nbad_c = _check_selection(got["selcol"], sel["selcol"], sel["cumcol"], case["rc"], tol)
     n = len(case["rh"])
-    # boundary cases must be rare: a wrong rule would disagree on a finite fraction of events
-    assert nbad_h <= max(2, n * tol * 100) and nbad_c <= max(2, n * tol * 100)
+    # boundary cases must be rare: r falls within tol of one of the ngood (ncol) boundaries with probability
+    # ~2 tol ngood; twice that is allowed.  A wrong rule would disagree on a finite fraction of events.
+    ngood, ncol = int(case["mask"].sum()), sel["cumcol"].shape[1]
+    assert nbad_h <= max(2, 4 * tol * ngood * n) and nbad_c <= max(2, 4 * tol * ncol * n)
     # selected helicities are good ones, colours are in range
     assert np.all(case["mask"][got["selhel"]] == 1)
     assert got["selcol"].min() >= 0 and got["selcol"].max() < sel["cumcol"].shape[1]

@@ -8,7 +8,7 @@ from oracle import oracle as O
 from paper_2503_21935_b200 import inputs as I
 
 
-@pytest.mark.parametrize("proc,nev", [("gg_tt", 3), ("gg_ttg", 3), ("gg_ttgg", 1)])
+@pytest.mark.parametrize("proc,nev", [("gg_tt", 3), ("gg_ttg", 3), ("gg_ttgg", 1), ("gg_ttggg", 1)])
 @pytest.mark.parametrize("wt", [0.0, 1.4915])
 def test_route_a_equals_route_b(proc, nev, wt):
     i = O.info(proc)
@@ -16,7 +16,7 @@ def test_route_a_equals_route_b(proc, nev, wt):
     ht = O.helicity_table(proc)
     flows = [tuple(r) for r in O.color_table(proc).tolist()]
     gs = 1.17
-    hels = range(i["ncomb"]) if proc != "gg_ttgg" else [0, 7, 21, 38, 63]
+    hels = {"gg_ttgg": [0, 7, 21, 38, 63], "gg_ttggg": [5, 42, 77, 100, 126]}.get(proc, range(i["ncomb"]))
     for e in range(nev):
         for h in hels:
             ja = O.jamps(proc, mom[e], gs, h, params=dict(wt=wt))
