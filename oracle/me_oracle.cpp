@@ -22,7 +22,8 @@
 // criterion, helicity/colour selection rule) are OUR reading (readings R10, R11): the
 // paper is silent, so orc_select is "parity unpinned" against the paper.
 //
-// Build: g++ -O2 -fopenmp -shared -fPIC me_oracle.cpp -o libme_oracle.so   (oracle/oracle.py does it)
+// Build: g++ -O2 -fopenmp -shared -fPIC me_oracle.cpp -o libme_oracle.so   (oracle/oracle.py does it), and the same
+// source with -DORC_COUNT -> libme_oracle_count.so: the operation-counting scalar of "counted mode" (see real_t).
 
 #include <algorithm>
 #include <cmath>
@@ -36,7 +37,53 @@
 #include <omp.h>
 #endif
 
-typedef std::complex<double> cd;
+// Scalar type of the amplitude arithmetic.  Plain build: double.  Counted build (-DORC_COUNT, "counted mode" of
+// SURVEY.md 8(d); BASELINE.json north_star "FLOPs per ME counted by the instrumented oracle"): a double that counts
+// every addition/subtraction, multiplication, division and square root it takes part in.  The source is the same,
+// so the counted build performs exactly the operations of the plain one.
+#ifdef ORC_COUNT
+struct OpCount { long add, mul, div, sqrt; };
+static OpCount g_ops = {0, 0, 0, 0};  // the counted build is driven single-threaded (orc_count_ops)
+struct real_t {
+  double v;
+  real_t() : v(0.0) {}
+  real_t(double x) : v(x) {}
+  real_t(int x) : v(x) {}
+};
+static inline real_t operator+(real_t a, real_t b) { g_ops.add++; return real_t(a.v + b.v); }
+static inline real_t operator-(real_t a, real_t b) { g_ops.add++; return real_t(a.v - b.v); }
+static inline real_t operator*(real_t a, real_t b) { g_ops.mul++; return real_t(a.v * b.v); }
+static inline real_t operator/(real_t a, real_t b) { g_ops.div++; return real_t(a.v / b.v); }
+static inline real_t operator-(real_t a) { return real_t(-a.v); }  // sign flip: not an arithmetic operation
+static inline real_t& operator+=(real_t& a, real_t b) { a = a + b; return a; }
+static inline real_t& operator-=(real_t& a, real_t b) { a = a - b; return a; }
+static inline real_t& operator*=(real_t& a, real_t b) { a = a * b; return a; }
+static inline real_t& operator/=(real_t& a, real_t b) { a = a / b; return a; }
+static inline bool operator==(real_t a, real_t b) { return a.v == b.v; }
+static inline bool operator!=(real_t a, real_t b) { return a.v != b.v; }
+static inline bool operator<(real_t a, real_t b) { return a.v < b.v; }
+static inline bool operator>(real_t a, real_t b) { return a.v > b.v; }
+static inline bool operator>=(real_t a, real_t b) { return a.v >= b.v; }
+static inline real_t SQRT(real_t a) { g_ops.sqrt++; return real_t(std::sqrt(a.v)); }
+static inline double to_double(real_t a) { return a.v; }
+#else
+typedef double real_t;
+static inline double SQRT(double a) { return std::sqrt(a); }
+static inline double to_double(double a) { return a; }
+#endif
+typedef std::complex<real_t> cd;
+typedef std::complex<double> cdd;  // colour algebra (Gell-Mann matrices, colour matrix): never counted
+// |z|^2 = re^2 + im^2 (what std::norm does for double; written out so that the counted scalar sees it)
+static inline real_t cnorm(const cd& z) { return z.real() * z.real() + z.imag() * z.imag(); }
+// complex division: the library routine in the plain build, the textbook formula for the counted scalar
+static inline cd cdiv(const cd& a, const cd& b) {
+#ifdef ORC_COUNT
+  real_t n = cnorm(b);
+  return cd((a.real() * b.real() + a.imag() * b.imag()) / n, (a.imag() * b.real() - a.real() * b.imag()) / n);
+#else
+  return a / b;
+#endif
+}
 static const cd I_(0.0, 1.0);
 
 // ----------------------------------------------------------------------------------------------
@@ -114,7 +161,7 @@ static cd row_col(const Sp& r, const Sp& c) {
   for (int i = 0; i < 4; i++) s += r.c[i] * c.c[i];
   return s;
 }
-static M4 madd_mass(const M4& a, double m) {  // a + m*1
+static M4 madd_mass(const M4& a, real_t m) {  // a + m*1
   M4 r = a;
   for (int i = 0; i < 4; i++) r.m[i][i] += m;
   return r;
@@ -128,11 +175,11 @@ static Sp bar(const Sp& u) {  // u^dagger gamma^0, gamma^0 = diag(1,1,-1,-1)
   return r;
 }
 // chirality projectors in the Dirac representation: gamma^5 = [[0,1],[1,0]] (2x2 blocks)
-static M4 chiral_coupling(double gL, double gR) {  // gL*P_L + gR*P_R, P_L/R = (1 -/+ gamma5)/2
+static M4 chiral_coupling(real_t gL, real_t gR) {  // gL*P_L + gR*P_R, P_L/R = (1 -/+ gamma5)/2
   M4 r;
   for (int i = 0; i < 4; i++)
     for (int j = 0; j < 4; j++) r.m[i][j] = 0.0;
-  double d = 0.5 * (gL + gR), o = 0.5 * (gR - gL);
+  real_t d = 0.5 * (gL + gR), o = 0.5 * (gR - gL);
   for (int i = 0; i < 4; i++) r.m[i][i] = d;
   r.m[0][2] = o; r.m[1][3] = o; r.m[2][0] = o; r.m[3][1] = o;
   return r;
@@ -153,8 +200,8 @@ static M4 mmul(const M4& a, const M4& b) {
 // of the given momenta).  Two-component helicity spinors chi_lambda(p), sigma.phat chi = lambda chi.
 // ----------------------------------------------------------------------------------------------
 static void chi(const double* p, int lam, cd out[2]) {
-  double px = p[1], py = p[2], pz = p[3];
-  double pp = std::sqrt(px * px + py * py + pz * pz);
+  real_t px = p[1], py = p[2], pz = p[3];
+  real_t pp = SQRT(px * px + py * py + pz * pz);
   if (pp == 0.0) {  // particle at rest: quantise along +z (reading R9)
     if (lam > 0) { out[0] = 1.0; out[1] = 0.0; } else { out[0] = 0.0; out[1] = 1.0; }
     return;
@@ -163,37 +210,37 @@ static void chi(const double* p, int lam, cd out[2]) {
     if (lam > 0) { out[0] = 0.0; out[1] = 1.0; } else { out[0] = -1.0; out[1] = 0.0; }
     return;
   }
-  double n = 1.0 / std::sqrt(2.0 * pp * (pp + pz));
+  real_t n = 1.0 / SQRT(2.0 * pp * (pp + pz));
   if (lam > 0) { out[0] = n * (pp + pz); out[1] = n * cd(px, py); }
   else         { out[0] = n * cd(-px, py); out[1] = n * (pp + pz); }
 }
 // u(p,lambda): particle spinor, Dirac representation: ( sqrt(E+m) chi ; lambda |p|/sqrt(E+m) chi )
-static Sp spinor_u(const double* p, double m, int lam) {
-  double pp = std::sqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
-  double up = std::sqrt(p[0] + m), lo = (up > 0.0) ? pp / up : 0.0;
+static Sp spinor_u(const double* p, real_t m, int lam) {
+  real_t pp = SQRT(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
+  real_t up = SQRT(p[0] + m), lo = (up > 0.0) ? pp / up : 0.0;
   cd x[2];
   chi(p, lam, x);
   Sp u;
   u.c[0] = up * x[0]; u.c[1] = up * x[1];
-  u.c[2] = double(lam) * lo * x[0]; u.c[3] = double(lam) * lo * x[1];
+  u.c[2] = real_t(lam) * lo * x[0]; u.c[3] = real_t(lam) * lo * x[1];
   return u;
 }
 // v(p,lambda): antiparticle spinor of physical helicity lambda: ( -lambda |p|/sqrt(E+m) chi_{-lambda} ; sqrt(E+m) chi_{-lambda} )
-static Sp spinor_v(const double* p, double m, int lam) {
-  double pp = std::sqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
-  double up = std::sqrt(p[0] + m), lo = (up > 0.0) ? pp / up : 0.0;
+static Sp spinor_v(const double* p, real_t m, int lam) {
+  real_t pp = SQRT(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
+  real_t up = SQRT(p[0] + m), lo = (up > 0.0) ? pp / up : 0.0;
   cd x[2];
   chi(p, -lam, x);
   Sp v;
-  v.c[0] = -double(lam) * lo * x[0]; v.c[1] = -double(lam) * lo * x[1];
+  v.c[0] = -real_t(lam) * lo * x[0]; v.c[1] = -real_t(lam) * lo * x[1];
   v.c[2] = up * x[0]; v.c[3] = up * x[1];
   return v;
 }
 // polarisation vector of a massless vector, helicity lambda: eps = (-lambda*e1 - i e2)/sqrt(2)
 static V4 polvec(const double* p, int lam) {
-  double px = p[1], py = p[2], pz = p[3];
-  double pt2 = px * px + py * py, pt = std::sqrt(pt2), pp = std::sqrt(pt2 + pz * pz);
-  double e1[3], e2[3];
+  real_t px = p[1], py = p[2], pz = p[3];
+  real_t pt2 = px * px + py * py, pt = SQRT(pt2), pp = SQRT(pt2 + pz * pz);
+  real_t e1[3], e2[3];
   if (pt == 0.0) {
     e1[0] = 1; e1[1] = 0; e1[2] = 0;
     e2[0] = 0; e2[1] = (pz >= 0 ? 1.0 : -1.0); e2[2] = 0;
@@ -203,8 +250,8 @@ static V4 polvec(const double* p, int lam) {
   }
   V4 e;
   e.c[0] = 0.0;
-  double s = 1.0 / std::sqrt(2.0);
-  for (int i = 0; i < 3; i++) e.c[i + 1] = s * cd(-double(lam) * e1[i], -e2[i]);
+  real_t s = 1.0 / SQRT(2.0);
+  for (int i = 0; i < 3; i++) e.c[i + 1] = s * cd(-real_t(lam) * e1[i], -e2[i]);
   return e;
 }
 static V4 vconj(const V4& a) {
@@ -217,7 +264,7 @@ static V4 vconj(const V4& a) {
 // Parameters
 // ----------------------------------------------------------------------------------------------
 struct Params {
-  double mt, wt, mz, wz, aewm1, gf;
+  real_t mt, wt, mz, wz, aewm1, gf;
 };
 static Params params_from(const double* p) {
   Params q;
@@ -233,27 +280,27 @@ static Params params_from(const double* p) {
 // (alpha, G_F, M_Z) scheme for sin^2 theta_W (reading R5).  The q_mu q_nu / MZ^2 term of the
 // Z propagator vanishes for massless leptons.
 // ----------------------------------------------------------------------------------------------
-static void ew_couplings(const Params& P, double& e, double& gL, double& gR) {
-  const double pi = M_PI;
-  double alpha = 1.0 / P.aewm1;
-  double mz2 = P.mz * P.mz;
-  double mw2 = 0.5 * mz2 + std::sqrt(0.25 * mz2 * mz2 - pi * alpha * mz2 / (std::sqrt(2.0) * P.gf));
-  double sw2 = 1.0 - mw2 / mz2;
-  double sw = std::sqrt(sw2), cw = std::sqrt(1.0 - sw2);
-  e = std::sqrt(4.0 * pi * alpha);
+static void ew_couplings(const Params& P, real_t& e, real_t& gL, real_t& gR) {
+  const real_t pi = M_PI;
+  real_t alpha = 1.0 / P.aewm1;
+  real_t mz2 = P.mz * P.mz;
+  real_t mw2 = 0.5 * mz2 + SQRT(0.25 * mz2 * mz2 - pi * alpha * mz2 / (SQRT(2.0) * P.gf));
+  real_t sw2 = 1.0 - mw2 / mz2;
+  real_t sw = SQRT(sw2), cw = SQRT(1.0 - sw2);
+  e = SQRT(4.0 * pi * alpha);
   gL = e / (sw * cw) * (-0.5 + sw2);
   gR = e / (sw * cw) * sw2;
 }
 static cd amp_eemumu(const Params& P, const double* mom, const int* hel) {
-  double e, gL, gR;
+  real_t e, gL, gR;
   ew_couplings(P, e, gL, gR);
   Sp vb = bar(spinor_v(mom + 0, 0.0, hel[0]));  // incoming e+ : vbar
   Sp u = spinor_u(mom + 4, 0.0, hel[1]);        // incoming e- : u
   Sp v = spinor_v(mom + 8, 0.0, hel[2]);        // outgoing mu+: v
   Sp ub = bar(spinor_u(mom + 12, 0.0, hel[3])); // outgoing mu-: ubar
-  double q[4];
+  real_t q[4];
   for (int i = 0; i < 4; i++) q[i] = mom[i] + mom[4 + i];
-  double s = q[0] * q[0] - q[1] * q[1] - q[2] * q[2] - q[3] * q[3];
+  real_t s = q[0] * q[0] - q[1] * q[1] - q[2] * q[2] - q[3] * q[3];
   M4 gz = chiral_coupling(gL, gR);
   // currents J^mu = vbar gamma^mu X u, computed with unit vectors through slash()
   cd amp(0, 0);
@@ -262,12 +309,12 @@ static cd amp_eemumu(const Params& P, const double* mom, const int* hel) {
     for (int i = 0; i < 4; i++) unit.c[i] = 0.0;
     unit.c[mu] = (mu == 0) ? 1.0 : -1.0;  // slash(unit) = gamma^mu g_{mu mu} * (+-1) -> gamma^mu
     M4 g = slash(unit);
-    double gmm = (mu == 0) ? 1.0 : -1.0;  // metric for the contraction J1^mu J2_mu
+    real_t gmm = (mu == 0) ? 1.0 : -1.0;  // metric for the contraction J1^mu J2_mu
     cd j1g = row_col(vb, times_col(g, u));
     cd j2g = row_col(ub, times_col(g, v));
     cd j1z = row_col(vb, times_col(mmul(g, gz), u));
     cd j2z = row_col(ub, times_col(mmul(g, gz), v));
-    amp += gmm * (e * e * j1g * j2g / s + j1z * j2z / cd(s - P.mz * P.mz, P.mz * P.wz));
+    amp += gmm * (e * e * j1g * j2g / s + cdiv(j1z * j2z, cd(s - P.mz * P.mz, P.mz * P.wz)));
   }
   return amp;
 }
@@ -450,11 +497,11 @@ static void enumerate_lines(Process& P, unsigned remaining, int node, const ColE
 
 // ---- SU(3): Gell-Mann matrices, T^a = lambda^a/2, f^{abc} = -2i Tr([T^a,T^b] T^c) ----
 struct SU3 {
-  cd T[8][3][3];
+  cdd T[8][3][3];
   double f[8][8][8];
   SU3() {
     memset(T, 0, sizeof(T));
-    cd i(0, 1);
+    cdd i(0, 1);
     T[0][0][1] = 1; T[0][1][0] = 1;
     T[1][0][1] = -i; T[1][1][0] = i;
     T[2][0][0] = 1; T[2][1][1] = -1;
@@ -470,12 +517,12 @@ struct SU3 {
     for (int a = 0; a < 8; a++)
       for (int b = 0; b < 8; b++)
         for (int c = 0; c < 8; c++) {
-          cd tr(0, 0);
+          cdd tr(0, 0);
           for (int r = 0; r < 3; r++)
             for (int s = 0; s < 3; s++)
               for (int t = 0; t < 3; t++)
                 tr += (T[a][r][s] * T[b][s][t] - T[b][r][s] * T[a][s][t]) * T[c][t][r];
-          f[a][b][c] = (cd(0, -2) * tr).real();
+          f[a][b][c] = (cdd(0, -2) * tr).real();
         }
   }
 };
@@ -485,13 +532,13 @@ static const SU3& su3() {
 }
 
 struct Mat3 {
-  cd m[3][3];
+  cdd m[3][3];
 };
 static Mat3 m3mul(const Mat3& a, const Mat3& b) {
   Mat3 r;
   for (int i = 0; i < 3; i++)
     for (int j = 0; j < 3; j++) {
-      cd s(0, 0);
+      cdd s(0, 0);
       for (int k = 0; k < 3; k++) s += a.m[i][k] * b.m[k][j];
       r.m[i][j] = s;
     }
@@ -531,7 +578,7 @@ static void build_color_matrix(Process& P) {
       }
       for (int s = 0; s < nc; s++)
         for (int t = 0; t < nc; t++) {
-          cd tr(0, 0);
+          cdd tr(0, 0);
           for (int i = 0; i < 3; i++)
             for (int j = 0; j < 3; j++) tr += str[s].m[i][j] * std::conj(str[t].m[i][j]);
           loc[(size_t)s * nc + t] += tr.real();
@@ -610,11 +657,11 @@ struct Census {
   long v3, v4, chain, closure, jamp_terms;
 };
 
-static void eval_jamps(const Process& P, const Params& par, const double* mom, double gs, int h, int ward_leg,
+static void eval_jamps(const Process& P, const Params& par, const double* mom, real_t gs, int h, int ward_leg,
                        std::vector<cd>& jamp, std::vector<cd>* amps, Census* census) {
   const int npar = P.npar;
   // incoming-convention momenta
-  double k[8][4];
+  real_t k[8][4];
   for (int i = 0; i < npar; i++)
     for (int m = 0; m < 4; m++) k[i][m] = (i < 2 ? 1.0 : -1.0) * mom[4 * i + m];
   // gluon tree currents (upper index, propagator included, colour stripped)
@@ -638,9 +685,9 @@ static void eval_jamps(const Process& P, const Params& par, const double* mom, d
       }
       continue;
     }
-    V4 k3 = vscale(-1.0, K);  // parent line momentum, incoming to this vertex
+    V4 k3 = vscale(cd(-1.0), K);  // parent line momentum, incoming to this vertex
     cd k2 = mdot(K, K);
-    cd prop = -I_ / k2;  // -i g_{mu nu} / k^2
+    cd prop = cdiv(-I_, k2);  // -i g_{mu nu} / k^2
     if (T.kind == 3) {
       const V4 &A = cur[T.ch[0]], &B = cur[T.ch[1]];
       const V4 &k1 = kk[T.ch[0]], &k2v = kk[T.ch[1]];
@@ -674,14 +721,14 @@ static void eval_jamps(const Process& P, const Params& par, const double* mom, d
     // propagator: fermion-arrow momentum q = p_t - (momentum injected so far) = -(k_t + sum_prefix k)
     V4 q;
     for (int m = 0; m < 4; m++) {
-      double s = k[2][m];
+      real_t s = k[2][m];
       for (int i = 0; i < npar; i++)
         if (N.mask & (1u << i)) s += k[i][m];
       q.c[m] = -s;
     }
     cd den = mdot(q, q) - par.mt * par.mt + I_ * par.mt * par.wt;
     Sp y = row_times(x, madd_mass(slash(q), par.mt));
-    for (int i = 0; i < 4; i++) y.c[i] *= I_ / den;
+    for (int i = 0; i < 4; i++) y.c[i] *= cdiv(I_, den);
     chain[n] = y;
     if (census) census->chain++;
   }
@@ -697,11 +744,11 @@ static void eval_jamps(const Process& P, const Params& par, const double* mom, d
   }
 }
 
-// |M_h|^2 = sum_{sigma,tau} conj(J_sigma) C_{sigma tau} J_tau  (plain double sum)
-static double color_sum(const Process& P, const std::vector<cd>& J) {
+// |M_h|^2 = sum_{sigma,tau} conj(J_sigma) C_{sigma tau} J_tau  (plain real_t sum)
+static real_t color_sum(const Process& P, const std::vector<cd>& J) {
   cd s(0, 0);
   for (int a = 0; a < P.ncol; a++)
-    for (int b = 0; b < P.ncol; b++) s += std::conj(J[a]) * P.C[(size_t)a * P.ncol + b] * J[b];
+    for (int b = 0; b < P.ncol; b++) s += std::conj(J[a]) * real_t(P.C[(size_t)a * P.ncol + b]) * J[b];
   return s.real();
 }
 
@@ -761,24 +808,24 @@ int orc_me_helicities(int proc, const double* params, const double* mom, const d
     const double* pm = mom + (size_t)e * npar * 4;
     std::vector<cd> J;
     for (int h = 0; h < ncomb; h++) {
-      double v = 0.0;
+      real_t v = 0.0;
       if (!mask || mask[h]) {
         if (proc == 0) {
           int hel[4];
           for (int k = 0; k < 4; k++) hel[k] = hel_of(h, k, 4);
           cd a = amp_eemumu(par, pm, hel);
-          v = std::norm(a);
-          if (jamp2) jamp2[((size_t)e * ncomb + h) * ncol] = v;
+          v = cnorm(a);
+          if (jamp2) jamp2[((size_t)e * ncomb + h) * ncol] = to_double(v);
         } else {
           eval_jamps(*P, par, pm, gs[e], h, -1, J, 0, 0);
           v = color_sum(*P, J);
           if (jamp2)
-            for (int c = 0; c < ncol; c++) jamp2[((size_t)e * ncomb + h) * ncol + c] = std::norm(J[c]);
+            for (int c = 0; c < ncol; c++) jamp2[((size_t)e * ncomb + h) * ncol + c] = to_double(cnorm(J[c]));
         }
       } else if (jamp2) {
         for (int c = 0; c < ncol; c++) jamp2[((size_t)e * ncomb + h) * ncol + c] = 0.0;
       }
-      mhel[(size_t)e * ncomb + h] = v;
+      mhel[(size_t)e * ncomb + h] = to_double(v);
     }
   }
   return 0;
@@ -793,10 +840,34 @@ int orc_jamps(int proc, const double* params, const double* mom, double gs, int 
   Params par = params_from(params);
   std::vector<cd> J, A;
   eval_jamps(*P, par, mom, gs, h, ward_leg, J, amps ? &A : 0, 0);
-  for (int c = 0; c < P->ncol; c++) { jamp[2 * c] = J[c].real(); jamp[2 * c + 1] = J[c].imag(); }
+  for (int c = 0; c < P->ncol; c++) { jamp[2 * c] = to_double(J[c].real()); jamp[2 * c + 1] = to_double(J[c].imag()); }
   if (amps)
-    for (size_t d = 0; d < A.size(); d++) { amps[2 * d] = A[d].real(); amps[2 * d + 1] = A[d].imag(); }
+    for (size_t d = 0; d < A.size(); d++) { amps[2 * d] = to_double(A[d].real()); amps[2 * d + 1] = to_double(A[d].imag()); }
   return 0;
+}
+
+// Counted mode (BASELINE.json north_star "FLOPs per ME counted by the instrumented oracle"): the
+// arithmetic operations the oracle performs for ONE event over the helicities of mask (NULL = all), every distinct
+// gluon-tree current and quark-line prefix evaluated once per helicity (eval_jamps memoises them), colour sum as the
+// plain double sum.  out4 = {additions+subtractions, multiplications, divisions, square roots}; *me_raw = sum of
+// |M_h|^2 (not divided by denom).  Only the -DORC_COUNT build counts; the plain build returns -2.
+int orc_count_ops(int proc, const double* params, const double* mom, double gs, const uint8_t* mask, long* out4,
+                  double* me_raw) {
+#ifdef ORC_COUNT
+  Process* P = get_process(proc);
+  if (!P) return -1;
+  std::vector<double> mhel(P->ncomb, 0.0);
+  g_ops = OpCount{0, 0, 0, 0};
+  int rc = orc_me_helicities(proc, params, mom, &gs, 1, mask, mhel.data(), 0, 1);
+  out4[0] = g_ops.add; out4[1] = g_ops.mul; out4[2] = g_ops.div; out4[3] = g_ops.sqrt;
+  double s = 0.0;
+  for (int h = 0; h < P->ncomb; h++) s += mhel[h];
+  *me_raw = s;
+  return rc;
+#else
+  (void)proc; (void)params; (void)mom; (void)gs; (void)mask; (void)out4; (void)me_raw;
+  return -2;
+#endif
 }
 
 // operation census of ONE helicity: number of three-/four-gluon currents, quark-line chain steps,
@@ -818,6 +889,7 @@ int orc_census(int proc, long* out5) {
 // explicit-colour brute force for one event and helicity: sum over all 8^n * 9 colour assignments of
 // | sum_d colourtensor_d(a_1..a_n; i, j) A_d |^2, colour tensors built from Gell-Mann matrices and
 // f^{abc} directly (NO trace-basis decomposition, NO colour matrix).  n <= 4.
+#ifndef ORC_COUNT
 int orc_brute_color(int proc, const double* params, const double* mom, double gs, int h, double* out) {
   Process* P = get_process(proc);
   if (!P || proc == 0 || P->ngl > 4) return -1;
@@ -871,7 +943,7 @@ int orc_brute_color(int proc, const double* params, const double* mom, double gs
       Mat3 m;
       for (int i = 0; i < 3; i++)
         for (int j = 0; j < 3; j++) {
-          cd s(0, 0);
+          cdd s(0, 0);
           for (int xx = 0; xx < 8; xx++) s += cv[t][xx] * S.T[xx][i][j];
           m.m[i][j] = s;
         }
@@ -884,7 +956,7 @@ int orc_brute_color(int proc, const double* params, const double* mom, double gs
     for (size_t d = 0; d < P->sub.size(); d++) {
       Mat3 c = m3mul(cm[P->sub[d].prefix], tree_matrix(P->sub[d].last));
       for (int i = 0; i < 3; i++)
-        for (int j = 0; j < 3; j++) M.m[i][j] += c.m[i][j] * A[d];
+        for (int j = 0; j < 3; j++) M.m[i][j] += c.m[i][j] * cdd(to_double(A[d].real()), to_double(A[d].imag()));
     }
     double s = 0.0;
     for (int i = 0; i < 3; i++)
@@ -894,6 +966,7 @@ int orc_brute_color(int proc, const double* params, const double* mom, double gs
   *out = total;
   return 0;
 }
+#endif
 
 // external wavefunctions for the algebra tests.  kind: 0 u, 1 v, 2 ubar, 3 vbar, 4 eps (upper index).
 int orc_wavefunction(int kind, const double* p, double m, int lam, double* out8) {
@@ -904,7 +977,7 @@ int orc_wavefunction(int kind, const double* p, double m, int lam, double* out8)
     if (kind >= 2) s = bar(s);
     for (int i = 0; i < 4; i++) r[i] = s.c[i];
   }
-  for (int i = 0; i < 4; i++) { out8[2 * i] = r[i].real(); out8[2 * i + 1] = r[i].imag(); }
+  for (int i = 0; i < 4; i++) { out8[2 * i] = to_double(r[i].real()); out8[2 * i + 1] = to_double(r[i].imag()); }
   return 0;
 }
 // slash(a) for a complex 4-vector a given as 8 doubles -> 16 complex (32 doubles), row-major
@@ -913,7 +986,7 @@ int orc_slash(const double* a8, double* out32) {
   for (int i = 0; i < 4; i++) a.c[i] = cd(a8[2 * i], a8[2 * i + 1]);
   M4 m = slash(a);
   for (int i = 0; i < 4; i++)
-    for (int j = 0; j < 4; j++) { out32[2 * (4 * i + j)] = m.m[i][j].real(); out32[2 * (4 * i + j) + 1] = m.m[i][j].imag(); }
+    for (int j = 0; j < 4; j++) { out32[2 * (4 * i + j)] = to_double(m.m[i][j].real()); out32[2 * (4 * i + j) + 1] = to_double(m.m[i][j].imag()); }
   return 0;
 }
 int orc_num_threads() {

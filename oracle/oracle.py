@@ -20,21 +20,25 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "me_oracle.cpp")
 _LIB = os.path.join(_HERE, "libme_oracle.so")
+_LIB_COUNT = os.path.join(_HERE, "libme_oracle_count.so")   # same source, -DORC_COUNT (counted mode)
 _lock = threading.Lock()
 _lib = None
+_lib_count = None
 
 PROC_ID = {"ee_mumu": 0, "gg_tt": 1, "gg_ttg": 2, "gg_ttgg": 3, "gg_ttggg": 4}
 DEFAULT_PARAMS = dict(mt=173.0, wt=1.4915, mz=91.188, wz=2.441, aewm1=132.507, gf=1.16639e-5)
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle shared library (g++ -O2 -fopenmp) if missing or stale."""
+    """Compile the oracle shared libraries (g++ -O2 -fopenmp) if missing or stale: the plain one and the
+    operation-counting one (same source with -DORC_COUNT)."""
     with _lock:
-        if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-            tmp = _LIB + ".tmp%d" % os.getpid()
-            cmd = ["g++", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c++14", _SRC, "-o", tmp]
-            subprocess.check_call(cmd)
-            os.replace(tmp, _LIB)
+        for target, extra in ((_LIB, []), (_LIB_COUNT, ["-DORC_COUNT"])):
+            if force or not os.path.exists(target) or os.path.getmtime(target) < os.path.getmtime(_SRC):
+                tmp = target + ".tmp%d" % os.getpid()
+                cmd = ["g++", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c++14"] + extra + [_SRC, "-o", tmp]
+                subprocess.check_call(cmd)
+                os.replace(tmp, target)
     return _LIB
 
 
@@ -227,6 +231,32 @@ def slash(a) -> np.ndarray:
     out = np.zeros(32)
     lib().orc_slash(_dp(a8), _dp(out))
     return (out[0::2] + 1j * out[1::2]).reshape(4, 4)
+
+
+def count_ops(process, momenta1, gs, mask=None, params=None) -> dict:
+    """Counted mode (north_star "FLOPs per ME counted by the instrumented oracle"): the arithmetic
+    operations of the oracle for ONE event over the helicities of mask, from the -DORC_COUNT build of the same
+    source (a double that counts its +,-,*,/ and sqrt).  flops = add + mul + div + sqrt, i.e. FMA = 2."""
+    global _lib_count
+    if _lib_count is None:
+        build()
+        L = ctypes.CDLL(_LIB_COUNT)
+        dp = ctypes.POINTER(ctypes.c_double)
+        L.orc_count_ops.argtypes = [ctypes.c_int, dp, dp, ctypes.c_double, ctypes.c_void_p, ctypes.POINTER(ctypes.c_long), dp]
+        _lib_count = L
+    i = info(process)
+    mom = np.ascontiguousarray(momenta1, dtype=np.float64).reshape(i["npar"], 4)
+    m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    out = (ctypes.c_long * 4)()
+    raw = ctypes.c_double()
+    p = _params(params)
+    rc = _lib_count.orc_count_ops(PROC_ID[process], _dp(p), _dp(mom), float(gs), None if m is None else m.ctypes.data,
+                                  out, ctypes.byref(raw))
+    assert rc == 0
+    d = dict(add=out[0], mul=out[1], div=out[2], sqrt=out[3])
+    d["flops"] = sum(d.values())
+    d["me"] = raw.value / i["denom"]
+    return d
 
 
 def num_threads() -> int:
