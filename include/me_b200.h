@@ -14,8 +14,13 @@
  * Conventions (readings R1-R16)
  *   - all `d_*` arguments are DEVICE pointers owned by the caller (8-byte aligned; int32 outputs 4-byte);
  *     everything else is a HOST pointer.  `stream` is a cudaStream_t passed as void*; work is enqueued
- *     on it and NOT synchronised unless stated.  The library allocates device memory only in
- *     me_create / me_filter_helicities (scratch, freed by me_destroy).
+ *     on it and NOT synchronised unless stated.  The library allocates device memory only in me_create (for
+ *     gg_ttgg / gg_ttggg: ~1 GiB of pipeline scratch holding one chunk of events between the three kernels of the
+ *     path), me_filter_helicities / me_set_good_helicities (selection scratch of the small processes) and
+ *     me_compute_host (staging, grows only); me_destroy frees it.  me_compute never allocates.  Every call makes
+ *     the handle's device current while it runs and restores the caller's current device before returning.
+ *   - one handle serves one stream at a time: calls on the same handle from different streams must not overlap
+ *     on the device (the scratch is per handle); use one handle per stream for concurrency.
  *   - momenta: [nevt][npar][4] doubles, (E, px, py, pz) in GeV, particle order = process string order,
  *     particles 0,1 incoming; for the gg processes 2 = t, 3 = tbar, 4.. = g; for ee_mumu
  *     0 = e+, 1 = e-, 2 = mu+, 3 = mu-.  No special frame is assumed.
@@ -109,8 +114,12 @@ int me_generate(me_handle* h, uint64_t seed, int64_t start, int64_t nevt, double
                 double* d_momenta, double* d_gs, double* d_rndhel, double* d_rndcol, double* d_weight, void* stream);
 
 /* launch geometry of the last me_compute (for reports): threads per block, blocks, registers per thread,
- * bytes of local (spill) memory per thread of the kernel used */
+ * bytes of local (spill) memory per thread of the dominant kernel (gg_ttgg / gg_ttggg: the amplitude kernel) */
 int me_launch_info(const me_handle* h, int* threads, int* blocks, int* regs, int* local_bytes);
+
+/* Kernels enqueued by the last me_compute (3 per chunk for gg_ttgg / gg_ttggg: setup, amplitudes, colour contraction;
+ * 1 otherwise), the events per chunk and the bytes of pipeline scratch the handle owns (0 if it has none) */
+int me_launch_stats(const me_handle* h, int* launches, int64_t* chunk_events, int64_t* scratch_bytes);
 
 /* Measured FMA peak of the device: a register-resident dependent-FMA-chain microbenchmark (best of 5
  * launches of a few ms, synchronous).  precision ME_FP64 or ME_FP32; *tflops receives TFLOP/s with

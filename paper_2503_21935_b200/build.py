@@ -2,8 +2,7 @@
 
     python -m paper_2503_21935_b200.build [--force] [--only gg_ttgg,...] [--verbose]
 
-nvcc cross-compiles without a GPU.  One translation unit per (process, precision) is compiled in
-parallel (the gg_ttggg units are straight-line code of ~10^5 instructions and take minutes).
+nvcc cross-compiles without a GPU.  One translation unit per (process, precision) is compiled in parallel.
 """
 from __future__ import annotations
 
@@ -27,9 +26,9 @@ NVCC_BASE = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", 
 
 # launch configuration per (process, precision): threads per block, min blocks per SM (register cap)
 TUNE = {
-    ("gg_ttggg", 0): (128, 1), ("gg_ttggg", 1): (128, 2), ("gg_ttggg", 2): (128, 1),
-    # lane-group layout: the block size is fixed by the layout, only min blocks/SM (the register cap) is tuned
-    ("gg_ttgg", 0): (64, 4), ("gg_ttgg", 1): (64, 8), ("gg_ttgg", 2): (64, 4),
+    # lane-group pipeline: the amplitude kernel runs one warp per block; min blocks/SM caps its registers
+    ("gg_ttggg", 0): (32, 6), ("gg_ttggg", 1): (32, 12), ("gg_ttggg", 2): (32, 6),
+    ("gg_ttgg", 0): (32, 8), ("gg_ttgg", 1): (32, 16), ("gg_ttgg", 2): (32, 8),
 }
 DEFAULT_TUNE = (128, 1)
 
@@ -41,8 +40,6 @@ def _units():
             defs = [f"-DME_PROC={p}", f"-DME_PROC_UP={p.upper()}", f"-DME_PREC={prec}", f"-DME_NT={nt}", f"-DME_MINB={minb}"]
             if p == "ee_mumu":
                 defs.append("-DME_IS_EE_MUMU")
-            if p == "gg_ttggg":
-                defs.append("-DME_CMAT_GLOBAL=1")
             src = "me_proc_group.cu" if p in GROUP_LAYOUT else "me_proc.cu"
             yield f"{p}_p{prec}", os.path.join(CSRC, src), defs
     yield "api", os.path.join(CSRC, "me_api.cu"), []

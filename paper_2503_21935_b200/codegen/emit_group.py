@@ -90,7 +90,8 @@ class Group:
         gluons in increasing order); a node with path (s1, p1..pk) consumes
           inner node: [path word: slot+sign of Jord(path), subset mask], then Jord(path[j:]) for j = 1..k
           leaf      : Jord(path[j:]) for j = 1..n-1 (the j = 0 block was contracted in the tree phase),
-                      then [flow word: flow index << 16]
+                      then [flow word: flow index << 16 | slot of the contracted full-length current (nslot + its
+                      task index in the top level) | sign of Jord(path) relative to the canonical sequence]
         word bits: 0-7 slot, 8-12 subset mask, 16-22 flow, 31 sign."""
         n = self.n
         others = [i for i in range(n) if i != s1]
@@ -104,7 +105,10 @@ class Group:
             if len(path) == n:
                 for j in range(1, n):
                     out.append(cur_word(path[j:]))
-                out.append((self.flow_index[path] << 16) | (mask_of(path) << 8))
+                can, sgn = canonical(path)
+                init = self.nslot + self.level_seqs[n].index(can)
+                assert init < 256
+                out.append((self.flow_index[path] << 16) | (mask_of(path) << 8) | init | ((1 << 31) if sgn < 0 else 0))
                 return
             out.append(cur_word(path))
             for j in range(1, len(path)):
@@ -136,7 +140,8 @@ class Group:
         o(f"__device__ const unsigned int kGrpRole_{self.name}[] = {{{', '.join(str(x) for x in roles)}}};")
         o(f"struct Grp_{self.name} {{")
         o(f"  static constexpr int n = {n}, npar = {n + 2}, ncomb = {1 << (n + 2)}, ncol = {len(self.flows)}, "
-          f"ndiag = {ndiag}, denom = {denom}, cden = {cmat_den}, nslot = {self.nslot}, nstream = {nstream};")
+          f"ndiag = {ndiag}, denom = {denom}, cden = {cmat_den}, nslot = {self.nslot}, ninit = {len(self.level_seqs[n])}, "
+          f"nstream = {nstream};")
         o("  __device__ __forceinline__ static const unsigned int* level(int L) {")
         o("    switch (L) {")
         for L in range(2, n + 1):

@@ -4,6 +4,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -53,6 +54,9 @@ struct me_handle {
   double* d_cum;
   size_t cum_bytes;
   unsigned long long* d_frac;
+  // lane-group pipeline (gg_ttgg, gg_ttggg): per-event data and jamps between its kernels, one chunk of events
+  void* d_scratch;
+  size_t scratch_bytes;
   // staging for me_compute_host
   void* d_stage;
   size_t stage_bytes;
@@ -104,6 +108,46 @@ int ensure(me_handle* h, void** p, size_t* have, size_t want) {
 
 bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) != 0; }
 
+// Makes the handle's device current for the duration of a call and restores the caller's device on every exit path
+struct DeviceGuard {
+  int prev;
+  cudaError_t err;
+  explicit DeviceGuard(int device) : prev(-1), err(cudaSuccess) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != device) err = cudaSetDevice(device);
+  }
+  ~DeviceGuard() {
+    int now = -1;
+    if (prev >= 0 && cudaGetDevice(&now) == cudaSuccess && now != prev) cudaSetDevice(prev);
+  }
+};
+
+// bytes of pipeline scratch: ME_B200_SCRATCH_MB (for experiments) or 1 GiB
+size_t scratch_target() {
+  const char* s = getenv("ME_B200_SCRATCH_MB");
+  long mb = s ? atol(s) : 0;
+  if (mb < 16) mb = 1024;
+  return (size_t)mb << 20;
+}
+
+// running helicity sums of the one-event-per-thread kernel [ngood][slots]: sized for the full persistent grid once the
+// good-helicity list is known (me_filter_helicities / me_set_good_helicities), so that me_compute never allocates
+int size_cum(me_handle* h) {
+  me::LaunchArgs a;
+  memset(&a, 0, sizeof(a));
+  a.nevt = 1ll << 40;  // geometry of the largest grid
+  a.good = h->good;
+  me::LaunchInfo info;
+  memset(&info, 0, sizeof(info));
+  int ce = h->proc->fn[h->precision](a, me::MODE_SELECT, nullptr, &info, 1);
+  if (ce) return cuda_fail(h, (cudaError_t)ce, "selection scratch geometry");
+  if (info.cum_slots <= 0) return 0;
+  void* p = h->d_cum;
+  int rc = ensure(h, &p, &h->cum_bytes, sizeof(double) * (size_t)h->good.n * (size_t)info.cum_slots);
+  h->d_cum = (double*)p;
+  return rc;
+}
+
 }  // namespace
 
 extern "C" {
@@ -136,12 +180,40 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
   }
   h->have_good = false; h->good.n = 0;
   h->d_cum = nullptr; h->cum_bytes = 0; h->d_frac = nullptr; h->d_stage = nullptr; h->stage_bytes = 0;
+  h->d_scratch = nullptr; h->scratch_bytes = 0;
   h->own_stream = nullptr;
-  h->last = me::LaunchInfo{0, 0, 0, 0, 0};
-  if ((e = cudaSetDevice(device)) != cudaSuccess || (e = cudaMalloc(&h->d_frac, 128 * sizeof(unsigned long long))) != cudaSuccess) {
+  memset(&h->last, 0, sizeof(h->last));
+  DeviceGuard guard(device);
+  if ((e = guard.err) != cudaSuccess || (e = cudaMalloc(&h->d_frac, 128 * sizeof(unsigned long long))) != cudaSuccess) {
     int rc = cuda_fail(nullptr, e, "me_create");
     delete h;
     return rc;
+  }
+  {  // lane-group pipeline: one chunk of scratch, allocated here and never again
+    me::LaunchArgs a;
+    memset(&a, 0, sizeof(a));
+    me::LaunchInfo i0, i1;
+    memset(&i0, 0, sizeof(i0)); memset(&i1, 0, sizeof(i1));
+    int ce = pd->fn[0](a, me::MODE_FILTER, nullptr, &i0, 1);
+    if (!ce) ce = pd->fn[precision](a, me::MODE_SELECT, nullptr, &i1, 1);
+    if (ce) {
+      int rc = cuda_fail(nullptr, (cudaError_t)ce, "me_create: launch geometry");
+      cudaFree(h->d_frac);
+      delete h;
+      return rc;
+    }
+    if (i0.scratch_per_event > 0 || i1.scratch_per_event > 0) {
+      size_t want = scratch_target();
+      const size_t floor_bytes = 64 * (size_t)(i0.scratch_per_event > i1.scratch_per_event ? i0.scratch_per_event : i1.scratch_per_event);
+      if (want < floor_bytes) want = floor_bytes;
+      if ((e = cudaMalloc(&h->d_scratch, want)) != cudaSuccess) {
+        int rc = fail(nullptr, ME_ERR_NOMEM, std::string("me_create: pipeline scratch: ") + cudaGetErrorString(e));
+        cudaFree(h->d_frac);
+        delete h;
+        return rc;
+      }
+      h->scratch_bytes = want;
+    }
   }
   *out = h;
   return ME_OK;
@@ -149,7 +221,8 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
 
 int me_destroy(me_handle* h) {
   if (!h) return ME_ERR_ARG;
-  cudaSetDevice(h->device);
+  DeviceGuard guard(h->device);
+  if (h->d_scratch) cudaFree(h->d_scratch);
   if (h->d_cum) cudaFree(h->d_cum);
   if (h->d_frac) cudaFree(h->d_frac);
   if (h->d_stage) cudaFree(h->d_stage);
@@ -227,7 +300,8 @@ int me_filter_helicities(me_handle* h, const double* d_momenta, const double* d_
   int rc = check_inputs(h, d_momenta, d_gs, nevt, "me_filter_helicities");
   if (rc) return rc;
   if (nevt == 0) return fail(h, ME_ERR_ARG, "me_filter_helicities: needs at least one event");
-  cudaError_t e = cudaSetDevice(h->device);
+  DeviceGuard guard(h->device);
+  cudaError_t e = guard.err;
   if (e != cudaSuccess) return cuda_fail(h, e, "me_filter_helicities");
   cudaStream_t st = (cudaStream_t)stream;
   if ((e = cudaMemsetAsync(h->d_frac, 0, 128 * sizeof(unsigned long long), st)) != cudaSuccess)
@@ -236,6 +310,7 @@ int me_filter_helicities(me_handle* h, const double* d_momenta, const double* d_
   memset(&a, 0, sizeof(a));
   a.mom = d_momenta; a.gs = d_gs; a.nevt = nevt < 16384 ? nevt : 16384;
   a.fracmax = h->d_frac; a.par = h->par;
+  a.scratch = h->d_scratch; a.scratch_bytes = h->scratch_bytes;
   int ce = h->proc->fn[0](a, me::MODE_FILTER, stream, nullptr, 0);  // always the fp64 build (reading R10)
   if (ce) return cuda_fail(h, (cudaError_t)ce, "me_filter_helicities: launch");
   unsigned long long bits[128];
@@ -250,7 +325,7 @@ int me_filter_helicities(me_handle* h, const double* d_momenta, const double* d_
   }
   h->have_good = true;
   if (h->good.n == 0) return fail(h, ME_ERR_NO_HELICITIES, "me_filter_helicities: no helicity passed the filter");
-  return ME_OK;
+  return size_cum(h);
 }
 
 int me_get_good_helicities(const me_handle* h, int* ngood, uint8_t* mask) {
@@ -273,7 +348,9 @@ int me_set_good_helicities(me_handle* h, const uint8_t* mask) {
   for (int r = 0; r < h->ncomb; r++)
     if (mask[r]) h->good.h[h->good.n++] = (uint8_t)r;
   h->have_good = true;
-  return ME_OK;
+  DeviceGuard guard(h->device);
+  if (guard.err != cudaSuccess) return cuda_fail(h, guard.err, "me_set_good_helicities");
+  return size_cum(h);
 }
 
 int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const double* d_rndhel,
@@ -288,12 +365,13 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
   if ((d_selhel && !d_rndhel) || (d_selcol && !d_rndcol))
     return fail(h, ME_ERR_ARG, "me_compute: a selection output needs its random-number input");
   if (nevt == 0) return ME_OK;
-  cudaError_t e = cudaSetDevice(h->device);
-  if (e != cudaSuccess) return cuda_fail(h, e, "me_compute");
+  DeviceGuard guard(h->device);
+  if (guard.err != cudaSuccess) return cuda_fail(h, guard.err, "me_compute");
   me::LaunchArgs a;
   memset(&a, 0, sizeof(a));
   a.mom = d_momenta; a.gs = d_gs; a.rndhel = d_rndhel; a.rndcol = d_rndcol; a.nevt = nevt;
   a.me = d_me; a.selhel = d_selhel; a.selcol = d_selcol; a.par = h->par; a.good = h->good;
+  a.scratch = h->d_scratch; a.scratch_bytes = h->scratch_bytes;
   a.good.mask[0] = a.good.mask[1] = 0ull;
   for (int i = 0; i < a.good.n; i++) a.good.mask[a.good.h[i] >> 6] |= 1ull << (a.good.h[i] & 63);
   const int mode = (d_selhel || d_selcol) ? me::MODE_SELECT : me::MODE_ME;
@@ -302,12 +380,9 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
   int ce = fn(a, mode, stream, &info, 1);
   if (ce) return cuda_fail(h, (cudaError_t)ce, "me_compute: launch geometry");
   if (mode == me::MODE_SELECT && info.cum_slots > 0) {
-    // running helicity sums [ngood][slots]; grows only when a larger grid is seen (no steady-state allocation)
-    size_t want = sizeof(double) * (size_t)h->good.n * (size_t)info.cum_slots;
-    void* p = h->d_cum;
-    rc = ensure(h, &p, &h->cum_bytes, want);
-    h->d_cum = (double*)p;
-    if (rc) return rc;
+    // running helicity sums [ngood][slots], sized by me_filter_helicities / me_set_good_helicities
+    if (sizeof(double) * (size_t)h->good.n * (size_t)info.cum_slots > h->cum_bytes)
+      return fail(h, ME_ERR_ARG, "me_compute: selection scratch smaller than the grid (internal)");
     a.cum = h->d_cum;
   }
   a.blocks = info.blocks;
@@ -323,7 +398,8 @@ int me_compute_host(me_handle* h, const double* momenta, const double* gs, const
   if (nevt < 0) return fail(h, ME_ERR_ARG, "me_compute_host: nevt < 0");
   if (nevt == 0) return ME_OK;
   if (!momenta || !me_out || (h->proc->ngl && !gs)) return fail(h, ME_ERR_ARG, "me_compute_host: null pointer");
-  cudaError_t e = cudaSetDevice(h->device);
+  DeviceGuard guard(h->device);
+  cudaError_t e = guard.err;
   if (e != cudaSuccess) return cuda_fail(h, e, "me_compute_host");
   if (!h->own_stream && (e = cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking)) != cudaSuccess)
     return cuda_fail(h, e, "me_compute_host: stream");
@@ -372,8 +448,8 @@ int me_generate(me_handle* h, uint64_t seed, int64_t start, int64_t nevt, double
   double msum = 0.0;
   for (int i = 0; i < nfin; i++) { a.mass[i] = (h->proc->ngl && i < 2) ? h->par.mt : 0.0; msum += a.mass[i]; }
   if (!(msum < sqrts)) return fail(h, ME_ERR_ARG, "me_generate: sqrts below the mass threshold");
-  cudaError_t e = cudaSetDevice(h->device);
-  if (e != cudaSuccess) return cuda_fail(h, e, "me_generate");
+  DeviceGuard guard(h->device);
+  if (guard.err != cudaSuccess) return cuda_fail(h, guard.err, "me_generate");
   int ce = me::launch_rambo(a, nfin, (unsigned long long)seed, stream);
   if (ce) return cuda_fail(h, (cudaError_t)ce, "me_generate: launch");
   return ME_OK;
@@ -385,6 +461,14 @@ int me_launch_info(const me_handle* h, int* threads, int* blocks, int* regs, int
   if (blocks) *blocks = h->last.blocks;
   if (regs) *regs = h->last.regs;
   if (local_bytes) *local_bytes = h->last.local_bytes;
+  return ME_OK;
+}
+
+int me_launch_stats(const me_handle* h, int* launches, int64_t* chunk_events, int64_t* scratch_bytes) {
+  if (!h) return ME_ERR_ARG;
+  if (launches) *launches = h->last.launches;
+  if (chunk_events) *chunk_events = h->last.chunk;
+  if (scratch_bytes) *scratch_bytes = (int64_t)h->scratch_bytes;
   return ME_OK;
 }
 

@@ -1,21 +1,31 @@
-// me_group.cuh -- the "lane-group" event kernel (layout B2) for g g -> t tbar + (n-2) g, n >= 4.
+// me_group.cuh -- the "lane-group" pipeline (layout B2) for g g -> t tbar + (n-2) g, n >= 4: three kernels per chunk
+// of events, the amplitudes on the FMA pipes and the colour contraction on the tensor cores.
 //
-// One CUDA block per event.  A GROUP of LPG lanes of one warp owns one combination of the n gluon helicities
-// (n = 4: 4 lanes, one per first gluon s1 of the colour flow, both t helicities walked by the same lane; n = 5:
-// 10 lanes (s1, h_t)); the four (h_t, h_tbar) combinations are handled inside the group, so the gluon currents
-// are computed once per gluon-helicity combination instead of once per helicity.
-// Per event the block first forms the helicity-independent data in shared memory (one branch-free phase, one
-// block barrier); then every group runs, warp-synchronously:
-//   leaves  lane i < n      : polarisation vector of gluon i (a2)                       -> shared memory slot
-//   tree    lane = sequence : colour-ordered currents Jord(seq), |seq| = 2..n-1 (a3)    -> shared memory slot
-//           |seq| = n       : contracted at once with the four t-tbar currents Q(h_t,h_tbar) -> J init (a4, a5)
-//   walk    lane = s1       : quark line for the flows that start with gluon s1 (a3-a5) -> J[flow][h_t][h_tbar]
-//   colour  task = (h_t,h_tbar[,re/im]): x^T C x over the n! flows (a6)                 -> |M_h|^2
-// and one warp sums the good helicities in table order (a7), selects helicity / colour (a8) and stores (a9).
-// Current operands of the walk are read from shared memory with 16-byte loads (the lanes of a quarter-warp read
-// different slots: chunk-swizzled in the fp64 build) and feed both t helicities; the running spinors stay in
-// registers.  fp32 build: the two t-helicity chains, the complex arithmetic of the tree vertices and the colour
-// sum are packed f32x2 operations (FFMA2).  DESIGN.md section 5 has the measured history of these choices.
+//   K0 setup_kernel   a1 + the helicity-independent part of a2/a3: momentum sums per gluon subset,
+//                     1/K^2, quark-line denominators (formed in fp64 from pairwise invariants, whatever the build),
+//                     polarisation / spinor bases, the four t-tbar currents Q(h_t,h_tbar) -> GrpEvent[event] in HBM.
+//   K1 amp_kernel     a2-a5.  One WARP per (event, unit); a GROUP of LPG lanes owns one combination of the n gluon
+//                     helicities (n = 4: 4 lanes, one per first gluon s1 of the colour flow, both t helicities walked
+//                     by the same lane; n = 5: 10 lanes (s1, h_t)), so the gluon currents are computed once per
+//                     gluon-helicity combination and shared by the four (h_t, h_tbar) rows.  Warp-synchronous:
+//                       leaves  lane i < n      : polarisation vector of gluon i                    -> shared-memory slot
+//                       tree    lane = sequence : colour-ordered currents Jord(seq), |seq| = 2..n-1 -> shared-memory slot
+//                               |seq| = n       : contracted at once with the four Q               -> "init" slot
+//                       walk    lane = s1       : quark line for the flows that start with gluon s1; at the leaf of
+//                               flow sigma  J_sigma = init + Psi.v  goes straight to HBM as X[event][combination][8][LD]
+//                               (row = 2 (2 h_t + h_tbar) + re/im, column = flow): the jamps never sit in shared memory.
+//   K2 colour_kernel  a6-a9.  One warp per event.  Per gluon-helicity combination the colour sum of its 8 real
+//                     vectors is the contraction  q_m = sum_ab X[m][a] C[a][b] X[m][b]  = [8 x ncol] . [ncol x ncol]
+//                     followed by a row dot: tensor-core MMAs with C in shared memory in fragment order, only the
+//                     upper triangle of 8 x 8 tiles (diagonal tiles halved, result doubled: C is symmetric).
+//                       fp64 build        : mma.sync m8n8k4 f64 (DMMA)
+//                       fp32 / mixed build: mma.sync m16n8k8 tf32, two combinations per tile, X split into
+//                                           hi + lo TF32 parts (the integer colour numerators are exact in TF32), so
+//                                           the products carry fp32 accuracy and the sum accumulates in fp32
+//                     then |M_h|^2 per helicity row, the helicity sum in table order (a7), helicity / colour selection
+//                     (a8) and the stores (a9).
+// The fp32 build packs the two h_t chains of the walk, the complex arithmetic of the tree vertices into f32x2
+// operations (FFMA2).  DESIGN.md section 5 has the measured history of these choices.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -49,21 +59,7 @@ template <> struct WalkPack<float, true> {
   __device__ __forceinline__ static PS widen(float x) { return mkf2(x, x); }
 };
 
-template <typename T, typename TC, int N>
-struct alignas(16) GrpEvent {
-  double mh[1 << (N + 2)];     // |M_h|^2 (colour-summed, un-normalised) per helicity row
-  alignas(16) T Ksub[1 << N][4];           // sum of the gluon momenta of a subset (bit i = gluon i)
-  alignas(16) T qsub[1 << N][4];           // -(k_t + K_S): momentum of the quark line after the gluons of S
-  T gd[1 << N][2];             // 1 / (q^2 - m^2 + i m Gamma)
-  T ik[1 << N];                // 1 / K_S^2
-  alignas(16) T Q[4][8];                   // ubar(h_t) gamma^mu v(h_tbar), index 2 h_t + h_tbar
-  alignas(16) T ub[2][8];
-  alignas(16) T v[2][8];
-  T pol[N][6];
-  T mt;
-  TC wc[5][(N == 4) ? 24 : (N == 5 ? 120 : 6)];  // per-warp colour weights (at most 4 warps per block)
-  unsigned char gmask[1 << N];  // per gluon-helicity combination: bit v set iff helicity row (combination, v) is good
-};
+
 
 template <typename T> struct GrpVec;
 template <> struct GrpVec<double> {
@@ -268,10 +264,24 @@ __device__ __forceinline__ void v4_acc(vec4<float>& acc, const vec4<float>& A, c
   }
 }
 
+
+// Helicity-independent data of one event: written by setup_kernel (K0) to HBM, staged in shared memory by the warp
+// that evaluates a unit of the event (K1).
+template <typename T, int N>
+struct alignas(16) GrpEvent {
+  alignas(16) T Ksub[1 << N][4];  // sum of the gluon momenta of a subset (bit i = gluon i)
+  alignas(16) T qsub[1 << N][4];  // -(k_t + K_S): momentum of the quark line after the gluons of S
+  T gd[1 << N][2];                // 1 / (q^2 - m^2 + i m Gamma)
+  T ik[1 << N];                   // 1 / K_S^2
+  alignas(16) T Q[4][8];          // ubar(h_t) gamma^mu v(h_tbar), index 2 h_t + h_tbar
+  alignas(16) T ub[2][8];
+  alignas(16) T v[2][8];
+  T pol[N][6];
+  T mt;
+};
+
 template <class G, typename T>
 struct GrpGeom {
-  // NGRP combinations per event, processed NPASS groups at a time (n = 4: all 16 at once; n = 5: shared memory
-  // holds 12 of the 32)
   // HTL: both t helicities are walked by the same lane (every current loaded from shared memory feeds two
   // quark-line products); otherwise lanes are (s1, h_t) pairs
 #ifdef ME_HTL
@@ -280,19 +290,147 @@ struct GrpGeom {
   static constexpr bool HTL = (G::n <= 4);
 #endif
   static constexpr int N = G::n, NHT = HTL ? 2 : 1, LPG = HTL ? N : 2 * N, GPW = 32 / LPG, NGRP = 1 << N;
-  static constexpr int NPASS = (N <= 4) ? NGRP : 12;
-  static constexpr int NW = (NPASS + GPW - 1) / GPW, NT = NW * 32;
-  // T units per group: current slots + J[ncol][4][2]; padded so that the byte stride is 32 mod 128
-  static constexpr int RAW = (G::nslot + G::ncol) * 8;
+  // T units per group: current slots + contracted full-length currents ("init"); padded so that the byte stride
+  // is 32 mod 128
+  static constexpr int RAW = (G::nslot + G::ninit) * 8;
   static constexpr int UNIT = 32 / (int)sizeof(T);  // T units in 32 bytes
   static constexpr int GS = ((RAW + 4 * UNIT - 1) / (4 * UNIT)) * (4 * UNIT) + UNIT;
+  static constexpr int EVB = (((int)sizeof(GrpEvent<T, G::n>) + 127) / 128) * 128;
+  static constexpr int SMEM = EVB + GPW * GS * (int)sizeof(T);
 };
 
+// Layout of the jamps in HBM between K1 and K2: X[event][listed combination][8][LD], row m = 2 (2 h_t + h_tbar) +
+// re/im, column = colour flow.  LD = ncol + 4 makes the row stride 96 mod 128 bytes (fp64) / 112 mod 128 (fp32): the
+// MMA A-fragment loads of K2 (8 rows x 4 consecutive columns) are free of bank conflicts.
+template <class G> struct XGeom {
+  static constexpr int NCOL = G::ncol, LD = NCOL + 4, NT = NCOL / 8, NPAIR = NT * (NT + 1) / 2;
+  static_assert(NCOL % 8 == 0 && LD % 16 == 12, "tile geometry");
+};
+
+// Arguments of the three kernels of one chunk of events (pointers already offset to the chunk)
+struct PipeArgs {
+  LaunchArgs a;
+  void* ev;                  // GrpEvent<T, N>[nevt]
+  void* xt;                  // TC[nevt][ncombo][8][LD] (+ one group of slack)
+  int ncombo;                // gluon-helicity combinations with at least one good helicity row
+  unsigned char combo[32];   // ... in increasing order
+  unsigned char vmask[32];   // per listed combination: bit v = 2 h_t + h_tbar set iff that helicity row is good
+};
+
+// helicity row of gluon-helicity combination gg (bit N-1-i = gluon i) and variant v = 2 h_t + h_tbar
+template <int N> __host__ __device__ __forceinline__ int grp_hel_of(int gg, int v) {
+  constexpr int NPAR = N + 2;
+  int h = 0;
+#pragma unroll
+  for (int i = 0; i < N; i++) {
+    const int p = (i < 2) ? i : i + 2;
+    h |= ((gg >> (N - 1 - i)) & 1) << (NPAR - 1 - p);
+  }
+  h |= (v >> 1) << (NPAR - 1 - 2);
+  h |= (v & 1) << (NPAR - 1 - 3);
+  return h;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// K0: per event, helicity-independent data.  Thread = (event, task); tasks: one per gluon subset, one per gluon
+// (polarisation basis), six for the quark line (ubar(t), v(tbar), the four Q).  Every task reads the momenta it needs
+// from global memory (incoming convention: +p for the initial, -p for the final state).
+// ------------------------------------------------------------------------------------------------------------------
+template <typename T, int N>
+__global__ void __launch_bounds__(128) setup_kernel(const LaunchArgs a, GrpEvent<T, N>* __restrict__ evs) {
+  constexpr int NPAR = N + 2, NSUB = 1 << N, NTASK = NSUB + N + 6, PT = (NTASK <= 32) ? 32 : 64;
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long e = gid / PT;
+  const int task = (int)(gid % PT);
+  if (e >= a.nevt || task >= NTASK) return;
+  GrpEvent<T, N>& ev = evs[e];
+  const double* pm = a.mom + e * (NPAR * 4);
+  auto kd = [&](int p, int c) { const double x = __ldg(pm + 4 * p + c); return (p < 2) ? x : -x; };
+  const double mw = a.par.mt * a.par.wt;
+  if (task < NSUB) {
+    // gluon subset m: momentum sum, quark-line momentum after it, 1/K^2, quark-line denominator; invariants from
+    // pairwise products 2 k_i.k_j in fp64 (never (sum k)^2, which cancels for collinear / soft gluons).
+    // Branch-free: members are picked with 0/1 factors (exact)
+    const int m = task;
+    double kg[N][4], kt[4];
+#pragma unroll
+    for (int i = 0; i < N; i++)
+#pragma unroll
+      for (int c = 0; c < 4; c++) kg[i][c] = kd((i < 2) ? i : i + 2, c);
+#pragma unroll
+    for (int c = 0; c < 4; c++) kt[c] = kd(2, c);
+    double k[4] = {0.0, 0.0, 0.0, 0.0}, pairs = 0.0, line = 0.0;
+#pragma unroll
+    for (int i = 0; i < N; i++) {
+      const double bi = ((m >> i) & 1) ? 1.0 : 0.0;
+#pragma unroll
+      for (int c = 0; c < 4; c++) k[c] += bi * kg[i][c];
+      line += bi * 2.0 * (kt[0] * kg[i][0] - kt[1] * kg[i][1] - kt[2] * kg[i][2] - kt[3] * kg[i][3]);
+#pragma unroll
+      for (int j = i + 1; j < N; j++) {
+        const double bj = ((m >> j) & 1) ? bi : 0.0;
+        pairs += bj * 2.0 * (kg[i][0] * kg[j][0] - kg[i][1] * kg[j][1] - kg[i][2] * kg[j][2] - kg[i][3] * kg[j][3]);
+      }
+    }
+    const int cnt = __popc(m);
+    for (int c = 0; c < 4; c++) {
+      ev.Ksub[m][c] = T(k[c]);
+      ev.qsub[m][c] = T(-(kt[c] + k[c]));
+    }
+    ev.ik[m] = (cnt >= 2) ? T(1.0 / pairs) : T(0);
+    const double den = line + pairs, nrm = 1.0 / (den * den + mw * mw);
+    ev.gd[m][0] = (cnt >= 1) ? T(den * nrm) : T(0);
+    ev.gd[m][1] = (cnt >= 1) ? T(-mw * nrm) : T(0);
+    if (m == 0) ev.mt = T(a.par.mt);
+  } else if (task < NSUB + N) {
+    const int i = task - NSUB, p = (i < 2) ? i : i + 2;
+    mom4<T> k;
+    for (int c = 0; c < 4; c++) k.c[c] = T(kd(p, c));
+    const polbasis<T> pb = make_polbasis<T>((p < 2) ? k : neg(k));
+    for (int c = 0; c < 3; c++) { ev.pol[i][c] = pb.e1[c]; ev.pol[i][3 + c] = pb.e2[c]; }
+  } else {
+    // tasks 0,1: ubar(t), v(tbar) for both helicities; tasks 2..5: Q(h_t, h_tbar) = ubar gamma^mu v
+    const int w = task - NSUB - N;
+    spin4<T> ub[2], vv[2];
+#pragma unroll
+    for (int which = 0; which < 2; which++) {
+      mom4<T> k;
+#pragma unroll
+      for (int c = 0; c < 4; c++) k.c[c] = T(-kd(2 + which, c));
+      const spinbasis<T> sb = make_spinbasis<T>(k, T(a.par.mt));
+#pragma unroll
+      for (int l = 0; l < 2; l++) {
+        if (which) vv[l] = spinor_v(sb, l ? 1 : -1);
+        else ub[l] = bar(spinor_u(sb, l ? 1 : -1));
+      }
+    }
+    if (w < 2) {
+#pragma unroll
+      for (int l = 0; l < 2; l++) {
+        T* o = w ? ev.v[l] : ev.ub[l];
+#pragma unroll
+        for (int c = 0; c < 4; c++) {
+          o[2 * c] = w ? vv[l].c[c].re : ub[l].c[c].re;
+          o[2 * c + 1] = w ? vv[l].c[c].im : ub[l].c[c].im;
+        }
+      }
+    } else {
+      const int v = w - 2;
+      vec4<T> JR, JL;
+      chiral_currents(select((v >> 1) != 0, ub[1], ub[0]), select((v & 1) != 0, vv[1], vv[0]), JR, JL);
+      for (int c = 0; c < 4; c++) { ev.Q[v][2 * c] = JR.c[c].re + JL.c[c].re; ev.Q[v][2 * c + 1] = JR.c[c].im + JL.c[c].im; }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// K1 pieces
+// ------------------------------------------------------------------------------------------------------------------
 // Colour-ordered gluon currents of one group, level by level (|seq| = 2 .. n).  One copy of the vertex code: the
 // levels, the tasks of a level and the terms of a task are run-time loops over the generated tables (keeps the
 // kernel small enough for the instruction cache; the loop bodies are ~100 FMA-pipe instructions each).
-template <class G, typename T, typename TC>
-__device__ __forceinline__ void grp_tree(const GrpEvent<T, TC, G::n>& ev, T* slots, T* J, int r, bool active) {
+template <class G, typename T>
+__device__ __forceinline__ void grp_tree(const GrpEvent<T, G::n>& ev, T* slots, int r, bool active) {
   constexpr int LPG = GrpGeom<G, T>::LPG;
 #pragma unroll 1
   for (int L = 2; L <= G::n; L++) {
@@ -328,18 +466,14 @@ __device__ __forceinline__ void grp_tree(const GrpEvent<T, TC, G::n>& ev, T* slo
         if (!TOP) {
           GrpSlot<T>::st(slots, h0 & 255u, acc);
         } else {
-          // the full-length current is contracted at once with the four t-tbar currents: initial J of the flow
-          // and of its reverse
-          const unsigned h1 = __ldg(tw + 1);
-          T* ja = J + (h1 & 127u) * 8;
-          T* jb = J + ((h1 >> 8) & 127u) * 8;
-          const T sb = (h1 >> 31) ? T(-1) : T(1);
+          // the full-length current is contracted at once with the four t-tbar currents: the j = 0 term of the
+          // jamps of this sequence and of its reverse ("init" slot t, read by the leaves of the walk)
+          T* ji = slots + (G::nslot + t) * 8;
 #pragma unroll
           for (int v = 0; v < 4; v++) {
             const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
             const cx<T> a = mdot(q, acc);
-            ja[2 * v] = a.re; ja[2 * v + 1] = a.im;
-            jb[2 * v] = sb * a.re; jb[2 * v + 1] = sb * a.im;
+            ji[2 * v] = a.re; ji[2 * v + 1] = a.im;
           }
         }
       }
@@ -348,13 +482,13 @@ __device__ __forceinline__ void grp_tree(const GrpEvent<T, TC, G::n>& ev, T* slo
   }
 }
 
-// Quark-line walk of lane (s1, h_t): depth-first loop nest over the gluons that follow s1.  The words are read
+// Quark-line walk of lane (s1[, h_t]): depth-first loop nest over the gluons that follow s1.  The words are read
 // in execution order from the role's stream (emit_group.py role_stream); psi[j] = Psi(path[:j]) stays in registers.
 template <class G, typename T, typename TC>
 struct GrpWalkCtx {
-  const GrpEvent<T, TC, G::n>* ev;
+  const GrpEvent<T, G::n>* ev;
   const T* slots;
-  T* J;
+  TC* X;  // jamps of this group in HBM: [8][LD]
   const unsigned* stream;
   int ht;
   __device__ __forceinline__ unsigned next() { return __ldg(stream++); }
@@ -384,16 +518,24 @@ struct GrpWalkCtx {
   }
   __device__ __forceinline__ static f2 pack(float x, float y) { return mkf2(x, y); }
   __device__ __forceinline__ static double pack(double x, double) { return x; }
-  // Psi = X (qslash + m) / (q^2 - m^2 + i m Gamma) after the gluons of word w; q, the denominator and m are shared
-  __device__ __forceinline__ static void addto(T* j, int h, int b, f2 re, f2 im) {
-    j[0 * 4 + 2 * b] += re.v.x; j[0 * 4 + 2 * b + 1] += im.v.x;
-    j[1 * 4 + 2 * b] += re.v.y; j[1 * 4 + 2 * b + 1] += im.v.y;
+  // J_flow(h_t, b) = sg * init + a  ->  X[2 (2 h_t + b) + re/im][flow]
+  __device__ __forceinline__ void put(const T* ji, T sg, int f, int h, int b, f2 re, f2 im) const {
+    constexpr int LD = XGeom<G>::LD;
+    X[(2 * b) * LD + f] = TC(fmaf(sg, ji[2 * b], re.v.x));              // h_t = 0: v = b
+    X[(2 * b + 1) * LD + f] = TC(fmaf(sg, ji[2 * b + 1], im.v.x));
+    X[(4 + 2 * b) * LD + f] = TC(fmaf(sg, ji[4 + 2 * b], re.v.y));      // h_t = 1: v = 2 + b
+    X[(5 + 2 * b) * LD + f] = TC(fmaf(sg, ji[5 + 2 * b], im.v.y));
   }
-  template <typename S> __device__ __forceinline__ static void addto(T* j, int h, int b, S re, S im) {
-    j[h * 4 + 2 * b] += re; j[h * 4 + 2 * b + 1] += im;
+  template <typename S> __device__ __forceinline__ void put(const T* ji, T sg, int f, int h, int b, S re, S im) const {
+    constexpr int LD = XGeom<G>::LD;
+    const int v = 2 * h + b;
+    X[(2 * v) * LD + f] = TC(fmad<T>(sg, ji[2 * v], re));
+    X[(2 * v + 1) * LD + f] = TC(fmad<T>(sg, ji[2 * v + 1], im));
   }
-  __device__ __forceinline__ void leaf(const spin4<PS> (&X)[WP::NCH], unsigned w) const {
-    T* j = J + ((w >> 16) & 127u) * 8;
+  __device__ __forceinline__ void leaf(const spin4<PS> (&Xs)[WP::NCH], unsigned w) const {
+    const int f = (w >> 16) & 127;
+    const T* ji = slots + (w & 255u) * 8;
+    const T sg = (w >> 31) ? T(-1) : T(1);
 #pragma unroll
     for (int b = 0; b < 2; b++) {
       const spin4<T> vb = ld_spin<T>(ev->v[b]);
@@ -402,8 +544,8 @@ struct GrpWalkCtx {
       for (int i = 0; i < 4; i++) vw.c[i] = mk<PS>(WP::widen(vb.c[i].re), WP::widen(vb.c[i].im));
 #pragma unroll
       for (int c = 0; c < WP::NCH; c++) {
-        const cx<PS> a = row_col(X[c], vw);
-        addto(j, GrpGeom<G, T>::HTL ? c : ht, b, a.re, a.im);
+        const cx<PS> a = row_col(Xs[c], vw);
+        put(ji, sg, f, GrpGeom<G, T>::HTL ? c : ht, b, a.re, a.im);
       }
     }
   }
@@ -465,27 +607,63 @@ struct GrpWalk<G, T, TC, G::n> {
   }
 };
 
-// x^T C x for the real vector x_a = J[a*8 + off] (a < ncol), C = integer numerators CM::at (symmetric)
-template <int NCOL, typename T, typename TC, class CM>
-__device__ __forceinline__ TC grp_quadform(const T* J, int off, TC* x2 /*[NCOL] += x_a^2 or nullptr*/, TC keep) {
-  static_assert(NCOL <= 24, "register-resident form (120 flows: the row-split loop of the kernel)");
-  TC s = TC(0);
+// ------------------------------------------------------------------------------------------------------------------
+// K1: one warp per (event, unit); a unit is GPW listed gluon-helicity combinations, one per lane group.
+// ------------------------------------------------------------------------------------------------------------------
+template <class G, typename T, typename TC, int MINB>
+__global__ void __launch_bounds__(32, MINB) amp_kernel(const PipeArgs p) {
+  typedef GrpGeom<G, T> GE;
+  constexpr int N = G::n, LPG = GE::LPG, GPW = GE::GPW, LD = XGeom<G>::LD;
+  typedef GrpEvent<T, N> EV;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  EV& ev = *reinterpret_cast<EV*>(smem_raw);
+  T* gbase = reinterpret_cast<T*>(smem_raw + GE::EVB);
+  const int lane = threadIdx.x;
+  const int gi = lane / LPG, r = lane - gi * LPG;
+  const int nunit = (p.ncombo + GPW - 1) / GPW;
+  const long long e = blockIdx.x / nunit;
+  const int unit = (int)(blockIdx.x - e * nunit);
+  T* slots = gbase + (size_t)((gi < GPW) ? gi : 0) * GE::GS;
+  // ---- a1: the event's helicity-independent data (K0), HBM -> shared memory, 16 bytes per lane and step
   {
-    TC x[NCOL];
-#pragma unroll
-    for (int a = 0; a < NCOL; a++) x[a] = TC(J[a * 8 + off]);
-#pragma unroll
-    for (int a = 0; a < NCOL; a++) {
-      TC y = TC(0.5) * CM::at(a * NCOL + a) * x[a];
-#pragma unroll
-      for (int b = a + 1; b < NCOL; b++) y += CM::at(a * NCOL + b) * x[b];
-      s += x[a] * y;
-      if (x2) x2[a] += keep * x[a] * x[a];
-    }
+    const int4* src = reinterpret_cast<const int4*>(reinterpret_cast<const EV*>(p.ev) + e);
+    int4* dst = reinterpret_cast<int4*>(&ev);
+#pragma unroll 4
+    for (int i = lane; i < (int)(sizeof(EV) / 16); i += 32) dst[i] = __ldg(src + i);
   }
-  return TC(2) * s;
+  __syncwarp();
+  const int ci = unit * GPW + gi;                       // position in the list of combinations
+  const bool active = (gi < GPW) && (ci < p.ncombo);
+  const int grp = p.combo[active ? ci : 0];             // gluon-helicity combination
+  // ---- a2: polarisation vectors of this group's gluon helicities
+  if (active && r < N) {
+    const int pp = (r < 2) ? r : r + 2;
+    const int lam = ((grp >> (N - 1 - r)) & 1) ? 1 : -1;
+    polbasis<T> pb;
+    for (int c = 0; c < 3; c++) { pb.e1[c] = ev.pol[r][c]; pb.e2[c] = ev.pol[r][3 + c]; }
+    GrpSlot<T>::st(slots, r, polvec(pb, lam, pp >= 2));
+  }
+  __syncwarp();
+  // ---- a3: colour-ordered gluon currents, level by level; the full-length ones are contracted with Q
+  grp_tree<G, T>(ev, slots, r, active);
+  // ---- a3-a5: quark line; every leaf completes one jamp and stores it
+  if (active) {
+    typedef GrpWalkCtx<G, T, TC> Ctx;
+    Ctx c;
+    c.ev = &ev; c.slots = slots;
+    c.X = reinterpret_cast<TC*>(p.xt) + ((size_t)e * p.ncombo + ci) * (8 * LD);
+    c.stream = G::role(GE::HTL ? r : (r >> 1));
+    c.ht = GE::HTL ? 0 : (r & 1);
+    spin4<typename Ctx::PS> psi[Ctx::WP::NCH][G::n];
+#pragma unroll
+    for (int h = 0; h < Ctx::WP::NCH; h++) psi[h][0] = c.psi0(h);
+    GrpWalk<G, T, TC, 1>::node(c, psi);
+  }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// K2 pieces
+// ------------------------------------------------------------------------------------------------------------------
 // One warp: in-order cumulative sums of PER consecutive values per lane (index = lane * PER + i; val = 0 where
 // !ok), their total, and the selection of reading R11: first index with rnd * total < cumulative sum, else the last
 // ok index.  Every lane returns the same total and sel.
@@ -515,373 +693,273 @@ __device__ __forceinline__ void grp_warp_select(const double (&val)[PER], const 
   else sel = bo ? __shfl_sync(0xffffffffu, lastok, 31 - __clz(bo)) : 0;
 }
 
-// float colour sum of one variant (h_t, h_tbar) with the real and imaginary parts of J as one packed f32x2 pair
-// (inline PTX on 64-bit registers: arrays of them unroll like scalars, arrays of float2 through the builtins did
-// not): returns Re(J^dagger C J) = x^T C x + y^T C y for J = x + i y, J_a at J[a*8 + 2*v .. +1]
-__device__ __forceinline__ unsigned long long pk2(float x, float y) {
-  unsigned long long r;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y));
-  return r;
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
 }
-__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
-  unsigned long long r;
-  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
-  return r;
-}
-__device__ __forceinline__ unsigned long long mul2(unsigned long long a, unsigned long long b) {
-  unsigned long long r;
-  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-  return r;
-}
-template <int NCOL, typename T, class CM>
-__device__ __forceinline__ float grp_quadform_pk(const T* J, int v, float* x2 /*[NCOL] += |J_a|^2 or nullptr*/, float keep) {
-  static_assert(NCOL <= 24, "register-resident form");
-  unsigned long long x[NCOL];
-  float xr[NCOL], xi[NCOL];
-#pragma unroll
-  for (int a = 0; a < NCOL; a++) {
-    xr[a] = float(J[a * 8 + 2 * v]); xi[a] = float(J[a * 8 + 2 * v + 1]);
-    x[a] = pk2(xr[a], xi[a]);
-  }
-  unsigned long long s = pk2(0.f, 0.f);
-#pragma unroll
-  for (int a = 0; a < NCOL; a++) {
-    const float caa = 0.5f * CM::at(a * NCOL + a);
-    unsigned long long y = mul2(pk2(caa, caa), x[a]);
-#pragma unroll
-    for (int b = a + 1; b < NCOL; b++) {
-      const float c = CM::at(a * NCOL + b);
-      y = fma2(pk2(c, c), x[b], y);
-    }
-    s = fma2(x[a], y, s);
-    if (x2) x2[a] += keep * (xr[a] * xr[a] + xi[a] * xi[a]);
-  }
-  float sx, sy;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(sx), "=f"(sy) : "l"(s));
-  return 2.f * (sx + sy);
-}
-template <typename TC> struct GrpIsFloat { static constexpr bool value = false; };
-template <> struct GrpIsFloat<float> { static constexpr bool value = true; };
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NLEFT> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NLEFT) : "memory"); }
 
-template <class G, typename T, typename TC, class CM, int MODE, int MINB>
-__global__ void __launch_bounds__(GrpGeom<G, T>::NT, MINB) group_kernel(const LaunchArgs a) {
-  typedef GrpGeom<G, T> GE;
-  constexpr int N = G::n, NPAR = N + 2, NCOMB = 1 << NPAR, LPG = GE::LPG, GPW = GE::GPW, NT = GE::NT;
-  typedef GrpEvent<T, TC, N> EV;
+// D(8x8) += A(8x4) . B(4x8) in fp64 on the tensor cores (SASS: DMMA.8x8x4); thread t holds A[t/4][t%4], B[t%4][t/4],
+// D[t/4][2 (t%4)], D[t/4][2 (t%4) + 1]
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+// D(16x8) += A(16x8) . B(8x8), TF32 inputs, fp32 accumulation (SASS: HMMA.1688.F32.TF32)
+__device__ __forceinline__ void hmma1688(float (&d)[4], const unsigned (&a)[4], unsigned b0, unsigned b1) {
+  asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ unsigned to_tf32(float x) {
+  unsigned r;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+  return r;
+}
+
+// Scalar type of the colour contraction and how many gluon-helicity combinations one MMA tile holds
+template <typename TC> struct ColTraits;
+template <> struct ColTraits<double> { static constexpr int GPT = 1; };
+template <> struct ColTraits<float> { static constexpr int GPT = 2; };
+
+// q_m = sum_{I <= J} X_I C'_{IJ} . X_J over the 8 x 8 tiles of C (C' = C with the diagonal tiles halved), m = row of
+// the staged tile xt[8][LD]; the caller doubles the result.  cf: C' in fragment order [pair(I,J)][k-step][lane].
+// Every lane of the quad t/4 = m returns the partial sum over its two columns per tile (the caller adds the quad).
+template <int NCOL>
+__device__ __forceinline__ double quad_tile(const double* xt, const double* cf, int lane) {
+  constexpr int NT = NCOL / 8, LD = NCOL + 4;
+  const int row = lane >> 2, kq = lane & 3;
+  double a[NCOL / 4];
+#pragma unroll
+  for (int ks = 0; ks < NCOL / 4; ks++) a[ks] = xt[row * LD + 4 * ks + kq];
+  double d[NT][2];
+#pragma unroll
+  for (int J = 0; J < NT; J++) d[J][0] = d[J][1] = 0.0;
+  // I outer, J inner: consecutive MMAs go to different accumulators
+#pragma unroll
+  for (int I = 0; I < NT; I++)
+#pragma unroll
+    for (int s = 0; s < 2; s++)
+#pragma unroll
+      for (int J = I; J < NT; J++) dmma884(d[J][0], d[J][1], a[2 * I + s], cf[((J * (J + 1) / 2 + I) * 2 + s) * 32 + lane]);
+  double q = 0.0;
+#pragma unroll
+  for (int J = 0; J < NT; J++) {
+    const double2 x = *reinterpret_cast<const double2*>(xt + row * LD + 8 * J + 2 * kq);
+    q = ::fma(d[J][0], x.x, q);
+    q = ::fma(d[J][1], x.y, q);
+  }
+  return q;
+}
+// The same for two combinations at once (rows 0-7 and 8-15 of xt[16][LD]) on the TF32 tensor cores; cf: C' as float2
+// (rows k, k + 4 of the tile) [pair(I,J)][lane].  X is split as hi + lo with hi = tf32(x), lo = tf32(x - hi).
+template <int NCOL>
+__device__ __forceinline__ void quad_tile(const float* xt, const float* cf, int lane, float& qa, float& qb) {
+  constexpr int NT = NCOL / 8, LD = NCOL + 4;
+  const int row = lane >> 2, kq = lane & 3;
+  unsigned ah[NT][4], al[NT][4];
+#pragma unroll
+  for (int ks = 0; ks < NT; ks++) {
+    const float x[4] = {xt[row * LD + 8 * ks + kq], xt[(row + 8) * LD + 8 * ks + kq], xt[row * LD + 8 * ks + kq + 4],
+                        xt[(row + 8) * LD + 8 * ks + kq + 4]};
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      ah[ks][i] = to_tf32(x[i]);
+      al[ks][i] = to_tf32(x[i] - __uint_as_float(ah[ks][i]));
+    }
+  }
+  float d[NT][4];
+#pragma unroll
+  for (int J = 0; J < NT; J++) d[J][0] = d[J][1] = d[J][2] = d[J][3] = 0.f;
+#pragma unroll
+  for (int I = 0; I < NT; I++)
+#pragma unroll
+    for (int J = I; J < NT; J++) {
+      const float2 b = *reinterpret_cast<const float2*>(cf + ((J * (J + 1) / 2 + I) * 32 + lane) * 2);
+      hmma1688(d[J], al[I], __float_as_uint(b.x), __float_as_uint(b.y));
+      hmma1688(d[J], ah[I], __float_as_uint(b.x), __float_as_uint(b.y));
+    }
+  qa = qb = 0.f;
+#pragma unroll
+  for (int J = 0; J < NT; J++) {
+    const float2 x = *reinterpret_cast<const float2*>(xt + row * LD + 8 * J + 2 * kq);
+    const float2 y = *reinterpret_cast<const float2*>(xt + (row + 8) * LD + 8 * J + 2 * kq);
+    qa = fmaf(d[J][0], x.x, qa); qa = fmaf(d[J][1], x.y, qa);
+    qb = fmaf(d[J][2], y.x, qb); qb = fmaf(d[J][3], y.y, qb);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// K2: one warp per event (persistent warps, grid-stride over the events of the chunk).
+// CM::at16(i): entry i of the row-major integer colour numerators (global memory).
+// ------------------------------------------------------------------------------------------------------------------
+template <class G, typename TC> struct ColGeom {
+  static constexpr int WARPS = 8, GPT = ColTraits<TC>::GPT, LD = XGeom<G>::LD, NCOL = G::ncol;
+  static constexpr int TILE = GPT * 8 * LD;                              // TC elements of one staged tile
+  static constexpr int CF = XGeom<G>::NPAIR * 64;                        // TC elements of C' in fragment order
+  static constexpr int PERW = 2 * TILE * (int)sizeof(TC) + (int)sizeof(double) * ((1 << (G::n + 2)) + NCOL);
+  static constexpr int SMEM = CF * (int)sizeof(TC) + WARPS * PERW;
+};
+
+template <class G, typename TC, class CM, int MODE>
+__global__ void __launch_bounds__(ColGeom<G, TC>::WARPS * 32, 1) colour_kernel(const PipeArgs p) {
+  typedef ColGeom<G, TC> CG;
+  constexpr int N = G::n, NPAR = N + 2, NCOMB = 1 << NPAR, NCOL = G::ncol, NT = NCOL / 8, LD = CG::LD, GPT = CG::GPT;
+  constexpr int TILE = CG::TILE;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  EV& ev = *reinterpret_cast<EV*>(smem_raw);
-  T* gbase = reinterpret_cast<T*>(smem_raw + ((sizeof(EV) + 127) / 128) * 128);
-  // optional shared-memory copy of the colour matrix as 16-bit integers (behind the group areas), made once
-  const short* cm16 = reinterpret_cast<const short*>(gbase + (size_t)GrpGeom<G, T>::NPASS * GrpGeom<G, T>::GS);
-  if constexpr (CM::smem16) {
-    const int4* src = reinterpret_cast<const int4*>(CM::table16());
-    int4* dst = reinterpret_cast<int4*>(const_cast<short*>(cm16));
-    for (int i = threadIdx.x; i < (G::ncol * G::ncol * 2 + 15) / 16; i += GrpGeom<G, T>::NT) dst[i] = __ldg(src + i);
-  }
+  TC* cf = reinterpret_cast<TC*>(smem_raw);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int gi = lane / LPG, r = lane - gi * LPG;
-  const int lgrp = warp * GPW + gi;                      // group slot of this lane within a pass
-  T* slots = gbase + (size_t)((gi < GPW && lgrp < GE::NPASS) ? lgrp : 0) * GE::GS;
-  T* J = slots + G::nslot * 8;
-  const double mw = a.par.mt * a.par.wt;
-
-  for (long long e = blockIdx.x; e < a.nevt; e += gridDim.x) {
-    __syncthreads();
-    // ---- a1 + per-event, helicity-independent data (a2 bases, invariants in fp64) in ONE phase: every task reads
-    // the momenta it needs from global memory (L1-resident after the first touch; incoming convention: +p for the
-    // initial, -p for the final state), so no task waits for another and one block barrier ends the setup
-    const double* pm = a.mom + e * (NPAR * 4);
-    auto kd = [&](int p, int c) { const double x = __ldg(pm + 4 * p + c); return (p < 2) ? x : -x; };
-    auto dot2 = [&](int p, int q) {  // 2 k_p . k_q
-      return 2.0 * (kd(p, 0) * kd(q, 0) - kd(p, 1) * kd(q, 1) - kd(p, 2) * kd(q, 2) - kd(p, 3) * kd(q, 3));
-    };
-    if (tid == 0) ev.mt = T(a.par.mt);
-    auto is_good = [&](int h) { return MODE == MODE_FILTER || ((a.good.mask[h >> 6] >> (h & 63)) & 1ull) != 0ull; };
-    auto hel_of = [&](int gg, int v) {  // helicity row of gluon-helicity combination gg and variant v = 2 h_t + h_tbar
-      int h = 0;
-      for (int i = 0; i < N; i++) {
-        const int p = (i < 2) ? i : i + 2;
-        h |= ((gg >> (N - 1 - i)) & 1) << (NPAR - 1 - p);
-      }
-      h |= (v >> 1) << (NPAR - 1 - 2);
-      h |= (v & 1) << (NPAR - 1 - 3);
-      return h;
-    };
-    if (MODE == MODE_SELECT && tid >= NT - GE::NGRP) {  // the last NGRP threads: good-helicity bits per combination
-      const int gg = tid - (NT - GE::NGRP);
-      int m = 0;
-      for (int v = 0; v < 4; v++) m |= is_good(hel_of(gg, v)) ? (1 << v) : 0;
-      ev.gmask[gg] = (unsigned char)m;
+  unsigned char* wbase = smem_raw + CG::CF * sizeof(TC) + (size_t)warp * CG::PERW;
+  TC* tile = reinterpret_cast<TC*>(wbase);                                   // [2][TILE]
+  double* mh = reinterpret_cast<double*>(wbase + 2 * TILE * sizeof(TC));     // [NCOMB] |M_h|^2 of this warp's event
+  double* wcs = mh + NCOMB;                                                  // [NCOL] colour weights
+  const LaunchArgs& a = p.a;
+  // ---- C' (diagonal tiles halved) in MMA fragment order, once per block
+  for (int i = tid; i < CG::CF; i += CG::WARPS * 32) {
+    const int l = i & 31;
+    int pair, ca, cb;
+    if (GPT == 1) {  // fp64: [pair][s][lane], B[k = l%4][n = l/4] of k-step s
+      pair = i >> 6;
+      const int s = (i >> 5) & 1;
+      ca = 4 * s + (l & 3); cb = l >> 2;
+    } else {         // tf32: [pair][lane][2], b0 = B[l%4][l/4], b1 = B[l%4 + 4][l/4]
+      pair = i >> 6;
+      const int l2 = (i >> 1) & 31;
+      ca = (l2 & 3) + 4 * (i & 1); cb = l2 >> 2;
     }
-    // the subset tasks run on warp 0, the wavefunction tasks on warp 1: different task types in one warp would
-    // diverge and run one after the other, and this section is pure latency for the whole block
-    static_assert((1 << N) <= 32 && NT >= 32 + N + 6, "setup task layout");
-    {
-      const int task = (tid < (1 << N)) ? tid : ((tid >= 32 && tid < 32 + N + 6) ? (1 << N) + tid - 32 : -1);
-      if (task < 0) {
-      } else if (task < (1 << N)) {
-        // gluon subset m: momentum sum, quark-line momentum after it, 1/K^2, quark-line denominator.
-        // Branch-free: every lane loads all gluon momenta and forms every 2 k_i.k_j, members are picked with
-        // 0/1 factors (exact), so the latency of this serial section is one round of loads + ~150 FP64 operations
-        const int m = task;
-        double kg[N][4], kt[4];
+    (void)l;
+    int J = 0;
+    while ((J + 1) * (J + 2) / 2 <= pair) J++;
+    const int I = pair - J * (J + 1) / 2;
+    const TC cv = TC(CM::at16((8 * I + ca) * NCOL + 8 * J + cb));
+    cf[i] = (I == J) ? TC(0.5) * cv : cv;
+  }
+  __syncthreads();
+  const long long wstride = (long long)gridDim.x * CG::WARPS;
+  const long long w0 = (long long)blockIdx.x * CG::WARPS + warp;
+  const int ntile = (p.ncombo + GPT - 1) / GPT;
+  const TC* xbase = reinterpret_cast<const TC*>(p.xt);
+  auto stage = [&](long long e, int ti, int buf) {
+    const char* src = reinterpret_cast<const char*>(xbase + ((size_t)e * p.ncombo + (size_t)ti * GPT) * (8 * LD));
+    char* dst = reinterpret_cast<char*>(tile + buf * TILE);
+    for (int i = lane; i < (int)(TILE * sizeof(TC) / 16); i += 32) cp_async16(dst + 16 * i, src + 16 * i);
+    cp_async_commit();
+  };
+  auto is_good = [&](int h) { return MODE == MODE_FILTER || ((a.good.mask[h >> 6] >> (h & 63)) & 1ull) != 0ull; };
+  int buf = 0;
+  if (w0 < a.nevt) stage(w0, 0, 0);
+  for (long long e = w0; e < a.nevt; e += wstride) {
+    for (int h = lane; h < NCOMB; h += 32) mh[h] = 0.0;
+    TC wc[(NCOL + 31) / 32];
 #pragma unroll
-        for (int i = 0; i < N; i++)
-#pragma unroll
-          for (int c = 0; c < 4; c++) kg[i][c] = kd((i < 2) ? i : i + 2, c);
-#pragma unroll
-        for (int c = 0; c < 4; c++) kt[c] = kd(2, c);
-        double k[4] = {0.0, 0.0, 0.0, 0.0}, pairs = 0.0, line = 0.0;
-#pragma unroll
-        for (int i = 0; i < N; i++) {
-          const double bi = ((m >> i) & 1) ? 1.0 : 0.0;
-#pragma unroll
-          for (int c = 0; c < 4; c++) k[c] += bi * kg[i][c];
-          line += bi * 2.0 * (kt[0] * kg[i][0] - kt[1] * kg[i][1] - kt[2] * kg[i][2] - kt[3] * kg[i][3]);
-#pragma unroll
-          for (int j = i + 1; j < N; j++) {
-            const double bj = ((m >> j) & 1) ? bi : 0.0;
-            pairs += bj * 2.0 * (kg[i][0] * kg[j][0] - kg[i][1] * kg[j][1] - kg[i][2] * kg[j][2] - kg[i][3] * kg[j][3]);
-          }
-        }
-        const int cnt = __popc(m);
-        for (int c = 0; c < 4; c++) {
-          ev.Ksub[m][c] = T(k[c]);
-          ev.qsub[m][c] = T(-(kt[c] + k[c]));
-        }
-        ev.ik[m] = (cnt >= 2) ? T(1.0 / pairs) : T(0);
-        const double den = line + pairs, nrm = 1.0 / (den * den + mw * mw);
-        ev.gd[m][0] = (cnt >= 1) ? T(den * nrm) : T(0);
-        ev.gd[m][1] = (cnt >= 1) ? T(-mw * nrm) : T(0);
-      } else if (task < (1 << N) + N) {
-        const int i = task - (1 << N), p = (i < 2) ? i : i + 2;
-        mom4<T> k;
-        for (int c = 0; c < 4; c++) k.c[c] = T(kd(p, c));
-        const polbasis<T> pb = make_polbasis<T>((p < 2) ? k : neg(k));
-        for (int c = 0; c < 3; c++) { ev.pol[i][c] = pb.e1[c]; ev.pol[i][3 + c] = pb.e2[c]; }
-      } else {
-        // tasks 0,1: ubar(t), v(tbar) for both helicities; tasks 2..5: Q(h_t, h_tbar) = ubar gamma^mu v
-        const int w = task - (1 << N) - N;
-        spin4<T> ub[2], vv[2];
-#pragma unroll
-        for (int which = 0; which < 2; which++) {
-          mom4<T> k;
-#pragma unroll
-          for (int c = 0; c < 4; c++) k.c[c] = T(-kd(2 + which, c));
-          const spinbasis<T> sb = make_spinbasis<T>(k, T(a.par.mt));
-#pragma unroll
-          for (int l = 0; l < 2; l++) {
-            if (which) vv[l] = spinor_v(sb, l ? 1 : -1);
-            else ub[l] = bar(spinor_u(sb, l ? 1 : -1));
-          }
-        }
-        if (w < 2) {
-#pragma unroll
-          for (int l = 0; l < 2; l++) {
-            T* o = w ? ev.v[l] : ev.ub[l];
-#pragma unroll
-            for (int c = 0; c < 4; c++) {
-              o[2 * c] = w ? vv[l].c[c].re : ub[l].c[c].re;
-              o[2 * c + 1] = w ? vv[l].c[c].im : ub[l].c[c].im;
-            }
-          }
-        } else {
-          const int v = w - 2;
-          vec4<T> JR, JL;
-          chiral_currents(select((v >> 1) != 0, ub[1], ub[0]), select((v & 1) != 0, vv[1], vv[0]), JR, JL);
-          for (int c = 0; c < 4; c++) { ev.Q[v][2 * c] = JR.c[c].re + JL.c[c].re; ev.Q[v][2 * c + 1] = JR.c[c].im + JL.c[c].im; }
-        }
-      }
-    }
-    __syncthreads();
-    if (MODE == MODE_SELECT)  // colour weights of this warp's groups (a8), accumulated over the passes
-      for (int c = lane; c < G::ncol; c += 32) ev.wc[warp][c] = TC(0);
-#pragma unroll 1
-    for (int pass0 = 0; pass0 < GE::NGRP; pass0 += GE::NPASS) {
-    const int grp = pass0 + lgrp;                        // gluon-helicity combination
-    const bool active = (gi < GPW) && (lgrp < GE::NPASS) && (grp < GE::NGRP);
-    // ---- a2: polarisation vectors of this group's gluon helicities
-    if (active && r < N) {
-      const int p = (r < 2) ? r : r + 2;
-      const int lam = ((grp >> (N - 1 - r)) & 1) ? 1 : -1;
-      polbasis<T> pb;
-      for (int c = 0; c < 3; c++) { pb.e1[c] = ev.pol[r][c]; pb.e2[c] = ev.pol[r][3 + c]; }
-      GrpSlot<T>::st(slots, r, polvec(pb, lam, p >= 2));
-    }
+    for (int k = 0; k < (NCOL + 31) / 32; k++) wc[k] = TC(0);
     __syncwarp();
-    // ---- a3: colour-ordered gluon currents, level by level; the full-length ones initialise J
-    grp_tree<G, T, TC>(ev, slots, J, r, active);
-    // ---- a3-a5: quark line
-    if (active) {
-      GrpWalkCtx<G, T, TC> c;
-      c.ev = &ev; c.slots = slots; c.J = J;
-      c.stream = G::role(GE::HTL ? r : (r >> 1));
-      c.ht = GE::HTL ? 0 : (r & 1);
-      typedef GrpWalkCtx<G, T, TC> Ctx;
-      spin4<typename Ctx::PS> psi[Ctx::WP::NCH][G::n];
-#pragma unroll
-      for (int h = 0; h < Ctx::WP::NCH; h++) psi[h][0] = c.psi0(h);
-      GrpWalk<G, T, TC, 1>::node(c, psi);
-    }
-    __syncwarp();
-    // ---- a6: colour sums.  Helicity row of variant v = 2 h_t + h_tbar of this group:
-    auto hel_row = [&](int v) { return hel_of(grp, v); };
-    if constexpr (G::ncol > 24) {
-      // rows of C split over the lanes of the group; every C_ab read once feeds the 8 real vectors
-      // (4 variants x re/im) of the group; partial sums meet in the (now free) current slots
-      TC part[8];
-#pragma unroll
-      for (int k = 0; k < 8; k++) part[k] = TC(0);
-      if (active) {
-        // RB rows of the lane at a time: every x_b fetched from shared memory feeds RB rows (the loop is bound by
-        // shared-memory wavefronts: the lanes are at different b, nothing is broadcast)
-        constexpr int RB = 4;
-        auto cmat = [&](int i) { return CM::smem16 ? TC(cm16[i]) : CM::at(i); };
 #pragma unroll 1
-        for (int a0 = r; a0 < G::ncol; a0 += RB * LPG) {
-          TC xa[RB][8], y[RB][8];
-          int row[RB];
-#pragma unroll
-          for (int j = 0; j < RB; j++) {
-            const int aj = a0 + j * LPG;
-            const bool on = aj < G::ncol;
-            row[j] = on ? aj : G::ncol - 1;
-            const vec4<T> ja = GrpVec<T>::ld(J + row[j] * 8, 0u);
-#pragma unroll
-            for (int k = 0; k < 4; k++) { xa[j][2 * k] = on ? TC(ja.c[k].re) : TC(0); xa[j][2 * k + 1] = on ? TC(ja.c[k].im) : TC(0); }
-            const TC caa = TC(0.5) * cmat(row[j] * G::ncol + row[j]);
-#pragma unroll
-            for (int k = 0; k < 8; k++) y[j][k] = caa * xa[j][k];
-            if (!on) row[j] = G::ncol;  // no column b > row: contributes nothing
-          }
-#pragma unroll 2
-          for (int b = a0 + 1; b < G::ncol; b++) {
-            const vec4<T> jb = GrpVec<T>::ld(J + b * 8, 0u);
-#pragma unroll
-            for (int j = 0; j < RB; j++) {
-              const TC c = (b > row[j]) ? cmat(row[j] * G::ncol + b) : TC(0);
-#pragma unroll
-              for (int k = 0; k < 4; k++) { y[j][2 * k] += c * TC(jb.c[k].re); y[j][2 * k + 1] += c * TC(jb.c[k].im); }
-            }
-          }
-#pragma unroll
-          for (int j = 0; j < RB; j++)
-#pragma unroll
-            for (int k = 0; k < 8; k++) part[k] += xa[j][k] * y[j][k];
-        }
-      }
-      __syncwarp();  // every lane of the group is done with the current slots
-      if (active) {
-        vec4<T> pv;
-#pragma unroll
-        for (int k = 0; k < 4; k++) pv.c[k] = mk<T>(T(part[2 * k]), T(part[2 * k + 1]));
-        GrpVec<T>::st(slots + r * 8, pv);
-      }
+    for (int ti = 0; ti < ntile; ti++) {
+      // prefetch the next tile (of this event or of the warp's next event) while this one is contracted
+      const bool more_here = ti + 1 < ntile;
+      const long long en = more_here ? e : e + wstride;
+      if (en < a.nevt) stage(en, more_here ? ti + 1 : 0, buf ^ 1);
+      else cp_async_commit();
+      cp_async_wait<1>();
       __syncwarp();
-      if (active && r < 4) {
-        double q = 0.0;
-        for (int l = 0; l < LPG; l++) q += (double)slots[l * 8 + 2 * r] + (double)slots[l * 8 + 2 * r + 1];
-        ev.mh[hel_row(r)] = 2.0 * q;
-      }
-    } else if constexpr (GrpIsFloat<TC>::value) {
-      // float colour sum: task = variant (4 per group), re and im of J as one packed f32x2 pair
-#pragma unroll 1
-      for (int k0 = 0; k0 < 4; k0 += LPG) {
-        const int v = k0 + r;
-        if (active && v < 4) {
-          const int h = hel_row(v);
-          const float keep = is_good(h) ? 1.f : 0.f;
-          ev.mh[h] = (double)grp_quadform_pk<G::ncol, T, CM>(J, v, nullptr, keep);
-        }
-      }
-    } else {
-      // task = (variant, re/im): 8 per group, lane r takes tasks r, r + LPG, ...; pairs are added by one shuffle
-#pragma unroll 1
-      for (int k0 = 0; k0 < 8; k0 += LPG) {
-        const int k = k0 + r;
-        TC q = TC(0);
-        int h = 0;
-        const bool on = active && k < 8;
-        if (on) {
-          h = hel_row(k >> 1);
-          const TC keep = is_good(h) ? TC(1) : TC(0);
-          q = grp_quadform<G::ncol, T, TC, CM>(J, k, nullptr, keep);
-        }
+      const TC* xt = tile + buf * TILE;
+      // ---- a6 on the tensor cores
+      if constexpr (GPT == 1) {
+        double q = quad_tile<NCOL>(xt, cf, lane);
         q += __shfl_xor_sync(0xffffffffu, q, 1);
-        if (on && !(k & 1)) ev.mh[h] = (double)q;
+        q += __shfl_xor_sync(0xffffffffu, q, 2);   // row m = lane / 4 complete
+        q += __shfl_xor_sync(0xffffffffu, q, 4);   // re + im rows of variant v = lane / 8
+        if ((lane & 7) == 0) mh[grp_hel_of<N>(p.combo[ti], lane >> 3)] = 2.0 * q;
+      } else {
+        float qa, qb;
+        quad_tile<NCOL>(xt, cf, lane, qa, qb);
+        qa += __shfl_xor_sync(0xffffffffu, qa, 1); qb += __shfl_xor_sync(0xffffffffu, qb, 1);
+        qa += __shfl_xor_sync(0xffffffffu, qa, 2); qb += __shfl_xor_sync(0xffffffffu, qb, 2);
+        qa += __shfl_xor_sync(0xffffffffu, qa, 4); qb += __shfl_xor_sync(0xffffffffu, qb, 4);
+        if ((lane & 7) == 0) {
+          mh[grp_hel_of<N>(p.combo[2 * ti], lane >> 3)] = (double)(2.f * qa);
+          if (2 * ti + 1 < p.ncombo) mh[grp_hel_of<N>(p.combo[2 * ti + 1], lane >> 3)] = (double)(2.f * qb);
+        }
       }
-    }
-    __syncwarp();
-    if (MODE == MODE_SELECT) {
-      // a8 colour weights w_c += sum over this warp's groups and the good (h_t, h_tbar) of |J_c|^2: lane = flow,
-      // read back from the J areas (cheaper than per-lane partial sums and a shuffle reduction per flow)
-      for (int c = lane; c < G::ncol; c += 32) {
-        TC w = TC(0);
-#pragma unroll 1
-        for (int g = 0; g < GPW; g++) {
-          const int lg = warp * GPW + g, gg = pass0 + lg;
-          if (lg < GE::NPASS && gg < GE::NGRP) {
-            const vec4<T> j = GrpVec<T>::ld(gbase + (size_t)lg * GE::GS + G::nslot * 8 + c * 8, 0u);
-            const int gm = ev.gmask[gg];
+      if (MODE == MODE_SELECT) {
+        // a8 colour weights w_c += sum over the good (h_t, h_tbar) of |J_c|^2: lane = flow
 #pragma unroll
-            for (int v = 0; v < 4; v++) {
-              const TC keep = ((gm >> v) & 1) ? TC(1) : TC(0);
-              w += keep * (TC(j.c[v].re) * TC(j.c[v].re) + TC(j.c[v].im) * TC(j.c[v].im));
+        for (int g = 0; g < GPT; g++) {
+          const int ci = ti * GPT + g;
+          if (ci < p.ncombo) {
+            const int gm = p.vmask[ci];
+#pragma unroll
+            for (int k = 0; k < (NCOL + 31) / 32; k++) {
+              const int c = lane + 32 * k;
+              if (c < NCOL) {
+                TC w = TC(0);
+#pragma unroll
+                for (int v = 0; v < 4; v++) {
+                  const TC keep = ((gm >> v) & 1) ? TC(1) : TC(0);
+                  const TC xr = xt[(g * 8 + 2 * v) * LD + c], xi = xt[(g * 8 + 2 * v + 1) * LD + c];
+                  w += keep * (xr * xr + xi * xi);
+                }
+                wc[k] += w;
+              }
             }
           }
         }
-        ev.wc[warp][c] += w;
       }
-      __syncwarp();
+      __syncwarp();  // every lane is done with this buffer before it is refilled
+      buf ^= 1;
     }
-    }  // passes
-    __syncthreads();
-    // ---- a7-a9
+    // ---- a7-a9 for this event
     if (MODE == MODE_FILTER) {
       double total = 0.0;
-      for (int h = 0; h < NCOMB; h++) total += ev.mh[h];
-      for (int h = tid; h < NCOMB; h += NT) {
-        const double f = (total > 0.0) ? ev.mh[h] / total : 0.0;
+      for (int h = 0; h < NCOMB; h++) total += mh[h];
+      for (int h = lane; h < NCOMB; h += 32) {
+        const double f = (total > 0.0) ? mh[h] / total : 0.0;
         atomicMax(a.fracmax + h, (unsigned long long)__double_as_longlong(f));
       }
-    } else if (warp == 0) {
-      // helicity sum in table order (a7), ME (a9) and helicity selection (a8): one warp, in-order scan
-      constexpr int PER = NCOMB / 32;
-      double val[PER];
-      bool ok[PER];
+    } else {
+      {
+        // helicity sum in table order (a7), ME (a9) and helicity selection (a8): in-order scan
+        constexpr int PER = NCOMB / 32;
+        double val[PER];
+        bool ok[PER];
 #pragma unroll
-      for (int i = 0; i < PER; i++) {
-        const int h = lane * PER + i;
-        ok[i] = is_good(h);
-        val[i] = ok[i] ? ev.mh[h] : 0.0;
+        for (int i = 0; i < PER; i++) {
+          const int h = lane * PER + i;
+          ok[i] = is_good(h);
+          val[i] = ok[i] ? mh[h] : 0.0;
+        }
+        double total;
+        int sel;
+        grp_warp_select<PER>(val, ok, (MODE == MODE_SELECT && a.selhel) ? a.rndhel[e] : 0.0, lane, total, sel);
+        if (lane == 0) {
+          const double g = a.gs[e];
+          a.me[e] = total * ipow<2 * N>(g) * (1.0 / (double(G::denom) * double(G::cden)));
+          if (MODE == MODE_SELECT && a.selhel) a.selhel[e] = sel;
+        }
       }
-      double total;
-      int sel;
-      grp_warp_select<PER>(val, ok, (MODE == MODE_SELECT && a.selhel) ? a.rndhel[e] : 0.0, lane, total, sel);
-      if (lane == 0) {
-        const double g = a.gs[e];
-        a.me[e] = total * ipow<2 * N>(g) * (1.0 / (double(G::denom) * double(G::cden)));
-        if (MODE == MODE_SELECT && a.selhel) a.selhel[e] = sel;
-      }
-    } else if (warp == 1 && MODE == MODE_SELECT && a.selcol) {
-      constexpr int PER = (G::ncol + 31) / 32;
-      double val[PER];
-      bool ok[PER];
+      if (MODE == MODE_SELECT && a.selcol) {
 #pragma unroll
-      for (int i = 0; i < PER; i++) {
-        const int c = lane * PER + i;
-        ok[i] = c < G::ncol;
-        TC w = TC(0);
-        if (ok[i])
-          for (int k = 0; k < GE::NW; k++) w += ev.wc[k][c];
-        val[i] = (double)w;
+        for (int k = 0; k < (NCOL + 31) / 32; k++)
+          if (lane + 32 * k < NCOL) wcs[lane + 32 * k] = (double)wc[k];
+        __syncwarp();
+        constexpr int PER = (NCOL + 31) / 32;
+        double val[PER];
+        bool ok[PER];
+#pragma unroll
+        for (int i = 0; i < PER; i++) {
+          const int c = lane * PER + i;
+          ok[i] = c < NCOL;
+          val[i] = ok[i] ? wcs[c] : 0.0;
+        }
+        double total;
+        int sel;
+        grp_warp_select<PER>(val, ok, a.rndcol[e], lane, total, sel);
+        if (lane == 0) a.selcol[e] = sel;
       }
-      double total;
-      int sel;
-      grp_warp_select<PER>(val, ok, a.rndcol[e], lane, total, sel);
-      if (lane == 0) a.selcol[e] = sel;
     }
+    __syncwarp();
   }
+  cp_async_wait<0>();
 }
 
 }  // namespace me

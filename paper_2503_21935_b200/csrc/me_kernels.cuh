@@ -32,13 +32,18 @@ struct LaunchArgs {
   double* cum;                 // scratch [ngood][nslots] running helicity sums (selection only)
   unsigned long long* fracmax; // filter: [ncomb] max over events of |M_h|^2 / sum (bit pattern of a double)
   int blocks;                  // 0 = choose
+  void* scratch;               // lane-group pipeline: per-event data and jamps between its kernels (owned by the handle)
+  size_t scratch_bytes;
   DevParams par;
   GoodList good;
 };
 
 struct LaunchInfo {
-  int threads, blocks, regs, local_bytes;
-  long long cum_slots;  // MODE_SELECT scratch: doubles per good helicity (0: the kernel keeps them on chip)
+  int threads, blocks, regs, local_bytes;   // of the dominant (amplitude) kernel
+  long long cum_slots;          // one-event-per-thread kernel, MODE_SELECT scratch: doubles per good helicity
+  long long scratch_per_event;  // lane-group pipeline: scratch bytes per event of a chunk (0: not used)
+  long long chunk;              // lane-group pipeline: events per chunk with the scratch given
+  int launches;                 // kernels enqueued by the call
 };
 
 enum { MODE_ME = 0, MODE_SELECT = 1, MODE_FILTER = 2 };

@@ -62,6 +62,9 @@ int run(double* tflops, double* ms_out) {
 
 extern "C" int me_fma_peak(int precision, int device, double* tflops) {
   if (!tflops || (precision != ME_FP64 && precision != ME_FP32)) return ME_ERR_ARG;
-  if (cudaSetDevice(device) != cudaSuccess) return ME_ERR_CUDA;
-  return precision == ME_FP64 ? run<double>(tflops, nullptr) : run<float>(tflops, nullptr);
+  int prev = -1;
+  if (cudaGetDevice(&prev) != cudaSuccess || cudaSetDevice(device) != cudaSuccess) return ME_ERR_CUDA;
+  const int rc = precision == ME_FP64 ? run<double>(tflops, nullptr) : run<float>(tflops, nullptr);
+  if (prev != device) cudaSetDevice(prev);  // leave the caller's current device as it was
+  return rc;
 }

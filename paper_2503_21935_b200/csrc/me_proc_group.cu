@@ -1,6 +1,8 @@
 // me_proc_group.cu -- one translation unit per (process, precision) in the lane-group layout (me_group.cuh):
-//   -DME_PROC=<name> -DME_PROC_UP=<NAME> -DME_PREC=<0|1|2> [-DME_MINB=<min blocks/SM>]
+//   -DME_PROC=<name> -DME_PROC_UP=<NAME> -DME_PREC=<0|1|2> [-DME_MINB=<min amplitude warps per SM>]
 // exports  me_launch_<name>_p<prec>  (C++ linkage, called from me_api.cu), same contract as me_proc.cu.
+// A call runs the events in chunks that fit the handle's scratch; per chunk three kernels on the caller's stream:
+// setup_kernel (K0) -> amp_kernel (K1) -> colour_kernel (K2).
 #include "me_group.cuh"
 
 #define ME_CAT_(a, b) a##b
@@ -13,9 +15,6 @@
 
 #ifndef ME_MINB
 #define ME_MINB 1
-#endif
-#ifndef ME_CMAT_GLOBAL
-#define ME_CMAT_GLOBAL 0
 #endif
 
 #if ME_PREC == 0
@@ -31,54 +30,89 @@ typedef float T_col;
 
 typedef ME_CAT(Grp_, ME_PROC) Grp;
 
-// colour-matrix numerators: integers, exactly representable in fp32 (<= 4096), as T_col
-// (constant memory up to 24 flows; the 120 x 120 matrix exceeds the 64 KB bank and is read through L1)
-#if ME_CMAT_GLOBAL
-__device__ const T_col c_cmat[Grp::ncol * Grp::ncol] = ME_CAT(ME_CMAT_, ME_PROC_UP);
-// the same numerators as 16-bit integers (|C| <= 4096): 28.8 KB, copied into shared memory by builds whose
-// amplitudes are fp64 (one block per SM anyway); the fp32 build keeps two blocks per SM and reads C through L1
+// colour-matrix numerators: integers of magnitude <= 4096 (exact in fp64, fp32 and TF32), read once per block of K2
 __device__ const short c_cmat16[Grp::ncol * Grp::ncol] = ME_CAT(ME_CMAT_, ME_PROC_UP);
 struct CMat {
-  static constexpr bool smem16 = (ME_PREC != 1);
-  __device__ __forceinline__ static T_col at(int i) { return __ldg(c_cmat + i); }
-  __device__ __forceinline__ static const short* table16() { return c_cmat16; }
+  __device__ __forceinline__ static int at16(int i) { return (int)__ldg(c_cmat16 + i); }
 };
-#else
-__constant__ T_col c_cmat[Grp::ncol * Grp::ncol] = ME_CAT(ME_CMAT_, ME_PROC_UP);
-struct CMat {
-  static constexpr bool smem16 = false;
-  __device__ __forceinline__ static T_col at(int i) { return c_cmat[i]; }
-  __device__ __forceinline__ static const short* table16() { return nullptr; }
-};
-#endif
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 template <int MODE, typename TA, typename TCo>
 static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo* info, bool dry) {
   typedef me::GrpGeom<Grp, TA> GE;
-  auto kern = me::group_kernel<Grp, TA, TCo, CMat, MODE, ME_MINB>;
-  const size_t ev_bytes = ((sizeof(me::GrpEvent<TA, TCo, Grp::n>) + 127) / 128) * 128;
-  const size_t smem = ev_bytes + (size_t)GE::NPASS * GE::GS * sizeof(TA) + (CMat::smem16 ? (size_t)Grp::ncol * Grp::ncol * 2 + 16 : 0);
-  cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  typedef me::ColGeom<Grp, TCo> CG;
+  typedef me::GrpEvent<TA, Grp::n> EV;
+  constexpr int N = Grp::n, LD = me::XGeom<Grp>::LD;
+  auto k0 = me::setup_kernel<TA, N>;
+  auto k1 = me::amp_kernel<Grp, TA, TCo, ME_MINB>;
+  auto k2 = me::colour_kernel<Grp, TCo, CMat, MODE>;
+  // the gluon-helicity combinations with at least one good helicity row
+  me::PipeArgs p;
+  memset(&p, 0, sizeof(p));
+  for (int gg = 0; gg < GE::NGRP; gg++) {
+    int m = 0;
+    for (int v = 0; v < 4; v++) {
+      const int h = me::grp_hel_of<N>(gg, v);
+      if (MODE == me::MODE_FILTER || ((a.good.mask[h >> 6] >> (h & 63)) & 1ull)) m |= 1 << v;
+    }
+    if (m) { p.combo[p.ncombo] = (unsigned char)gg; p.vmask[p.ncombo] = (unsigned char)m; p.ncombo++; }
+  }
+  const size_t evb = sizeof(EV), grpb = (size_t)8 * LD * sizeof(TCo);
+  const size_t per_event = evb + (size_t)p.ncombo * grpb, slack = 2 * grpb + 512;
+  long long chunk = (a.scratch_bytes > slack) ? (long long)((a.scratch_bytes - slack) / per_event) : 0;
+  if (chunk > (1 << 20)) chunk = 1 << 20;
+  const int nunit = (p.ncombo + GE::GPW - 1) / GE::GPW;
+  int dev = 0, sms = 0;
+  cudaError_t err = cudaGetDevice(&dev);
+  if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   if (err != cudaSuccess) return (int)err;
-  long long blocks = a.nevt;
-  if (a.blocks > 0) blocks = a.blocks;
-  if (blocks > (1ll << 30)) blocks = 1ll << 30;
-  if (blocks < 1) blocks = 1;
   if (info) {
     cudaFuncAttributes fa;
-    err = cudaFuncGetAttributes(&fa, kern);
+    err = cudaFuncGetAttributes(&fa, k1);
     if (err != cudaSuccess) return (int)err;
-    info->threads = GE::NT;
-    info->blocks = (int)blocks;
+    info->threads = 32;
+    info->blocks = (int)((a.nevt < chunk ? a.nevt : chunk) * nunit);
     info->regs = fa.numRegs;
     info->local_bytes = (int)fa.localSizeBytes;
     info->cum_slots = 0;
+    info->scratch_per_event = (long long)(sizeof(EV) + (size_t)GE::NGRP * grpb);
+    info->chunk = chunk;
+    info->launches = (chunk > 0) ? (int)(3 * ((a.nevt + chunk - 1) / chunk)) : 0;
   }
   if (dry || a.nevt == 0) return 0;
-  kern<<<(unsigned)blocks, GE::NT, smem, st>>>(a);
-  return (int)cudaGetLastError();
+  if (p.ncombo == 0 || chunk < 1 || !a.scratch) return (int)cudaErrorInvalidValue;
+  err = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, GE::SMEM);
+  if (err == cudaSuccess) err = cudaFuncSetAttribute(k1, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  if (err == cudaSuccess) err = cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, CG::SMEM);
+  if (err != cudaSuccess) return (int)err;
+  for (long long e0 = 0; e0 < a.nevt; e0 += chunk) {
+    const long long n = (a.nevt - e0 < chunk) ? (a.nevt - e0) : chunk;
+    p.a = a;
+    p.a.nevt = n;
+    p.a.mom = a.mom + e0 * (Grp::npar * 4);
+    p.a.gs = a.gs + e0;
+    p.a.rndhel = a.rndhel ? a.rndhel + e0 : nullptr;
+    p.a.rndcol = a.rndcol ? a.rndcol + e0 : nullptr;
+    p.a.me = a.me ? a.me + e0 : nullptr;
+    p.a.selhel = a.selhel ? a.selhel + e0 : nullptr;
+    p.a.selcol = a.selcol ? a.selcol + e0 : nullptr;
+    p.ev = a.scratch;
+    p.xt = (char*)a.scratch + align_up((size_t)n * evb, 256);
+    constexpr int PT = ((1 << N) + N + 6 <= 32) ? 32 : 64;
+    k0<<<(unsigned)((n * PT + 127) / 128), 128, 0, st>>>(p.a, (EV*)p.ev);
+    k1<<<(unsigned)(n * nunit), 32, GE::SMEM, st>>>(p);
+    long long b2 = (n + CG::WARPS - 1) / CG::WARPS;
+    if (b2 > sms) b2 = sms;
+    k2<<<(unsigned)b2, CG::WARPS * 32, CG::SMEM, st>>>(p);
+    err = cudaGetLastError();
+    if (err != cudaSuccess) return (int)err;
+  }
+  return 0;
 }
 
+// mode: me::MODE_*; dry = only report the launch geometry in *info.
+// The filter always runs in fp64 (reading R10).  Returns a cudaError_t value.
 int ME_CAT(ME_CAT(me_launch_, ME_PROC), ME_CAT(_p, ME_PREC))(const me::LaunchArgs& a, int mode, void* stream,
                                                               me::LaunchInfo* info, int dry) {
   cudaStream_t st = (cudaStream_t)stream;

@@ -19,7 +19,7 @@ PROCESSES = ("ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg")
 
 EXPORTS = ("me_create", "me_destroy", "me_last_error", "me_info", "me_helicity_table", "me_color_table",
            "me_color_matrix", "me_filter_helicities", "me_get_good_helicities", "me_set_good_helicities",
-           "me_compute", "me_compute_host", "me_generate", "me_launch_info", "me_fma_peak")
+           "me_compute", "me_compute_host", "me_generate", "me_launch_info", "me_launch_stats", "me_fma_peak")
 
 
 class MEError(RuntimeError):
@@ -57,6 +57,7 @@ def load_library(path: str = LIB_PATH):
     L.me_compute_host.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, vp]
     L.me_generate.argtypes = [vp, ctypes.c_uint64, i64, i64, ctypes.c_double, ctypes.c_double, vp, vp, vp, vp, vp, vp]
     L.me_launch_info.argtypes = [vp, ip, ip, ip, ip]
+    L.me_launch_stats.argtypes = [vp, ip, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
     L.me_fma_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
     for n in EXPORTS:
         if n != "me_last_error":
@@ -213,7 +214,11 @@ class MatrixElement:
     def launch_info(self) -> dict:
         v = [ctypes.c_int() for _ in range(4)]
         self._check(self._L.me_launch_info(self._h, *[ctypes.byref(x) for x in v]))
-        return dict(zip(("threads", "blocks", "regs", "local_bytes"), (x.value for x in v)))
+        d = dict(zip(("threads", "blocks", "regs", "local_bytes"), (x.value for x in v)))
+        n, c, b = ctypes.c_int(), ctypes.c_int64(), ctypes.c_int64()
+        self._check(self._L.me_launch_stats(self._h, ctypes.byref(n), ctypes.byref(c), ctypes.byref(b)))
+        d.update(launches=n.value, chunk_events=c.value, scratch_bytes=b.value)
+        return d
 
 
 def fma_peak(precision: str = "fp64", device: int = 0) -> float:
