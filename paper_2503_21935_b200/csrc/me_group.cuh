@@ -12,12 +12,16 @@
 //                       tree    lane = sequence : colour-ordered currents Jord(seq), |seq| = 2..n-1 -> shared-memory slot
 //                               |seq| = n       : contracted at once with the four Q               -> "init" slot
 //                       walk    lane = s1       : quark line for the flows that start with gluon s1; at the leaf of
-//                               flow sigma  J_sigma = init + Psi.v  goes straight to HBM as X[event][combination][8][LD]
-//                               (row = 2 (2 h_t + h_tbar) + re/im, column = flow): the jamps never sit in shared memory.
+//                               flow sigma  J_sigma = init + Psi.v  goes straight to HBM as X[event][combination][flow][8]
+//                               (8 = 2 (2 h_t + h_tbar) + re/im; 16- or 32-byte stores): the jamps never sit in
+//                               shared memory.
 //   K2 colour_kernel  a6-a9.  One warp per event.  Per gluon-helicity combination the colour sum of its 8 real
 //                     vectors is the contraction  q_m = sum_ab X[m][a] C[a][b] X[m][b]  = [8 x ncol] . [ncol x ncol]
-//                     followed by a row dot: tensor-core MMAs with C in shared memory in fragment order, only the
-//                     upper triangle of 8 x 8 tiles (diagonal tiles halved, result doubled: C is symmetric).
+//                     followed by a row dot: tensor-core MMAs with X loaded from HBM straight into A fragments
+//                     (256 / 128 contiguous bytes per warp load), C in shared memory in fragment order, only the
+//                     upper triangle of 8 x 8 tiles (diagonal tiles halved, result doubled: C is symmetric); the
+//                     columns of every tile are permuted so that the D fragment of a thread meets the X values it
+//                     already holds (the row dot needs no second load).
 //                       fp64 build        : mma.sync m8n8k4 f64 (DMMA)
 //                       fp32 / mixed build: mma.sync m16n8k8 tf32, two combinations per tile, X split into
 //                                           hi + lo TF32 parts (the integer colour numerators are exact in TF32), so
@@ -299,19 +303,18 @@ struct GrpGeom {
   static constexpr int SMEM = EVB + GPW * GS * (int)sizeof(T);
 };
 
-// Layout of the jamps in HBM between K1 and K2: X[event][listed combination][8][LD], row m = 2 (2 h_t + h_tbar) +
-// re/im, column = colour flow.  LD = ncol + 4 makes the row stride 96 mod 128 bytes (fp64) / 112 mod 128 (fp32): the
-// MMA A-fragment loads of K2 (8 rows x 4 consecutive columns) are free of bank conflicts.
+// Layout of the jamps in HBM between K1 and K2: X[event][listed combination][flow][8], the 8 = 2 (2 h_t + h_tbar) +
+// re/im.  A warp of K2 reads 4 (fp64) or 2 x 4 (fp32) consecutive flows = 256 / 128 contiguous bytes per load.
 template <class G> struct XGeom {
-  static constexpr int NCOL = G::ncol, LD = NCOL + 4, NT = NCOL / 8, NPAIR = NT * (NT + 1) / 2;
-  static_assert(NCOL % 8 == 0 && LD % 16 == 12, "tile geometry");
+  static constexpr int NCOL = G::ncol, NT = NCOL / 8, NPAIR = NT * (NT + 1) / 2, GRP = NCOL * 8;
+  static_assert(NCOL % 8 == 0, "tile geometry");
 };
 
 // Arguments of the three kernels of one chunk of events (pointers already offset to the chunk)
 struct PipeArgs {
   LaunchArgs a;
   void* ev;                  // GrpEvent<T, N>[nevt]
-  void* xt;                  // TC[nevt][ncombo][8][LD] (+ one group of slack)
+  void* xt;                  // TC[nevt][ncombo][ncol][8] (+ one group of slack)
   int ncombo;                // gluon-helicity combinations with at least one good helicity row
   unsigned char combo[32];   // ... in increasing order
   unsigned char vmask[32];   // per listed combination: bit v = 2 h_t + h_tbar set iff that helicity row is good
@@ -488,7 +491,7 @@ template <class G, typename T, typename TC>
 struct GrpWalkCtx {
   const GrpEvent<T, G::n>* ev;
   const T* slots;
-  TC* X;  // jamps of this group in HBM: [8][LD]
+  TC* X;  // jamps of this group in HBM: [ncol][8]
   const unsigned* stream;
   int ht;
   __device__ __forceinline__ unsigned next() { return __ldg(stream++); }
@@ -518,19 +521,17 @@ struct GrpWalkCtx {
   }
   __device__ __forceinline__ static f2 pack(float x, float y) { return mkf2(x, y); }
   __device__ __forceinline__ static double pack(double x, double) { return x; }
-  // J_flow(h_t, b) = sg * init + a  ->  X[2 (2 h_t + b) + re/im][flow]
+  // J_flow(h_t, b) = sg * init + a  ->  X[flow][2 (2 h_t + b) + re/im]; stores bypass L1 (the table words live there)
+  __device__ __forceinline__ static void st2(double* q, double x, double y) { __stcg(reinterpret_cast<double2*>(q), make_double2(x, y)); }
+  __device__ __forceinline__ static void st2(float* q, float x, float y) { __stcg(reinterpret_cast<float2*>(q), make_float2(x, y)); }
   __device__ __forceinline__ void put(const T* ji, T sg, int f, int h, int b, f2 re, f2 im) const {
-    constexpr int LD = XGeom<G>::LD;
-    X[(2 * b) * LD + f] = TC(fmaf(sg, ji[2 * b], re.v.x));              // h_t = 0: v = b
-    X[(2 * b + 1) * LD + f] = TC(fmaf(sg, ji[2 * b + 1], im.v.x));
-    X[(4 + 2 * b) * LD + f] = TC(fmaf(sg, ji[4 + 2 * b], re.v.y));      // h_t = 1: v = 2 + b
-    X[(5 + 2 * b) * LD + f] = TC(fmaf(sg, ji[5 + 2 * b], im.v.y));
+    TC* q = X + f * 8;
+    st2(q + 2 * b, TC(fmaf(sg, ji[2 * b], re.v.x)), TC(fmaf(sg, ji[2 * b + 1], im.v.x)));              // h_t = 0: v = b
+    st2(q + 4 + 2 * b, TC(fmaf(sg, ji[4 + 2 * b], re.v.y)), TC(fmaf(sg, ji[5 + 2 * b], im.v.y)));      // h_t = 1: v = 2 + b
   }
   template <typename S> __device__ __forceinline__ void put(const T* ji, T sg, int f, int h, int b, S re, S im) const {
-    constexpr int LD = XGeom<G>::LD;
     const int v = 2 * h + b;
-    X[(2 * v) * LD + f] = TC(fmad<T>(sg, ji[2 * v], re));
-    X[(2 * v + 1) * LD + f] = TC(fmad<T>(sg, ji[2 * v + 1], im));
+    st2(X + f * 8 + 2 * v, TC(fmad<T>(sg, ji[2 * v], re)), TC(fmad<T>(sg, ji[2 * v + 1], im)));
   }
   __device__ __forceinline__ void leaf(const spin4<PS> (&Xs)[WP::NCH], unsigned w) const {
     const int f = (w >> 16) & 127;
@@ -613,7 +614,7 @@ struct GrpWalk<G, T, TC, G::n> {
 template <class G, typename T, typename TC, int MINB>
 __global__ void __launch_bounds__(32, MINB) amp_kernel(const PipeArgs p) {
   typedef GrpGeom<G, T> GE;
-  constexpr int N = G::n, LPG = GE::LPG, GPW = GE::GPW, LD = XGeom<G>::LD;
+  constexpr int N = G::n, LPG = GE::LPG, GPW = GE::GPW;
   typedef GrpEvent<T, N> EV;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   EV& ev = *reinterpret_cast<EV*>(smem_raw);
@@ -651,7 +652,7 @@ __global__ void __launch_bounds__(32, MINB) amp_kernel(const PipeArgs p) {
     typedef GrpWalkCtx<G, T, TC> Ctx;
     Ctx c;
     c.ev = &ev; c.slots = slots;
-    c.X = reinterpret_cast<TC*>(p.xt) + ((size_t)e * p.ncombo + ci) * (8 * LD);
+    c.X = reinterpret_cast<TC*>(p.xt) + ((size_t)e * p.ncombo + ci) * XGeom<G>::GRP;
     c.stream = G::role(GE::HTL ? r : (r >> 1));
     c.ht = GE::HTL ? 0 : (r & 1);
     spin4<typename Ctx::PS> psi[Ctx::WP::NCH][G::n];
@@ -693,13 +694,6 @@ __device__ __forceinline__ void grp_warp_select(const double (&val)[PER], const 
   else sel = bo ? __shfl_sync(0xffffffffu, lastok, 31 - __clz(bo)) : 0;
 }
 
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int NLEFT> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NLEFT) : "memory"); }
-
 // D(8x8) += A(8x4) . B(4x8) in fp64 on the tensor cores (SASS: DMMA.8x8x4); thread t holds A[t/4][t%4], B[t%4][t/4],
 // D[t/4][2 (t%4)], D[t/4][2 (t%4) + 1]
 __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
@@ -716,120 +710,153 @@ __device__ __forceinline__ unsigned to_tf32(float x) {
   return r;
 }
 
-// Scalar type of the colour contraction and how many gluon-helicity combinations one MMA tile holds
-template <typename TC> struct ColTraits;
-template <> struct ColTraits<double> { static constexpr int GPT = 1; };
-template <> struct ColTraits<float> { static constexpr int GPT = 2; };
-
-// q_m = sum_{I <= J} X_I C'_{IJ} . X_J over the 8 x 8 tiles of C (C' = C with the diagonal tiles halved), m = row of
-// the staged tile xt[8][LD]; the caller doubles the result.  cf: C' in fragment order [pair(I,J)][k-step][lane].
-// Every lane of the quad t/4 = m returns the partial sum over its two columns per tile (the caller adds the quad).
-template <int NCOL>
-__device__ __forceinline__ double quad_tile(const double* xt, const double* cf, int lane) {
-  constexpr int NT = NCOL / 8, LD = NCOL + 4;
-  const int row = lane >> 2, kq = lane & 3;
-  double a[NCOL / 4];
-#pragma unroll
-  for (int ks = 0; ks < NCOL / 4; ks++) a[ks] = xt[row * LD + 4 * ks + kq];
-  double d[NT][2];
-#pragma unroll
-  for (int J = 0; J < NT; J++) d[J][0] = d[J][1] = 0.0;
-  // I outer, J inner: consecutive MMAs go to different accumulators
-#pragma unroll
-  for (int I = 0; I < NT; I++)
-#pragma unroll
-    for (int s = 0; s < 2; s++)
-#pragma unroll
-      for (int J = I; J < NT; J++) dmma884(d[J][0], d[J][1], a[2 * I + s], cf[((J * (J + 1) / 2 + I) * 2 + s) * 32 + lane]);
-  double q = 0.0;
-#pragma unroll
-  for (int J = 0; J < NT; J++) {
-    const double2 x = *reinterpret_cast<const double2*>(xt + row * LD + 8 * J + 2 * kq);
-    q = ::fma(d[J][0], x.x, q);
-    q = ::fma(d[J][1], x.y, q);
-  }
-  return q;
-}
-// The same for two combinations at once (rows 0-7 and 8-15 of xt[16][LD]) on the TF32 tensor cores; cf: C' as float2
-// (rows k, k + 4 of the tile) [pair(I,J)][lane].  X is split as hi + lo with hi = tf32(x), lo = tf32(x - hi).
-template <int NCOL>
-__device__ __forceinline__ void quad_tile(const float* xt, const float* cf, int lane, float& qa, float& qb) {
-  constexpr int NT = NCOL / 8, LD = NCOL + 4;
-  const int row = lane >> 2, kq = lane & 3;
-  unsigned ah[NT][4], al[NT][4];
-#pragma unroll
-  for (int ks = 0; ks < NT; ks++) {
-    const float x[4] = {xt[row * LD + 8 * ks + kq], xt[(row + 8) * LD + 8 * ks + kq], xt[row * LD + 8 * ks + kq + 4],
-                        xt[(row + 8) * LD + 8 * ks + kq + 4]};
-#pragma unroll
-    for (int i = 0; i < 4; i++) {
-      ah[ks][i] = to_tf32(x[i]);
-      al[ks][i] = to_tf32(x[i] - __uint_as_float(ah[ks][i]));
-    }
-  }
-  float d[NT][4];
-#pragma unroll
-  for (int J = 0; J < NT; J++) d[J][0] = d[J][1] = d[J][2] = d[J][3] = 0.f;
-#pragma unroll
-  for (int I = 0; I < NT; I++)
-#pragma unroll
-    for (int J = I; J < NT; J++) {
-      const float2 b = *reinterpret_cast<const float2*>(cf + ((J * (J + 1) / 2 + I) * 32 + lane) * 2);
-      hmma1688(d[J], al[I], __float_as_uint(b.x), __float_as_uint(b.y));
-      hmma1688(d[J], ah[I], __float_as_uint(b.x), __float_as_uint(b.y));
-    }
-  qa = qb = 0.f;
-#pragma unroll
-  for (int J = 0; J < NT; J++) {
-    const float2 x = *reinterpret_cast<const float2*>(xt + row * LD + 8 * J + 2 * kq);
-    const float2 y = *reinterpret_cast<const float2*>(xt + (row + 8) * LD + 8 * J + 2 * kq);
-    qa = fmaf(d[J][0], x.x, qa); qa = fmaf(d[J][1], x.y, qa);
-    qb = fmaf(d[J][2], y.x, qb); qb = fmaf(d[J][3], y.y, qb);
-  }
-}
 
 // ------------------------------------------------------------------------------------------------------------------
-// K2: one warp per event (persistent warps, grid-stride over the events of the chunk).
-// CM::at16(i): entry i of the row-major integer colour numerators (global memory).
+// K2: the colour contraction as tensor-core MMAs.  Per gluon-helicity combination, the 8 real vectors x_m (row m = 2
+// (2 h_t + h_tbar) + re/im of X[flow][8]) give  q_m = sum_{I <= J} X_I C'_{IJ} . X_J  over the 8 x 8 tiles of C
+// (C' = C with the diagonal tiles halved; the caller doubles the result: C is symmetric).
+//   A fragment   thread (row = lane / 4, c = lane % 4) holds x_row at the flows 4 idx + c, idx < ncol / 4, loaded
+//                straight from HBM (one 8- or 4-byte load per thread = 256 / 128 contiguous bytes per warp);
+//   B fragment   C' from shared memory in fragment order; the columns of a tile are permuted, n -> flow
+//                8 J + n / 2 + 4 (n % 2), so that the two D columns of a thread are flows 8 J + c and 8 J + c + 4:
+//                flows whose x the thread already holds, and the row dot q_m += D . x needs no second load.
 // ------------------------------------------------------------------------------------------------------------------
+template <int NCOL, typename TC> struct ColFrag;
+
+// fp64: mma.sync m8n8k4 f64, one combination per tile
+template <int NCOL> struct ColFrag<NCOL, double> {
+  static constexpr int GPT = 1, NW = NCOL / 4, NT = NCOL / 8, JB = (NT < 5) ? NT : 5;
+  static_assert(NT % JB == 0, "tile blocking");
+  double a[NW];
+  __device__ __forceinline__ void load(const double* X, int lane) {
+    const double* p = X + (lane & 3) * 8 + (lane >> 2);
+#pragma unroll
+    for (int i = 0; i < NW; i++) a[i] = __ldcg(p + 32 * i);
+  }
+  // cf: [pair(I,J)][k-step s][lane]: B[k = lane % 4][n = lane / 4] = C'[8 I + 4 s + k][8 J + perm(n)]
+  __device__ __forceinline__ void quad(const double* cf, int lane, double& qa, double& qb) const {
+    double q = 0.0;
+#pragma unroll
+    for (int J0 = 0; J0 < NT; J0 += JB) {
+      double d[JB][2];
+#pragma unroll
+      for (int j = 0; j < JB; j++) d[j][0] = d[j][1] = 0.0;
+      // I outer, J inner: consecutive MMAs go to different accumulators
+#pragma unroll
+      for (int I = 0; I < J0 + JB; I++)
+#pragma unroll
+        for (int s = 0; s < 2; s++)
+#pragma unroll
+          for (int j = 0; j < JB; j++) {
+            const int J = J0 + j;
+            if (J >= I) dmma884(d[j][0], d[j][1], a[2 * I + s], cf[((J * (J + 1) / 2 + I) * 2 + s) * 32 + lane]);
+          }
+#pragma unroll
+      for (int j = 0; j < JB; j++) {
+        q = ::fma(d[j][0], a[2 * (J0 + j)], q);
+        q = ::fma(d[j][1], a[2 * (J0 + j) + 1], q);
+      }
+    }
+    qa = q; qb = 0.0;
+  }
+  // w[idx] += |x|^2 of the flows 4 idx + c for the rows whose helicity is good (summed over rows by the caller)
+  __device__ __forceinline__ void weights(double (&w)[NW], bool keepa, bool) const {
+#pragma unroll
+    for (int i = 0; i < NW; i++) w[i] = keepa ? ::fma(a[i], a[i], w[i]) : w[i];
+  }
+};
+
+// fp32 / mixed: mma.sync m16n8k8 tf32, two combinations per tile (rows 0-7 and 8-15); X split as hi + lo with
+// hi = tf32(x), lo = tf32(x - hi): the integer colour numerators are exact in TF32, so every product carries fp32
+// accuracy and the sum accumulates in fp32
+template <int NCOL> struct ColFrag<NCOL, float> {
+  static constexpr int GPT = 2, NW = NCOL / 4, NT = NCOL / 8, JB = (NT < 5) ? NT : 5;
+  static_assert(NT % JB == 0, "tile blocking");
+  float x[NT][4];  // [k-block][a0: group A flow 8 I + c, a1: group B same flow, a2: A flow 8 I + c + 4, a3: B ...]
+  __device__ __forceinline__ void load(const float* X, int lane) {
+    const float* p = X + (lane & 3) * 8 + (lane >> 2);
+#pragma unroll
+    for (int I = 0; I < NT; I++) {
+      x[I][0] = __ldcg(p + 64 * I);
+      x[I][1] = __ldcg(p + NCOL * 8 + 64 * I);
+      x[I][2] = __ldcg(p + 64 * I + 32);
+      x[I][3] = __ldcg(p + NCOL * 8 + 64 * I + 32);
+    }
+  }
+  // cf: [pair(I,J)][lane][2]: b0 = C'[8 I + lane % 4][8 J + perm(lane / 4)], b1 = C'[8 I + lane % 4 + 4][...]
+  __device__ __forceinline__ void quad(const float* cf, int lane, float& qa, float& qb) const {
+    qa = qb = 0.f;
+#pragma unroll
+    for (int J0 = 0; J0 < NT; J0 += JB) {
+      float d[JB][4];
+#pragma unroll
+      for (int j = 0; j < JB; j++) d[j][0] = d[j][1] = d[j][2] = d[j][3] = 0.f;
+#pragma unroll
+      for (int I = 0; I < J0 + JB; I++) {
+        unsigned ah[4], al[4];
+#pragma unroll
+        for (int i = 0; i < 4; i++) {
+          ah[i] = to_tf32(x[I][i]);
+          al[i] = to_tf32(x[I][i] - __uint_as_float(ah[i]));
+        }
+#pragma unroll
+        for (int j = 0; j < JB; j++) {
+          const int J = J0 + j;
+          if (J >= I) {
+            const float2 b = *reinterpret_cast<const float2*>(cf + ((J * (J + 1) / 2 + I) * 32 + lane) * 2);
+            hmma1688(d[j], al, __float_as_uint(b.x), __float_as_uint(b.y));
+            hmma1688(d[j], ah, __float_as_uint(b.x), __float_as_uint(b.y));
+          }
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < JB; j++) {
+        qa = fmaf(d[j][0], x[J0 + j][0], qa); qa = fmaf(d[j][1], x[J0 + j][2], qa);
+        qb = fmaf(d[j][2], x[J0 + j][1], qb); qb = fmaf(d[j][3], x[J0 + j][3], qb);
+      }
+    }
+  }
+  __device__ __forceinline__ void weights(float (&w)[NW], bool keepa, bool keepb) const {
+#pragma unroll
+    for (int I = 0; I < NT; I++) {
+      w[2 * I] = keepa ? fmaf(x[I][0], x[I][0], w[2 * I]) : w[2 * I];
+      w[2 * I] = keepb ? fmaf(x[I][1], x[I][1], w[2 * I]) : w[2 * I];
+      w[2 * I + 1] = keepa ? fmaf(x[I][2], x[I][2], w[2 * I + 1]) : w[2 * I + 1];
+      w[2 * I + 1] = keepb ? fmaf(x[I][3], x[I][3], w[2 * I + 1]) : w[2 * I + 1];
+    }
+  }
+};
+
 template <class G, typename TC> struct ColGeom {
-  static constexpr int WARPS = 8, GPT = ColTraits<TC>::GPT, LD = XGeom<G>::LD, NCOL = G::ncol;
-  static constexpr int TILE = GPT * 8 * LD;                              // TC elements of one staged tile
+  static constexpr int WARPS = 8, GPT = ColFrag<G::ncol, TC>::GPT, NCOL = G::ncol;
   static constexpr int CF = XGeom<G>::NPAIR * 64;                        // TC elements of C' in fragment order
-  static constexpr int PERW = 2 * TILE * (int)sizeof(TC) + (int)sizeof(double) * ((1 << (G::n + 2)) + NCOL);
+  static constexpr int PERW = (int)sizeof(double) * ((1 << (G::n + 2)) + NCOL);   // per warp: |M_h|^2, colour weights
   static constexpr int SMEM = CF * (int)sizeof(TC) + WARPS * PERW;
 };
 
+// One warp per event (persistent warps, grid-stride over the events of the chunk).
+// CM::at16(i): entry i of the row-major integer colour numerators (global memory).
 template <class G, typename TC, class CM, int MODE>
 __global__ void __launch_bounds__(ColGeom<G, TC>::WARPS * 32, 1) colour_kernel(const PipeArgs p) {
   typedef ColGeom<G, TC> CG;
-  constexpr int N = G::n, NPAR = N + 2, NCOMB = 1 << NPAR, NCOL = G::ncol, NT = NCOL / 8, LD = CG::LD, GPT = CG::GPT;
-  constexpr int TILE = CG::TILE;
+  typedef ColFrag<G::ncol, TC> Frag;
+  constexpr int N = G::n, NPAR = N + 2, NCOMB = 1 << NPAR, NCOL = G::ncol, GPT = CG::GPT, NW = Frag::NW;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TC* cf = reinterpret_cast<TC*>(smem_raw);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  unsigned char* wbase = smem_raw + CG::CF * sizeof(TC) + (size_t)warp * CG::PERW;
-  TC* tile = reinterpret_cast<TC*>(wbase);                                   // [2][TILE]
-  double* mh = reinterpret_cast<double*>(wbase + 2 * TILE * sizeof(TC));     // [NCOMB] |M_h|^2 of this warp's event
-  double* wcs = mh + NCOMB;                                                  // [NCOL] colour weights
+  double* mh = reinterpret_cast<double*>(smem_raw + CG::CF * sizeof(TC) + (size_t)warp * CG::PERW);  // [NCOMB]
+  double* wcs = mh + NCOMB;                                                                           // [NCOL]
   const LaunchArgs& a = p.a;
-  // ---- C' (diagonal tiles halved) in MMA fragment order, once per block
+  // ---- C' (diagonal tiles halved, tile columns permuted) in MMA fragment order, once per block
   for (int i = tid; i < CG::CF; i += CG::WARPS * 32) {
-    const int l = i & 31;
-    int pair, ca, cb;
-    if (GPT == 1) {  // fp64: [pair][s][lane], B[k = l%4][n = l/4] of k-step s
-      pair = i >> 6;
-      const int s = (i >> 5) & 1;
-      ca = 4 * s + (l & 3); cb = l >> 2;
-    } else {         // tf32: [pair][lane][2], b0 = B[l%4][l/4], b1 = B[l%4 + 4][l/4]
-      pair = i >> 6;
-      const int l2 = (i >> 1) & 31;
-      ca = (l2 & 3) + 4 * (i & 1); cb = l2 >> 2;
-    }
-    (void)l;
+    const int pair = i >> 6;
+    int ca, n;
+    if (GPT == 1) { const int l = i & 31, s = (i >> 5) & 1; ca = 4 * s + (l & 3); n = l >> 2; }
+    else { const int l = (i >> 1) & 31; ca = (l & 3) + 4 * (i & 1); n = l >> 2; }
     int J = 0;
     while ((J + 1) * (J + 2) / 2 <= pair) J++;
     const int I = pair - J * (J + 1) / 2;
+    const int cb = (n >> 1) + 4 * (n & 1);
     const TC cv = TC(CM::at16((8 * I + ca) * NCOL + 8 * J + cb));
     cf[i] = (I == J) ? TC(0.5) * cv : cv;
   }
@@ -838,76 +865,43 @@ __global__ void __launch_bounds__(ColGeom<G, TC>::WARPS * 32, 1) colour_kernel(c
   const long long w0 = (long long)blockIdx.x * CG::WARPS + warp;
   const int ntile = (p.ncombo + GPT - 1) / GPT;
   const TC* xbase = reinterpret_cast<const TC*>(p.xt);
-  auto stage = [&](long long e, int ti, int buf) {
-    const char* src = reinterpret_cast<const char*>(xbase + ((size_t)e * p.ncombo + (size_t)ti * GPT) * (8 * LD));
-    char* dst = reinterpret_cast<char*>(tile + buf * TILE);
-    for (int i = lane; i < (int)(TILE * sizeof(TC) / 16); i += 32) cp_async16(dst + 16 * i, src + 16 * i);
-    cp_async_commit();
-  };
+  auto tile_ptr = [&](long long e, int ti) { return xbase + ((size_t)e * p.ncombo + (size_t)ti * GPT) * XGeom<G>::GRP; };
   auto is_good = [&](int h) { return MODE == MODE_FILTER || ((a.good.mask[h >> 6] >> (h & 63)) & 1ull) != 0ull; };
-  int buf = 0;
-  if (w0 < a.nevt) stage(w0, 0, 0);
+  const int row = lane >> 2, var = lane >> 3;
+  Frag cur, nxt;
+  if (w0 < a.nevt) cur.load(tile_ptr(w0, 0), lane);
   for (long long e = w0; e < a.nevt; e += wstride) {
     for (int h = lane; h < NCOMB; h += 32) mh[h] = 0.0;
-    TC wc[(NCOL + 31) / 32];
+    TC wacc[NW];
 #pragma unroll
-    for (int k = 0; k < (NCOL + 31) / 32; k++) wc[k] = TC(0);
+    for (int i = 0; i < NW; i++) wacc[i] = TC(0);
     __syncwarp();
 #pragma unroll 1
     for (int ti = 0; ti < ntile; ti++) {
-      // prefetch the next tile (of this event or of the warp's next event) while this one is contracted
+      // the next tile (of this event or of the warp's next event) is on its way while this one is contracted
       const bool more_here = ti + 1 < ntile;
       const long long en = more_here ? e : e + wstride;
-      if (en < a.nevt) stage(en, more_here ? ti + 1 : 0, buf ^ 1);
-      else cp_async_commit();
-      cp_async_wait<1>();
-      __syncwarp();
-      const TC* xt = tile + buf * TILE;
+      if (en < a.nevt) nxt.load(tile_ptr(en, more_here ? ti + 1 : 0), lane);
       // ---- a6 on the tensor cores
-      if constexpr (GPT == 1) {
-        double q = quad_tile<NCOL>(xt, cf, lane);
-        q += __shfl_xor_sync(0xffffffffu, q, 1);
-        q += __shfl_xor_sync(0xffffffffu, q, 2);   // row m = lane / 4 complete
-        q += __shfl_xor_sync(0xffffffffu, q, 4);   // re + im rows of variant v = lane / 8
-        if ((lane & 7) == 0) mh[grp_hel_of<N>(p.combo[ti], lane >> 3)] = 2.0 * q;
-      } else {
-        float qa, qb;
-        quad_tile<NCOL>(xt, cf, lane, qa, qb);
-        qa += __shfl_xor_sync(0xffffffffu, qa, 1); qb += __shfl_xor_sync(0xffffffffu, qb, 1);
-        qa += __shfl_xor_sync(0xffffffffu, qa, 2); qb += __shfl_xor_sync(0xffffffffu, qb, 2);
-        qa += __shfl_xor_sync(0xffffffffu, qa, 4); qb += __shfl_xor_sync(0xffffffffu, qb, 4);
-        if ((lane & 7) == 0) {
-          mh[grp_hel_of<N>(p.combo[2 * ti], lane >> 3)] = (double)(2.f * qa);
-          if (2 * ti + 1 < p.ncombo) mh[grp_hel_of<N>(p.combo[2 * ti + 1], lane >> 3)] = (double)(2.f * qb);
-        }
+      TC qa, qb;
+      cur.quad(cf, lane, qa, qb);
+      qa += __shfl_xor_sync(0xffffffffu, qa, 1); qb += __shfl_xor_sync(0xffffffffu, qb, 1);
+      qa += __shfl_xor_sync(0xffffffffu, qa, 2); qb += __shfl_xor_sync(0xffffffffu, qb, 2);   // row m complete
+      qa += __shfl_xor_sync(0xffffffffu, qa, 4); qb += __shfl_xor_sync(0xffffffffu, qb, 4);   // re + im rows
+      const int ca = ti * GPT, cb = ti * GPT + 1;
+      if ((lane & 7) == 0) {
+        mh[grp_hel_of<N>(p.combo[ca], var)] = (double)(TC(2) * qa);
+        if (GPT == 2 && cb < p.ncombo) mh[grp_hel_of<N>(p.combo[cb], var)] = (double)(TC(2) * qb);
       }
       if (MODE == MODE_SELECT) {
-        // a8 colour weights w_c += sum over the good (h_t, h_tbar) of |J_c|^2: lane = flow
-#pragma unroll
-        for (int g = 0; g < GPT; g++) {
-          const int ci = ti * GPT + g;
-          if (ci < p.ncombo) {
-            const int gm = p.vmask[ci];
-#pragma unroll
-            for (int k = 0; k < (NCOL + 31) / 32; k++) {
-              const int c = lane + 32 * k;
-              if (c < NCOL) {
-                TC w = TC(0);
-#pragma unroll
-                for (int v = 0; v < 4; v++) {
-                  const TC keep = ((gm >> v) & 1) ? TC(1) : TC(0);
-                  const TC xr = xt[(g * 8 + 2 * v) * LD + c], xi = xt[(g * 8 + 2 * v + 1) * LD + c];
-                  w += keep * (xr * xr + xi * xi);
-                }
-                wc[k] += w;
-              }
-            }
-          }
-        }
+        // a8 colour weights: |J_c|^2 of the good (h_t, h_tbar) rows, per thread for its row; rows are added below
+        const bool ka = (p.vmask[ca] >> (row >> 1)) & 1;
+        const bool kb = (GPT == 2 && cb < p.ncombo) ? ((p.vmask[cb] >> (row >> 1)) & 1) : false;
+        cur.weights(wacc, ka, kb);
       }
-      __syncwarp();  // every lane is done with this buffer before it is refilled
-      buf ^= 1;
+      cur = nxt;
     }
+    __syncwarp();
     // ---- a7-a9 for this event
     if (MODE == MODE_FILTER) {
       double total = 0.0;
@@ -938,9 +932,15 @@ __global__ void __launch_bounds__(ColGeom<G, TC>::WARPS * 32, 1) colour_kernel(c
         }
       }
       if (MODE == MODE_SELECT && a.selcol) {
+        // rows 0..7 of the warp hold partial weights of the same flows: add them, lanes 0..3 publish flow 4 idx + c
 #pragma unroll
-        for (int k = 0; k < (NCOL + 31) / 32; k++)
-          if (lane + 32 * k < NCOL) wcs[lane + 32 * k] = (double)wc[k];
+        for (int i = 0; i < NW; i++) {
+          TC w = wacc[i];
+          w += __shfl_xor_sync(0xffffffffu, w, 4);
+          w += __shfl_xor_sync(0xffffffffu, w, 8);
+          w += __shfl_xor_sync(0xffffffffu, w, 16);
+          if (lane < 4) wcs[4 * i + lane] = (double)w;
+        }
         __syncwarp();
         constexpr int PER = (NCOL + 31) / 32;
         double val[PER];
@@ -959,7 +959,6 @@ __global__ void __launch_bounds__(ColGeom<G, TC>::WARPS * 32, 1) colour_kernel(c
     }
     __syncwarp();
   }
-  cp_async_wait<0>();
 }
 
 }  // namespace me

@@ -43,7 +43,7 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
   typedef me::GrpGeom<Grp, TA> GE;
   typedef me::ColGeom<Grp, TCo> CG;
   typedef me::GrpEvent<TA, Grp::n> EV;
-  constexpr int N = Grp::n, LD = me::XGeom<Grp>::LD;
+  constexpr int N = Grp::n;
   auto k0 = me::setup_kernel<TA, N>;
   auto k1 = me::amp_kernel<Grp, TA, TCo, ME_MINB>;
   auto k2 = me::colour_kernel<Grp, TCo, CMat, MODE>;
@@ -58,7 +58,7 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     }
     if (m) { p.combo[p.ncombo] = (unsigned char)gg; p.vmask[p.ncombo] = (unsigned char)m; p.ncombo++; }
   }
-  const size_t evb = sizeof(EV), grpb = (size_t)8 * LD * sizeof(TCo);
+  const size_t evb = sizeof(EV), grpb = (size_t)me::XGeom<Grp>::GRP * sizeof(TCo);
   const size_t per_event = evb + (size_t)p.ncombo * grpb, slack = 2 * grpb + 512;
   long long chunk = (a.scratch_bytes > slack) ? (long long)((a.scratch_bytes - slack) / per_event) : 0;
   if (chunk > (1 << 20)) chunk = 1 << 20;
@@ -82,10 +82,16 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
   }
   if (dry || a.nevt == 0) return 0;
   if (p.ncombo == 0 || chunk < 1 || !a.scratch) return (int)cudaErrorInvalidValue;
+  // shared memory: what ME_MINB amplitude warps need and no more (the rest of the 256 KB stays L1 for the table words)
+  int carve = (int)((size_t)ME_MINB * (GE::SMEM + 1024) * 100 / (228 * 1024)) + 1;
+  if (carve > 100) carve = 100;
   err = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, GE::SMEM);
-  if (err == cudaSuccess) err = cudaFuncSetAttribute(k1, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  if (err == cudaSuccess) err = cudaFuncSetAttribute(k1, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
   if (err == cudaSuccess) err = cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, CG::SMEM);
+  int k2_per_sm = 1;
+  if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&k2_per_sm, k2, CG::WARPS * 32, CG::SMEM);
   if (err != cudaSuccess) return (int)err;
+  if (k2_per_sm < 1) k2_per_sm = 1;
   for (long long e0 = 0; e0 < a.nevt; e0 += chunk) {
     const long long n = (a.nevt - e0 < chunk) ? (a.nevt - e0) : chunk;
     p.a = a;
@@ -103,7 +109,7 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     k0<<<(unsigned)((n * PT + 127) / 128), 128, 0, st>>>(p.a, (EV*)p.ev);
     k1<<<(unsigned)(n * nunit), 32, GE::SMEM, st>>>(p);
     long long b2 = (n + CG::WARPS - 1) / CG::WARPS;
-    if (b2 > sms) b2 = sms;
+    if (b2 > (long long)sms * k2_per_sm) b2 = (long long)sms * k2_per_sm;
     k2<<<(unsigned)b2, CG::WARPS * 32, CG::SMEM, st>>>(p);
     err = cudaGetLastError();
     if (err != cudaSuccess) return (int)err;
