@@ -57,6 +57,8 @@ struct me_handle {
   // lane-group pipeline (gg_ttgg, gg_ttggg): per-event data and jamps between its kernels, one chunk of events
   void* d_scratch;
   size_t scratch_bytes;
+  me::PipeCtx pipe;   // internal streams / events of the pipeline (valid iff d_scratch)
+  bool have_pipe;
   // staging for me_compute_host
   void* d_stage;
   size_t stage_bytes;
@@ -180,7 +182,8 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
   }
   h->have_good = false; h->good.n = 0;
   h->d_cum = nullptr; h->cum_bytes = 0; h->d_frac = nullptr; h->d_stage = nullptr; h->stage_bytes = 0;
-  h->d_scratch = nullptr; h->scratch_bytes = 0;
+  h->d_scratch = nullptr; h->scratch_bytes = 0; h->have_pipe = false;
+  memset(&h->pipe, 0, sizeof(h->pipe));
   h->own_stream = nullptr;
   memset(&h->last, 0, sizeof(h->last));
   DeviceGuard guard(device);
@@ -213,6 +216,23 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
         return rc;
       }
       h->scratch_bytes = want;
+      // internal streams: two for the setup + amplitude kernels of alternating chunks, a high-priority one for the
+      // colour kernels; events carry the dependencies (nothing is synchronised on the host)
+      int lo = 0, hi = 0;
+      e = cudaDeviceGetStreamPriorityRange(&lo, &hi);
+      me::PipeCtx& px = h->pipe;
+      if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&px.sa, cudaStreamNonBlocking, lo);
+      if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&px.sb, cudaStreamNonBlocking, lo);
+      if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&px.s2, cudaStreamNonBlocking, hi);
+      cudaEvent_t* evs[5] = {&px.fork, &px.k1[0], &px.k1[1], &px.k2[0], &px.k2[1]};
+      for (int i = 0; i < 5 && e == cudaSuccess; i++) e = cudaEventCreateWithFlags(evs[i], cudaEventDisableTiming);
+      if (e != cudaSuccess) {
+        int rc = cuda_fail(nullptr, e, "me_create: pipeline streams");
+        cudaFree(h->d_scratch); cudaFree(h->d_frac);
+        delete h;
+        return rc;
+      }
+      h->have_pipe = true;
     }
   }
   *out = h;
@@ -222,6 +242,11 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
 int me_destroy(me_handle* h) {
   if (!h) return ME_ERR_ARG;
   DeviceGuard guard(h->device);
+  if (h->have_pipe) {
+    cudaStreamDestroy(h->pipe.sa); cudaStreamDestroy(h->pipe.sb); cudaStreamDestroy(h->pipe.s2);
+    cudaEventDestroy(h->pipe.fork);
+    for (int i = 0; i < 2; i++) { cudaEventDestroy(h->pipe.k1[i]); cudaEventDestroy(h->pipe.k2[i]); }
+  }
   if (h->d_scratch) cudaFree(h->d_scratch);
   if (h->d_cum) cudaFree(h->d_cum);
   if (h->d_frac) cudaFree(h->d_frac);
@@ -310,7 +335,7 @@ int me_filter_helicities(me_handle* h, const double* d_momenta, const double* d_
   memset(&a, 0, sizeof(a));
   a.mom = d_momenta; a.gs = d_gs; a.nevt = nevt < 16384 ? nevt : 16384;
   a.fracmax = h->d_frac; a.par = h->par;
-  a.scratch = h->d_scratch; a.scratch_bytes = h->scratch_bytes;
+  a.scratch = h->d_scratch; a.scratch_bytes = h->scratch_bytes; a.pipe = h->have_pipe ? &h->pipe : nullptr;
   int ce = h->proc->fn[0](a, me::MODE_FILTER, stream, nullptr, 0);  // always the fp64 build (reading R10)
   if (ce) return cuda_fail(h, (cudaError_t)ce, "me_filter_helicities: launch");
   unsigned long long bits[128];
@@ -371,7 +396,7 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
   memset(&a, 0, sizeof(a));
   a.mom = d_momenta; a.gs = d_gs; a.rndhel = d_rndhel; a.rndcol = d_rndcol; a.nevt = nevt;
   a.me = d_me; a.selhel = d_selhel; a.selcol = d_selcol; a.par = h->par; a.good = h->good;
-  a.scratch = h->d_scratch; a.scratch_bytes = h->scratch_bytes;
+  a.scratch = h->d_scratch; a.scratch_bytes = h->scratch_bytes; a.pipe = h->have_pipe ? &h->pipe : nullptr;
   a.good.mask[0] = a.good.mask[1] = 0ull;
   for (int i = 0; i < a.good.n; i++) a.good.mask[a.good.h[i] >> 6] |= 1ull << (a.good.h[i] & 63);
   const int mode = (d_selhel || d_selcol) ? me::MODE_SELECT : me::MODE_ME;

@@ -34,8 +34,17 @@ struct LaunchArgs {
   int blocks;                  // 0 = choose
   void* scratch;               // lane-group pipeline: per-event data and jamps between its kernels (owned by the handle)
   size_t scratch_bytes;
+  const struct PipeCtx* pipe;  // lane-group pipeline: the handle's internal streams and events (host side only)
   DevParams par;
   GoodList good;
+};
+
+// Internal streams of a handle (lane-group pipeline): consecutive chunks of events alternate between sa and sb
+// (setup + amplitude kernels) so that the tail of one chunk's amplitude kernel is filled by the next chunk's, and
+// every colour kernel runs on the high-priority stream s2 beside the amplitude kernel of the following chunk.
+struct PipeCtx {
+  cudaStream_t sa, sb, s2;
+  cudaEvent_t fork, k1[2], k2[2];
 };
 
 struct LaunchInfo {

@@ -59,10 +59,21 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     if (m) { p.combo[p.ncombo] = (unsigned char)gg; p.vmask[p.ncombo] = (unsigned char)m; p.ncombo++; }
   }
   const size_t evb = sizeof(EV), grpb = (size_t)me::XGeom<Grp>::GRP * sizeof(TCo);
-  const size_t per_event = evb + (size_t)p.ncombo * grpb, slack = 2 * grpb + 512;
-  long long chunk = (a.scratch_bytes > slack) ? (long long)((a.scratch_bytes - slack) / per_event) : 0;
-  if (chunk > (1 << 20)) chunk = 1 << 20;
+  const size_t per_event = evb + (size_t)p.ncombo * grpb, slack = 2 * grpb + 1024;
   const int nunit = (p.ncombo + GE::GPW - 1) / GE::GPW;
+  // Chunks: the scratch is used as two halves; with at least two chunks, consecutive chunks run on alternating
+  // internal streams and the colour kernel of chunk c overlaps the amplitude kernel of chunk c + 1.
+  const size_t half = (a.scratch_bytes / 2) & ~(size_t)255;
+  long long cap = (half > slack) ? (long long)((half - slack) / per_event) : 0;   // events per half
+  if (cap > (1 << 20)) cap = 1 << 20;
+  const long long min_chunk = (8 * 1184 + nunit - 1) / nunit;   // >= 8 waves of amplitude warps on 148 SMs
+  long long chunk = cap;
+  if (chunk > 0 && a.nevt > 0) {
+    long long want = (a.nevt + 3) / 4;                            // aim at four chunks per call
+    if (want < min_chunk) want = min_chunk;
+    if (want < chunk) chunk = want;
+  }
+  const long long nchunks = (chunk > 0) ? (a.nevt + chunk - 1) / chunk : 0;
   int dev = 0, sms = 0;
   cudaError_t err = cudaGetDevice(&dev);
   if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -78,7 +89,7 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     info->cum_slots = 0;
     info->scratch_per_event = (long long)(sizeof(EV) + (size_t)GE::NGRP * grpb);
     info->chunk = chunk;
-    info->launches = (chunk > 0) ? (int)(3 * ((a.nevt + chunk - 1) / chunk)) : 0;
+    info->launches = (int)(3 * nchunks);
   }
   if (dry || a.nevt == 0) return 0;
   if (p.ncombo == 0 || chunk < 1 || !a.scratch) return (int)cudaErrorInvalidValue;
@@ -92,8 +103,19 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
   if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&k2_per_sm, k2, CG::WARPS * 32, CG::SMEM);
   if (err != cudaSuccess) return (int)err;
   if (k2_per_sm < 1) k2_per_sm = 1;
-  for (long long e0 = 0; e0 < a.nevt; e0 += chunk) {
+  const me::PipeCtx* px = (nchunks > 1) ? a.pipe : nullptr;
+  if (px) {  // fork: the internal streams start after everything already enqueued on the caller's stream
+    err = cudaEventRecord(px->fork, st);
+    if (err == cudaSuccess) err = cudaStreamWaitEvent(px->sa, px->fork, 0);
+    if (err == cudaSuccess) err = cudaStreamWaitEvent(px->sb, px->fork, 0);
+    if (err == cudaSuccess) err = cudaStreamWaitEvent(px->s2, px->fork, 0);
+    if (err != cudaSuccess) return (int)err;
+  }
+  long long c = 0;
+  for (long long e0 = 0; e0 < a.nevt; e0 += chunk, c++) {
     const long long n = (a.nevt - e0 < chunk) ? (a.nevt - e0) : chunk;
+    const int hf = (int)(c & 1);
+    char* base = (char*)a.scratch + (px ? (size_t)hf * half : 0);
     p.a = a;
     p.a.nevt = n;
     p.a.mom = a.mom + e0 * (Grp::npar * 4);
@@ -103,15 +125,26 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     p.a.me = a.me ? a.me + e0 : nullptr;
     p.a.selhel = a.selhel ? a.selhel + e0 : nullptr;
     p.a.selcol = a.selcol ? a.selcol + e0 : nullptr;
-    p.ev = a.scratch;
-    p.xt = (char*)a.scratch + align_up((size_t)n * evb, 256);
+    p.ev = base;
+    p.xt = base + align_up((size_t)n * evb, 256);
     constexpr int PT = ((1 << N) + N + 6 <= 32) ? 32 : 64;
-    k0<<<(unsigned)((n * PT + 127) / 128), 128, 0, st>>>(p.a, (EV*)p.ev);
-    k1<<<(unsigned)(n * nunit), 32, GE::SMEM, st>>>(p);
+    cudaStream_t s1 = px ? (hf ? px->sb : px->sa) : st, s2 = px ? px->s2 : st;
+    if (px && c >= 2 && (err = cudaStreamWaitEvent(s1, px->k2[hf], 0)) != cudaSuccess) return (int)err;  // half free again
+    k0<<<(unsigned)((n * PT + 127) / 128), 128, 0, s1>>>(p.a, (EV*)p.ev);
+    k1<<<(unsigned)(n * nunit), 32, GE::SMEM, s1>>>(p);
+    if (px) {
+      if ((err = cudaEventRecord(px->k1[hf], s1)) != cudaSuccess) return (int)err;
+      if ((err = cudaStreamWaitEvent(s2, px->k1[hf], 0)) != cudaSuccess) return (int)err;
+    }
     long long b2 = (n + CG::WARPS - 1) / CG::WARPS;
     if (b2 > (long long)sms * k2_per_sm) b2 = (long long)sms * k2_per_sm;
-    k2<<<(unsigned)b2, CG::WARPS * 32, CG::SMEM, st>>>(p);
+    k2<<<(unsigned)b2, CG::WARPS * 32, CG::SMEM, s2>>>(p);
+    if (px && (err = cudaEventRecord(px->k2[hf], s2)) != cudaSuccess) return (int)err;
     err = cudaGetLastError();
+    if (err != cudaSuccess) return (int)err;
+  }
+  if (px) {  // join: the caller's stream continues after the last colour kernel (s2 is in order, and follows sa / sb)
+    err = cudaStreamWaitEvent(st, px->k2[(int)((c - 1) & 1)], 0);
     if (err != cudaSuccess) return (int)err;
   }
   return 0;
