@@ -27,7 +27,7 @@ NVCC_BASE = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", 
 # launch configuration per (process, precision): threads per block, min blocks per SM (register cap)
 TUNE = {
     # lane-group pipeline: the amplitude kernel runs one warp per block; min blocks/SM caps its registers
-    ("gg_ttggg", 0): (32, 6), ("gg_ttggg", 1): (32, 12), ("gg_ttggg", 2): (32, 6),
+    ("gg_ttggg", 0): (32, 9), ("gg_ttggg", 1): (32, 16), ("gg_ttggg", 2): (32, 9),
     ("gg_ttgg", 0): (32, 8), ("gg_ttgg", 1): (32, 16), ("gg_ttgg", 2): (32, 8),
 }
 DEFAULT_TUNE = (128, 1)

@@ -36,6 +36,10 @@
 
 #include "me_kernels.cuh"
 
+#ifndef ME_UNROLL_T
+#define ME_UNROLL_T 1   // unroll factor of the term loops of the tree (loads of term j + 1 overlap the arithmetic of term j)
+#endif
+
 namespace me {
 
 // Packed pair of floats: lane-local SIMD over the two t helicities of the quark-line walk in the fp32 build
@@ -284,6 +288,18 @@ struct alignas(16) GrpEvent {
   T mt;
 };
 
+// Where the contracted full-length currents ("init": the j = 0 term of every jamp) wait for the walk: in the jamp
+// buffer itself (HBM/L2; the leaf reads, adds and overwrites) when shared memory bounds the number of resident warps
+// (n = 5: 6 -> 9 warps per SM in fp64, measured +9 % fp64, +30 % mixed), in shared memory when registers do (n = 4:
+// the extra global round trip costs 7-15 %, measured).
+template <class G> struct GrpInit {
+#ifdef ME_INIT_GLOBAL
+  static constexpr bool GLOBAL = (ME_INIT_GLOBAL != 0);
+#else
+  static constexpr bool GLOBAL = (G::n >= 5);
+#endif
+};
+
 template <class G, typename T>
 struct GrpGeom {
   // HTL: both t helicities are walked by the same lane (every current loaded from shared memory feeds two
@@ -296,7 +312,7 @@ struct GrpGeom {
   static constexpr int N = G::n, NHT = HTL ? 2 : 1, LPG = HTL ? N : 2 * N, GPW = 32 / LPG, NGRP = 1 << N;
   // T units per group: current slots + contracted full-length currents ("init"); padded so that the byte stride
   // is 32 mod 128
-  static constexpr int RAW = (G::nslot + G::ninit) * 8;
+  static constexpr int RAW = (G::nslot + (GrpInit<G>::GLOBAL ? 0 : G::ninit)) * 8;
   static constexpr int UNIT = 32 / (int)sizeof(T);  // T units in 32 bytes
   static constexpr int GS = ((RAW + 4 * UNIT - 1) / (4 * UNIT)) * (4 * UNIT) + UNIT;
   static constexpr int EVB = (((int)sizeof(GrpEvent<T, G::n>) + 127) / 128) * 128;
@@ -429,12 +445,14 @@ __global__ void __launch_bounds__(128) setup_kernel(const LaunchArgs a, GrpEvent
 // ------------------------------------------------------------------------------------------------------------------
 // K1 pieces
 // ------------------------------------------------------------------------------------------------------------------
+template <class G, typename T, typename TC> struct GrpWalkCtx;
+
 // Colour-ordered gluon currents of one group, level by level (|seq| = 2 .. n).  One copy of the vertex code: the
 // levels, the tasks of a level and the terms of a task are run-time loops over the generated tables (keeps the
 // kernel small enough for the instruction cache; the loop bodies are ~100 FMA-pipe instructions each).
-template <class G, typename T>
-__device__ __forceinline__ void grp_tree(const GrpEvent<T, G::n>& ev, T* slots, int r, bool active) {
-  constexpr int LPG = GrpGeom<G, T>::LPG;
+template <class G, typename T, typename TC>
+__device__ __forceinline__ void grp_tree(const GrpEvent<T, G::n>& ev, T* slots, TC* X, int r, bool active) {
+  constexpr int LPG = GrpGeom<G, T>::LPG, UT = ME_UNROLL_T;
 #pragma unroll 1
   for (int L = 2; L <= G::n; L++) {
     const int NV3 = L - 1, NV4 = (L - 1) * (L - 2) / 2, W = 2 + NV3 + NV4;
@@ -448,14 +466,14 @@ __device__ __forceinline__ void grp_tree(const GrpEvent<T, G::n>& ev, T* slots, 
         const unsigned* tw = tab + t * W;
         const unsigned h0 = __ldg(tw);
         vec4<T> acc = zero_vec4<T>();
-#pragma unroll 1
+#pragma unroll(UT)
         for (int j = 0; j < NV3; j++) {
           const unsigned w = __ldg(tw + 2 + j);
           const vec4<T> A = GrpSlot<T>::ld(slots, w & 255u, w >> 31);
           const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
           v3_acc(acc, A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
         }
-#pragma unroll 1
+#pragma unroll(UT)
         for (int j = 0; j < NV4; j++) {
           const unsigned w = __ldg(tw + 2 + NV3 + j);
           const vec4<T> A = GrpSlot<T>::ld(slots, w & 255u, w >> 31);
@@ -470,13 +488,30 @@ __device__ __forceinline__ void grp_tree(const GrpEvent<T, G::n>& ev, T* slots, 
           GrpSlot<T>::st(slots, h0 & 255u, acc);
         } else {
           // the full-length current is contracted at once with the four t-tbar currents: the j = 0 term of the
-          // jamps of this sequence and of its reverse ("init" slot t, read by the leaves of the walk)
-          T* ji = slots + (G::nslot + t) * 8;
+          // jamps of this sequence and of its reverse
+          if constexpr (GrpInit<G>::GLOBAL) {
+            // ... parked in the jamp buffer itself (rows of the two flows), where the leaves of the walk pick it
+            // up: it stays in L2 until the leaf overwrites it with the finished jamp
+            const unsigned h1 = __ldg(tw + 1);
+            TC* ja = X + (h1 & 127u) * 8;
+            TC* jb = X + ((h1 >> 8) & 127u) * 8;
+            const T sb = (h1 >> 31) ? T(-1) : T(1);
 #pragma unroll
-          for (int v = 0; v < 4; v++) {
-            const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
-            const cx<T> a = mdot(q, acc);
-            ji[2 * v] = a.re; ji[2 * v + 1] = a.im;
+            for (int v = 0; v < 4; v++) {
+              const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
+              const cx<T> a = mdot(q, acc);
+              GrpWalkCtx<G, T, TC>::st2(ja + 2 * v, TC(a.re), TC(a.im));
+              GrpWalkCtx<G, T, TC>::st2(jb + 2 * v, TC(sb * a.re), TC(sb * a.im));
+            }
+          } else {
+            // ... in "init" slot t of shared memory, read by the leaves of the walk
+            T* ji = slots + (G::nslot + t) * 8;
+#pragma unroll
+            for (int v = 0; v < 4; v++) {
+              const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
+              const cx<T> a = mdot(q, acc);
+              ji[2 * v] = a.re; ji[2 * v + 1] = a.im;
+            }
           }
         }
       }
@@ -521,22 +556,27 @@ struct GrpWalkCtx {
   }
   __device__ __forceinline__ static f2 pack(float x, float y) { return mkf2(x, y); }
   __device__ __forceinline__ static double pack(double x, double) { return x; }
-  // J_flow(h_t, b) = sg * init + a  ->  X[flow][2 (2 h_t + b) + re/im]; stores bypass L1 (the table words live there)
+  // J_flow(h_t, b) = init + a  ->  X[flow][2 (2 h_t + b) + re/im]; stores bypass L1 (the table words live there)
   __device__ __forceinline__ static void st2(double* q, double x, double y) { __stcg(reinterpret_cast<double2*>(q), make_double2(x, y)); }
   __device__ __forceinline__ static void st2(float* q, float x, float y) { __stcg(reinterpret_cast<float2*>(q), make_float2(x, y)); }
-  __device__ __forceinline__ void put(const T* ji, T sg, int f, int h, int b, f2 re, f2 im) const {
-    TC* q = X + f * 8;
-    st2(q + 2 * b, TC(fmaf(sg, ji[2 * b], re.v.x)), TC(fmaf(sg, ji[2 * b + 1], im.v.x)));              // h_t = 0: v = b
-    st2(q + 4 + 2 * b, TC(fmaf(sg, ji[4 + 2 * b], re.v.y)), TC(fmaf(sg, ji[5 + 2 * b], im.v.y)));      // h_t = 1: v = 2 + b
-  }
-  template <typename S> __device__ __forceinline__ void put(const T* ji, T sg, int f, int h, int b, S re, S im) const {
-    const int v = 2 * h + b;
-    st2(X + f * 8 + 2 * v, TC(fmad<T>(sg, ji[2 * v], re)), TC(fmad<T>(sg, ji[2 * v + 1], im)));
-  }
+  __device__ __forceinline__ static void ld2(const double* q, double& x, double& y) { const double2 t = __ldcg(reinterpret_cast<const double2*>(q)); x = t.x; y = t.y; }
+  __device__ __forceinline__ static void ld2(const float* q, float& x, float& y) { const float2 t = __ldcg(reinterpret_cast<const float2*>(q)); x = t.x; y = t.y; }
   __device__ __forceinline__ void leaf(const spin4<PS> (&Xs)[WP::NCH], unsigned w) const {
+    constexpr bool HTL = GrpGeom<G, T>::HTL;
+    constexpr int NV = HTL ? 4 : 2;          // (h_t, b) values this lane completes: v = v0 + k
     const int f = (w >> 16) & 127;
-    const T* ji = slots + (w & 255u) * 8;
-    const T sg = (w >> 31) ? T(-1) : T(1);
+    const int v0 = HTL ? 0 : 2 * ht;
+    TC* q = X + f * 8 + 2 * v0;
+    T ini[NV][2];
+    if constexpr (GrpInit<G>::GLOBAL) {
+#pragma unroll
+      for (int k = 0; k < NV; k++) { TC x, y; ld2(q + 2 * k, x, y); ini[k][0] = T(x); ini[k][1] = T(y); }
+    } else {
+      const T* ji = slots + (w & 255u) * 8 + 2 * v0;
+      const T sg = (w >> 31) ? T(-1) : T(1);
+#pragma unroll
+      for (int k = 0; k < NV; k++) { ini[k][0] = sg * ji[2 * k]; ini[k][1] = sg * ji[2 * k + 1]; }
+    }
 #pragma unroll
     for (int b = 0; b < 2; b++) {
       const spin4<T> vb = ld_spin<T>(ev->v[b]);
@@ -546,9 +586,19 @@ struct GrpWalkCtx {
 #pragma unroll
       for (int c = 0; c < WP::NCH; c++) {
         const cx<PS> a = row_col(Xs[c], vw);
-        put(ji, sg, f, GrpGeom<G, T>::HTL ? c : ht, b, a.re, a.im);
+        fin(q, ini, HTL ? c : 0, b, a.re, a.im);
       }
     }
+  }
+  // finished jamp(s) of (chain c, b): packed pair = both h_t at once
+  __device__ __forceinline__ static void fin(TC* q, const T (&ini)[GrpGeom<G, T>::HTL ? 4 : 2][2], int c, int b, f2 re, f2 im) {
+    st2(q + 2 * b, TC(ini[b][0] + re.v.x), TC(ini[b][1] + im.v.x));                  // h_t = 0: v = b
+    st2(q + 4 + 2 * b, TC(ini[2 + b][0] + re.v.y), TC(ini[2 + b][1] + im.v.y));      // h_t = 1: v = 2 + b
+  }
+  template <typename S>
+  __device__ __forceinline__ static void fin(TC* q, const T (&ini)[GrpGeom<G, T>::HTL ? 4 : 2][2], int c, int b, S re, S im) {
+    const int k = 2 * c + b;   // HTL: c = h_t; otherwise c = 0 and q already points at the lane's h_t
+    st2(q + 2 * k, TC(ini[k][0] + re), TC(ini[k][1] + im));
   }
 };
 
@@ -622,43 +672,47 @@ __global__ void __launch_bounds__(32, MINB) amp_kernel(const PipeArgs p) {
   const int lane = threadIdx.x;
   const int gi = lane / LPG, r = lane - gi * LPG;
   const int nunit = (p.ncombo + GPW - 1) / GPW;
-  const long long e = blockIdx.x / nunit;
-  const int unit = (int)(blockIdx.x - e * nunit);
   T* slots = gbase + (size_t)((gi < GPW) ? gi : 0) * GE::GS;
-  // ---- a1: the event's helicity-independent data (K0), HBM -> shared memory, 16 bytes per lane and step
+  // One warp per (event, unit).  (Persistent warps over a range of units measured 0-12 % slower: warps that start at
+  // different times mix their tree and walk phases on the FP64 pipe, persistent ones run them in step.)
   {
-    const int4* src = reinterpret_cast<const int4*>(reinterpret_cast<const EV*>(p.ev) + e);
-    int4* dst = reinterpret_cast<int4*>(&ev);
+    const long long e = blockIdx.x / nunit;
+    const int unit = (int)(blockIdx.x - e * nunit);
+    {
+      // ---- a1: the event's helicity-independent data (K0), HBM -> shared memory past L1 (the table words live there)
+      const int4* src = reinterpret_cast<const int4*>(reinterpret_cast<const EV*>(p.ev) + e);
+      int4* dst = reinterpret_cast<int4*>(&ev);
 #pragma unroll 4
-    for (int i = lane; i < (int)(sizeof(EV) / 16); i += 32) dst[i] = __ldg(src + i);
-  }
-  __syncwarp();
-  const int ci = unit * GPW + gi;                       // position in the list of combinations
-  const bool active = (gi < GPW) && (ci < p.ncombo);
-  const int grp = p.combo[active ? ci : 0];             // gluon-helicity combination
-  // ---- a2: polarisation vectors of this group's gluon helicities
-  if (active && r < N) {
-    const int pp = (r < 2) ? r : r + 2;
-    const int lam = ((grp >> (N - 1 - r)) & 1) ? 1 : -1;
-    polbasis<T> pb;
-    for (int c = 0; c < 3; c++) { pb.e1[c] = ev.pol[r][c]; pb.e2[c] = ev.pol[r][3 + c]; }
-    GrpSlot<T>::st(slots, r, polvec(pb, lam, pp >= 2));
-  }
-  __syncwarp();
-  // ---- a3: colour-ordered gluon currents, level by level; the full-length ones are contracted with Q
-  grp_tree<G, T>(ev, slots, r, active);
-  // ---- a3-a5: quark line; every leaf completes one jamp and stores it
-  if (active) {
-    typedef GrpWalkCtx<G, T, TC> Ctx;
-    Ctx c;
-    c.ev = &ev; c.slots = slots;
-    c.X = reinterpret_cast<TC*>(p.xt) + ((size_t)e * p.ncombo + ci) * XGeom<G>::GRP;
-    c.stream = G::role(GE::HTL ? r : (r >> 1));
-    c.ht = GE::HTL ? 0 : (r & 1);
-    spin4<typename Ctx::PS> psi[Ctx::WP::NCH][G::n];
+      for (int i = lane; i < (int)(sizeof(EV) / 16); i += 32) dst[i] = __ldcg(src + i);
+    }
+    __syncwarp();
+    const int ci = unit * GPW + gi;                       // position in the list of combinations
+    const bool active = (gi < GPW) && (ci < p.ncombo);
+    const int grp = p.combo[active ? ci : 0];             // gluon-helicity combination
+    // ---- a2: polarisation vectors of this group's gluon helicities
+    if (active && r < N) {
+      const int pp = (r < 2) ? r : r + 2;
+      const int lam = ((grp >> (N - 1 - r)) & 1) ? 1 : -1;
+      polbasis<T> pb;
+      for (int c = 0; c < 3; c++) { pb.e1[c] = ev.pol[r][c]; pb.e2[c] = ev.pol[r][3 + c]; }
+      GrpSlot<T>::st(slots, r, polvec(pb, lam, pp >= 2));
+    }
+    __syncwarp();
+    // ---- a3: colour-ordered gluon currents, level by level; the full-length ones are contracted with Q
+    grp_tree<G, T, TC>(ev, slots, reinterpret_cast<TC*>(p.xt) + ((size_t)e * p.ncombo + (active ? ci : 0)) * XGeom<G>::GRP, r, active);
+    // ---- a3-a5: quark line; every leaf completes one jamp and stores it
+    if (active) {
+      typedef GrpWalkCtx<G, T, TC> Ctx;
+      Ctx c;
+      c.ev = &ev; c.slots = slots;
+      c.X = reinterpret_cast<TC*>(p.xt) + ((size_t)e * p.ncombo + ci) * XGeom<G>::GRP;
+      c.stream = G::role(GE::HTL ? r : (r >> 1));
+      c.ht = GE::HTL ? 0 : (r & 1);
+      spin4<typename Ctx::PS> psi[Ctx::WP::NCH][G::n];
 #pragma unroll
-    for (int h = 0; h < Ctx::WP::NCH; h++) psi[h][0] = c.psi0(h);
-    GrpWalk<G, T, TC, 1>::node(c, psi);
+      for (int h = 0; h < Ctx::WP::NCH; h++) psi[h][0] = c.psi0(h);
+      GrpWalk<G, T, TC, 1>::node(c, psi);
+    }
   }
 }
 
