@@ -224,8 +224,8 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
       if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&px.sa, cudaStreamNonBlocking, lo);
       if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&px.sb, cudaStreamNonBlocking, lo);
       if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&px.s2, cudaStreamNonBlocking, hi);
-      cudaEvent_t* evs[5] = {&px.fork, &px.k1[0], &px.k1[1], &px.k2[0], &px.k2[1]};
-      for (int i = 0; i < 5 && e == cudaSuccess; i++) e = cudaEventCreateWithFlags(evs[i], cudaEventDisableTiming);
+      cudaEvent_t* evs[7] = {&px.fork, &px.k1[0], &px.k1[1], &px.k2[0], &px.k2[1], &px.k2[2], &px.k2[3]};
+      for (int i = 0; i < 7 && e == cudaSuccess; i++) e = cudaEventCreateWithFlags(evs[i], cudaEventDisableTiming);
       if (e != cudaSuccess) {
         int rc = cuda_fail(nullptr, e, "me_create: pipeline streams");
         cudaFree(h->d_scratch); cudaFree(h->d_frac);
@@ -245,7 +245,8 @@ int me_destroy(me_handle* h) {
   if (h->have_pipe) {
     cudaStreamDestroy(h->pipe.sa); cudaStreamDestroy(h->pipe.sb); cudaStreamDestroy(h->pipe.s2);
     cudaEventDestroy(h->pipe.fork);
-    for (int i = 0; i < 2; i++) { cudaEventDestroy(h->pipe.k1[i]); cudaEventDestroy(h->pipe.k2[i]); }
+    for (int i = 0; i < 2; i++) cudaEventDestroy(h->pipe.k1[i]);
+    for (int i = 0; i < 4; i++) cudaEventDestroy(h->pipe.k2[i]);
   }
   if (h->d_scratch) cudaFree(h->d_scratch);
   if (h->d_cum) cudaFree(h->d_cum);

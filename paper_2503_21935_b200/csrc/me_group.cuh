@@ -329,8 +329,12 @@ template <class G> struct XGeom {
 // Arguments of the three kernels of one chunk of events (pointers already offset to the chunk)
 struct PipeArgs {
   LaunchArgs a;
+#ifdef ME_DEBUG_TIMES
+  unsigned long long* dbg;   // [4]: first start / last end of the amplitude kernel, of the colour kernel (globaltimer ns)
+#endif
   void* ev;                  // GrpEvent<T, N>[nevt]
   void* xt;                  // TC[nevt][ncombo][ncol][8] (+ one group of slack)
+  const void* cfrag;         // 120 flows: C' in MMA fragment order (global memory), else unused
   int ncombo;                // gluon-helicity combinations with at least one good helicity row
   unsigned char combo[32];   // ... in increasing order
   unsigned char vmask[32];   // per listed combination: bit v = 2 h_t + h_tbar set iff that helicity row is good
@@ -670,6 +674,10 @@ __global__ void __launch_bounds__(32, MINB) amp_kernel(const PipeArgs p) {
   EV& ev = *reinterpret_cast<EV*>(smem_raw);
   T* gbase = reinterpret_cast<T*>(smem_raw + GE::EVB);
   const int lane = threadIdx.x;
+#ifdef ME_DEBUG_TIMES
+  struct Stamp { unsigned long long* d; __device__ Stamp(unsigned long long* q) : d(q) { if (d && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); atomicMin(d, t); } }
+                 __device__ ~Stamp() { if (d && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); atomicMax(d + 1, t); } } } stamp(p.dbg);
+#endif
   const int gi = lane / LPG, r = lane - gi * LPG;
   const int nunit = (p.ncombo + GPW - 1) / GPW;
   T* slots = gbase + (size_t)((gi < GPW) ? gi : 0) * GE::GS;
@@ -777,7 +785,14 @@ __device__ __forceinline__ unsigned to_tf32(float x) {
 // ------------------------------------------------------------------------------------------------------------------
 template <int NCOL, typename TC> struct ColFrag;
 
-// fp64: mma.sync m8n8k4 f64, one combination per tile
+// C' entry: from shared memory, or (120 flows) from the fragment-ordered copy in global memory past L1 (the
+// amplitude warps running beside the colour warps keep their table words there)
+template <bool GLOBAL, typename V> __device__ __forceinline__ V cf_ld(const V* q) {
+  if constexpr (GLOBAL) return __ldcg(q);
+  else return *q;
+}
+
+// fp64: mma.sync m8n8k4 f64, one combination per tile; MMA row m = row of X[flow][8]
 template <int NCOL> struct ColFrag<NCOL, double> {
   static constexpr int GPT = 1, NW = NCOL / 4, NT = NCOL / 8, JB = (NT < 5) ? NT : 5;
   static_assert(NT % JB == 0, "tile blocking");
@@ -788,7 +803,8 @@ template <int NCOL> struct ColFrag<NCOL, double> {
     for (int i = 0; i < NW; i++) a[i] = __ldcg(p + 32 * i);
   }
   // cf: [pair(I,J)][k-step s][lane]: B[k = lane % 4][n = lane / 4] = C'[8 I + 4 s + k][8 J + perm(n)]
-  __device__ __forceinline__ void quad(const double* cf, int lane, double& qa, double& qb) const {
+  // returns the thread's part of q_m (m = lane / 4); the quad sum and the re + im sum are the caller's
+  template <bool CFG> __device__ __forceinline__ double quad(const double* cf, int lane) const {
     double q = 0.0;
 #pragma unroll
     for (int J0 = 0; J0 < NT; J0 += JB) {
@@ -803,7 +819,7 @@ template <int NCOL> struct ColFrag<NCOL, double> {
 #pragma unroll
           for (int j = 0; j < JB; j++) {
             const int J = J0 + j;
-            if (J >= I) dmma884(d[j][0], d[j][1], a[2 * I + s], cf[((J * (J + 1) / 2 + I) * 2 + s) * 32 + lane]);
+            if (J >= I) dmma884(d[j][0], d[j][1], a[2 * I + s], cf_ld<CFG>(cf + ((J * (J + 1) / 2 + I) * 2 + s) * 32 + lane));
           }
 #pragma unroll
       for (int j = 0; j < JB; j++) {
@@ -811,35 +827,37 @@ template <int NCOL> struct ColFrag<NCOL, double> {
         q = ::fma(d[j][1], a[2 * (J0 + j) + 1], q);
       }
     }
-    qa = q; qb = 0.0;
+    return q;
   }
-  // w[idx] += |x|^2 of the flows 4 idx + c for the rows whose helicity is good (summed over rows by the caller)
-  __device__ __forceinline__ void weights(double (&w)[NW], bool keepa, bool) const {
+  // w[idx] += |x|^2 of the flows 4 idx + c if the thread's row belongs to a good helicity (rows are added by the caller)
+  __device__ __forceinline__ void weights(double (&w)[NW], bool keep) const {
 #pragma unroll
-    for (int i = 0; i < NW; i++) w[i] = keepa ? ::fma(a[i], a[i], w[i]) : w[i];
+    for (int i = 0; i < NW; i++) w[i] = keep ? ::fma(a[i], a[i], w[i]) : w[i];
   }
 };
 
-// fp32 / mixed: mma.sync m16n8k8 tf32, two combinations per tile (rows 0-7 and 8-15); X split as hi + lo with
-// hi = tf32(x), lo = tf32(x - hi): the integer colour numerators are exact in TF32, so every product carries fp32
-// accuracy and the sum accumulates in fp32
+// fp32 / mixed: mma.sync m16n8k8 tf32, two combinations per tile.  Thread (g = lane / 4, c = lane % 4) owns the
+// re and im rows of variant v = g % 4 of combination g / 4: MMA rows g and g + 8, one 8-byte load per flow.  X is
+// split as hi + lo with hi = tf32(x), lo = tf32(x - hi): the integer colour numerators are exact in TF32, so every
+// product carries fp32 accuracy and the sum accumulates in fp32
 template <int NCOL> struct ColFrag<NCOL, float> {
   static constexpr int GPT = 2, NW = NCOL / 4, NT = NCOL / 8, JB = (NT < 5) ? NT : 5;
   static_assert(NT % JB == 0, "tile blocking");
-  float x[NT][4];  // [k-block][a0: group A flow 8 I + c, a1: group B same flow, a2: A flow 8 I + c + 4, a3: B ...]
+  float x[NT][4];  // [k-block][a0: re row, flow 8 I + c; a1: im row, same flow; a2: re row, flow 8 I + c + 4; a3: im row]
   __device__ __forceinline__ void load(const float* X, int lane) {
-    const float* p = X + (lane & 3) * 8 + (lane >> 2);
+    const int g = lane >> 2;
+    const float* p = X + (g >> 2) * (NCOL * 8) + (lane & 3) * 8 + 2 * (g & 3);
 #pragma unroll
     for (int I = 0; I < NT; I++) {
-      x[I][0] = __ldcg(p + 64 * I);
-      x[I][1] = __ldcg(p + NCOL * 8 + 64 * I);
-      x[I][2] = __ldcg(p + 64 * I + 32);
-      x[I][3] = __ldcg(p + NCOL * 8 + 64 * I + 32);
+      const float2 u = __ldcg(reinterpret_cast<const float2*>(p + 64 * I));
+      const float2 w = __ldcg(reinterpret_cast<const float2*>(p + 64 * I + 32));
+      x[I][0] = u.x; x[I][1] = u.y; x[I][2] = w.x; x[I][3] = w.y;
     }
   }
   // cf: [pair(I,J)][lane][2]: b0 = C'[8 I + lane % 4][8 J + perm(lane / 4)], b1 = C'[8 I + lane % 4 + 4][...]
-  __device__ __forceinline__ void quad(const float* cf, int lane, float& qa, float& qb) const {
-    qa = qb = 0.f;
+  // returns the thread's part of q_re + q_im of its variant
+  template <bool CFG> __device__ __forceinline__ float quad(const float* cf, int lane) const {
+    float q = 0.f;
 #pragma unroll
     for (int J0 = 0; J0 < NT; J0 += JB) {
       float d[JB][4];
@@ -857,7 +875,7 @@ template <int NCOL> struct ColFrag<NCOL, float> {
         for (int j = 0; j < JB; j++) {
           const int J = J0 + j;
           if (J >= I) {
-            const float2 b = *reinterpret_cast<const float2*>(cf + ((J * (J + 1) / 2 + I) * 32 + lane) * 2);
+            const float2 b = cf_ld<CFG>(reinterpret_cast<const float2*>(cf + ((J * (J + 1) / 2 + I) * 32 + lane) * 2));
             hmma1688(d[j], al, __float_as_uint(b.x), __float_as_uint(b.y));
             hmma1688(d[j], ah, __float_as_uint(b.x), __float_as_uint(b.y));
           }
@@ -865,63 +883,89 @@ template <int NCOL> struct ColFrag<NCOL, float> {
       }
 #pragma unroll
       for (int j = 0; j < JB; j++) {
-        qa = fmaf(d[j][0], x[J0 + j][0], qa); qa = fmaf(d[j][1], x[J0 + j][2], qa);
-        qb = fmaf(d[j][2], x[J0 + j][1], qb); qb = fmaf(d[j][3], x[J0 + j][3], qb);
+        q = fmaf(d[j][0], x[J0 + j][0], q); q = fmaf(d[j][1], x[J0 + j][2], q);
+        q = fmaf(d[j][2], x[J0 + j][1], q); q = fmaf(d[j][3], x[J0 + j][3], q);
       }
     }
+    return q;
   }
-  __device__ __forceinline__ void weights(float (&w)[NW], bool keepa, bool keepb) const {
+  __device__ __forceinline__ void weights(float (&w)[NW], bool keep) const {
 #pragma unroll
     for (int I = 0; I < NT; I++) {
-      w[2 * I] = keepa ? fmaf(x[I][0], x[I][0], w[2 * I]) : w[2 * I];
-      w[2 * I] = keepb ? fmaf(x[I][1], x[I][1], w[2 * I]) : w[2 * I];
-      w[2 * I + 1] = keepa ? fmaf(x[I][2], x[I][2], w[2 * I + 1]) : w[2 * I + 1];
-      w[2 * I + 1] = keepb ? fmaf(x[I][3], x[I][3], w[2 * I + 1]) : w[2 * I + 1];
+      w[2 * I] = keep ? fmaf(x[I][1], x[I][1], fmaf(x[I][0], x[I][0], w[2 * I])) : w[2 * I];
+      w[2 * I + 1] = keep ? fmaf(x[I][3], x[I][3], fmaf(x[I][2], x[I][2], w[2 * I + 1])) : w[2 * I + 1];
     }
   }
 };
 
 template <class G, typename TC> struct ColGeom {
-  static constexpr int WARPS = 8, GPT = ColFrag<G::ncol, TC>::GPT, NCOL = G::ncol;
+  // 24 flows: C' is 1.5-3 KB, so a block is ONE warp with a few KB of shared memory and < 3 K registers: such blocks
+  // become resident beside the amplitude warps of the following chunk and run under them (high-priority stream).
+  // 120 flows: C' is 30-61 KB in shared memory, shared by the 8 warps of a block.  (A copy in global memory read by
+  // one-warp blocks was measured: 4.6 TB/s of L2 traffic in fp32, the amplitude kernel beside it 20 % slower.)
+  static constexpr int WARPS = (G::ncol <= 24) ? 1 : 8;
+  static constexpr bool CF_GLOBAL = false;
+  static constexpr int WPS = (G::ncol <= 24) ? 32 : 8;   // colour warps per SM (grid sizing; 4, 8, 16, 32 measured)
+  static constexpr int GPT = ColFrag<G::ncol, TC>::GPT, NCOL = G::ncol;
   static constexpr int CF = XGeom<G>::NPAIR * 64;                        // TC elements of C' in fragment order
   static constexpr int PERW = (int)sizeof(double) * ((1 << (G::n + 2)) + NCOL);   // per warp: |M_h|^2, colour weights
-  static constexpr int SMEM = CF * (int)sizeof(TC) + WARPS * PERW;
+  static constexpr int SMEM = (CF_GLOBAL ? 0 : CF * (int)sizeof(TC)) + WARPS * PERW;
 };
 
-// One warp per event (persistent warps, grid-stride over the events of the chunk).
-// CM::at16(i): entry i of the row-major integer colour numerators (global memory).
+// C' (diagonal tiles halved, tile columns permuted) in MMA fragment order; CM::at16(i): entry i of the row-major
+// integer colour numerators (global memory)
+template <class G, typename TC, class CM>
+__device__ __forceinline__ TC cfrag_entry(int i) {
+  constexpr int GPT = ColFrag<G::ncol, TC>::GPT, NCOL = G::ncol;
+  const int pair = i >> 6;
+  int ca, n;
+  if (GPT == 1) { const int l = i & 31, s = (i >> 5) & 1; ca = 4 * s + (l & 3); n = l >> 2; }
+  else { const int l = (i >> 1) & 31; ca = (l & 3) + 4 * (i & 1); n = l >> 2; }
+  int J = 0;
+  while ((J + 1) * (J + 2) / 2 <= pair) J++;
+  const int I = pair - J * (J + 1) / 2;
+  const int cb = (n >> 1) + 4 * (n & 1);
+  const TC cv = TC(CM::at16((8 * I + ca) * NCOL + 8 * J + cb));
+  return (I == J) ? TC(0.5) * cv : cv;
+}
+template <class G, typename TC, class CM>
+__global__ void cfrag_kernel(TC* out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < ColGeom<G, TC>::CF) out[i] = cfrag_entry<G, TC, CM>(i);
+}
+
+// K2: one warp per event (the warps stride over the events of the chunk).
 template <class G, typename TC, class CM, int MODE>
-__global__ void __launch_bounds__(ColGeom<G, TC>::WARPS * 32, 1) colour_kernel(const PipeArgs p) {
+__global__ void __launch_bounds__(ColGeom<G, TC>::WARPS * 32) colour_kernel(const PipeArgs p) {
   typedef ColGeom<G, TC> CG;
   typedef ColFrag<G::ncol, TC> Frag;
   constexpr int N = G::n, NPAR = N + 2, NCOMB = 1 << NPAR, NCOL = G::ncol, GPT = CG::GPT, NW = Frag::NW;
+  constexpr bool CFG = CG::CF_GLOBAL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  TC* cf = reinterpret_cast<TC*>(smem_raw);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  double* mh = reinterpret_cast<double*>(smem_raw + CG::CF * sizeof(TC) + (size_t)warp * CG::PERW);  // [NCOMB]
-  double* wcs = mh + NCOMB;                                                                           // [NCOL]
+#ifdef ME_DEBUG_TIMES
+  struct Stamp { unsigned long long* d; __device__ Stamp(unsigned long long* q) : d(q) { if (d && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); atomicMin(d, t); } }
+                 __device__ ~Stamp() { if (d && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); atomicMax(d + 1, t); } } } stamp(p.dbg ? p.dbg + 2 : nullptr);
+#endif
+  constexpr size_t CFB = CFG ? 0 : CG::CF * sizeof(TC);
+  double* mh = reinterpret_cast<double*>(smem_raw + CFB + (size_t)warp * CG::PERW);  // [NCOMB]
+  double* wcs = mh + NCOMB;                                                          // [NCOL]
   const LaunchArgs& a = p.a;
-  // ---- C' (diagonal tiles halved, tile columns permuted) in MMA fragment order, once per block
-  for (int i = tid; i < CG::CF; i += CG::WARPS * 32) {
-    const int pair = i >> 6;
-    int ca, n;
-    if (GPT == 1) { const int l = i & 31, s = (i >> 5) & 1; ca = 4 * s + (l & 3); n = l >> 2; }
-    else { const int l = (i >> 1) & 31; ca = (l & 3) + 4 * (i & 1); n = l >> 2; }
-    int J = 0;
-    while ((J + 1) * (J + 2) / 2 <= pair) J++;
-    const int I = pair - J * (J + 1) / 2;
-    const int cb = (n >> 1) + 4 * (n & 1);
-    const TC cv = TC(CM::at16((8 * I + ca) * NCOL + 8 * J + cb));
-    cf[i] = (I == J) ? TC(0.5) * cv : cv;
+  const TC* cf;
+  if constexpr (CFG) {
+    cf = reinterpret_cast<const TC*>(p.cfrag);
+  } else {
+    TC* cfs = reinterpret_cast<TC*>(smem_raw);
+    for (int i = tid; i < CG::CF; i += CG::WARPS * 32) cfs[i] = cfrag_entry<G, TC, CM>(i);
+    __syncthreads();
+    cf = cfs;
   }
-  __syncthreads();
   const long long wstride = (long long)gridDim.x * CG::WARPS;
   const long long w0 = (long long)blockIdx.x * CG::WARPS + warp;
   const int ntile = (p.ncombo + GPT - 1) / GPT;
   const TC* xbase = reinterpret_cast<const TC*>(p.xt);
   auto tile_ptr = [&](long long e, int ti) { return xbase + ((size_t)e * p.ncombo + (size_t)ti * GPT) * XGeom<G>::GRP; };
   auto is_good = [&](int h) { return MODE == MODE_FILTER || ((a.good.mask[h >> 6] >> (h & 63)) & 1ull) != 0ull; };
-  const int row = lane >> 2, var = lane >> 3;
   Frag cur, nxt;
   if (w0 < a.nevt) cur.load(tile_ptr(w0, 0), lane);
   for (long long e = w0; e < a.nevt; e += wstride) {
@@ -937,21 +981,21 @@ __global__ void __launch_bounds__(ColGeom<G, TC>::WARPS * 32, 1) colour_kernel(c
       const long long en = more_here ? e : e + wstride;
       if (en < a.nevt) nxt.load(tile_ptr(en, more_here ? ti + 1 : 0), lane);
       // ---- a6 on the tensor cores
-      TC qa, qb;
-      cur.quad(cf, lane, qa, qb);
-      qa += __shfl_xor_sync(0xffffffffu, qa, 1); qb += __shfl_xor_sync(0xffffffffu, qb, 1);
-      qa += __shfl_xor_sync(0xffffffffu, qa, 2); qb += __shfl_xor_sync(0xffffffffu, qb, 2);   // row m complete
-      qa += __shfl_xor_sync(0xffffffffu, qa, 4); qb += __shfl_xor_sync(0xffffffffu, qb, 4);   // re + im rows
-      const int ca = ti * GPT, cb = ti * GPT + 1;
-      if ((lane & 7) == 0) {
-        mh[grp_hel_of<N>(p.combo[ca], var)] = (double)(TC(2) * qa);
-        if (GPT == 2 && cb < p.ncombo) mh[grp_hel_of<N>(p.combo[cb], var)] = (double)(TC(2) * qb);
+      TC q = cur.template quad<CFG>(cf, lane);
+      q += __shfl_xor_sync(0xffffffffu, q, 1);
+      q += __shfl_xor_sync(0xffffffffu, q, 2);   // MMA row(s) of the quad complete
+      int ci, v;                                  // listed combination and variant of this thread's row(s)
+      if constexpr (GPT == 1) {
+        q += __shfl_xor_sync(0xffffffffu, q, 4);  // re + im rows of variant v = lane / 8
+        ci = ti; v = lane >> 3;
+        if ((lane & 7) == 0) mh[grp_hel_of<N>(p.combo[ci], v)] = 2.0 * q;
+      } else {
+        ci = 2 * ti + (lane >> 4); v = (lane >> 2) & 3;   // the thread's rows are re and im of one variant
+        if ((lane & 3) == 0 && ci < p.ncombo) mh[grp_hel_of<N>(p.combo[ci], v)] = (double)(2.f * q);
       }
-      if (MODE == MODE_SELECT) {
-        // a8 colour weights: |J_c|^2 of the good (h_t, h_tbar) rows, per thread for its row; rows are added below
-        const bool ka = (p.vmask[ca] >> (row >> 1)) & 1;
-        const bool kb = (GPT == 2 && cb < p.ncombo) ? ((p.vmask[cb] >> (row >> 1)) & 1) : false;
-        cur.weights(wacc, ka, kb);
+      if (MODE == MODE_SELECT && a.selcol) {
+        // a8 colour weights: |J_c|^2 of the good (h_t, h_tbar) rows, per thread for its row(s); rows are added below
+        cur.weights(wacc, ci < p.ncombo && ((p.vmask[ci < p.ncombo ? ci : 0] >> v) & 1));
       }
       cur = nxt;
     }

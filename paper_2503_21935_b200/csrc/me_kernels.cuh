@@ -44,7 +44,7 @@ struct LaunchArgs {
 // every colour kernel runs on the high-priority stream s2 beside the amplitude kernel of the following chunk.
 struct PipeCtx {
   cudaStream_t sa, sb, s2;
-  cudaEvent_t fork, k1[2], k2[2];
+  cudaEvent_t fork, k1[2], k2[4];
 };
 
 struct LaunchInfo {

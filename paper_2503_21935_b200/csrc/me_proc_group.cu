@@ -16,6 +16,11 @@
 #ifndef ME_MINB
 #define ME_MINB 1
 #endif
+#ifndef ME_NPART
+#define ME_NPART 2   // parts of the scratch (me::PipeCtx holds 4 events for them); 2, 3 and 4 measured: 2 is best
+#endif
+#include <cstdio>
+#include <cstdlib>
 
 #if ME_PREC == 0
 typedef double T_amp;
@@ -35,6 +40,10 @@ __device__ const short c_cmat16[Grp::ncol * Grp::ncol] = ME_CAT(ME_CMAT_, ME_PRO
 struct CMat {
   __device__ __forceinline__ static int at16(int i) { return (int)__ldg(c_cmat16 + i); }
 };
+
+// 120 flows: C' in MMA fragment order, written by cfrag_kernel at the start of every call (a few microseconds; no
+// state to keep: concurrent calls write the same values)
+__device__ T_col g_cfrag[me::ColGeom<Grp, T_col>::CF_GLOBAL ? me::ColGeom<Grp, T_col>::CF : 1];
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -61,15 +70,16 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
   const size_t evb = sizeof(EV), grpb = (size_t)me::XGeom<Grp>::GRP * sizeof(TCo);
   const size_t per_event = evb + (size_t)p.ncombo * grpb, slack = 2 * grpb + 1024;
   const int nunit = (p.ncombo + GE::GPW - 1) / GE::GPW;
-  // Chunks: the scratch is used as two halves; with at least two chunks, consecutive chunks run on alternating
-  // internal streams and the colour kernel of chunk c overlaps the amplitude kernel of chunk c + 1.
-  const size_t half = (a.scratch_bytes / 2) & ~(size_t)255;
+  // Chunks: the scratch is used as NPART parts in turn; with at least two chunks, consecutive chunks run on
+  // alternating internal streams and the colour kernel of chunk c overlaps the amplitude kernels of later chunks.
+  const int NPART = ME_NPART;
+  const size_t half = (a.scratch_bytes / NPART) & ~(size_t)255;
   long long cap = (half > slack) ? (long long)((half - slack) / per_event) : 0;   // events per half
   if (cap > (1 << 20)) cap = 1 << 20;
   const long long min_chunk = (8 * 1184 + nunit - 1) / nunit;   // >= 8 waves of amplitude warps on 148 SMs
   long long chunk = cap;
   if (chunk > 0 && a.nevt > 0) {
-    long long want = (a.nevt + 3) / 4;                            // aim at four chunks per call
+    long long want = (a.nevt + 2 * NPART - 1) / (2 * NPART);      // aim at two rounds of the parts per call
     if (want < min_chunk) want = min_chunk;
     if (want < chunk) chunk = want;
   }
@@ -89,7 +99,7 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     info->cum_slots = 0;
     info->scratch_per_event = (long long)(sizeof(EV) + (size_t)GE::NGRP * grpb);
     info->chunk = chunk;
-    info->launches = (int)(3 * nchunks);
+    info->launches = (int)(3 * nchunks) + (CG::CF_GLOBAL ? 1 : 0);
   }
   if (dry || a.nevt == 0) return 0;
   if (p.ncombo == 0 || chunk < 1 || !a.scratch) return (int)cudaErrorInvalidValue;
@@ -103,6 +113,14 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
   if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&k2_per_sm, k2, CG::WARPS * 32, CG::SMEM);
   if (err != cudaSuccess) return (int)err;
   if (k2_per_sm < 1) k2_per_sm = 1;
+  if (CG::CF_GLOBAL) {
+    void* sym = nullptr;
+    static_assert(sizeof(TCo) == sizeof(T_col), "the filter (fp64) is compiled in the fp64 unit only");
+    err = cudaGetSymbolAddress(&sym, g_cfrag);
+    if (err != cudaSuccess) return (int)err;
+    me::cfrag_kernel<Grp, TCo, CMat><<<(CG::CF + 255) / 256, 256, 0, st>>>((TCo*)sym);
+    p.cfrag = sym;
+  }
   const me::PipeCtx* px = (nchunks > 1) ? a.pipe : nullptr;
   if (px) {  // fork: the internal streams start after everything already enqueued on the caller's stream
     err = cudaEventRecord(px->fork, st);
@@ -111,11 +129,21 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     if (err == cudaSuccess) err = cudaStreamWaitEvent(px->s2, px->fork, 0);
     if (err != cudaSuccess) return (int)err;
   }
+#ifdef ME_DEBUG_TIMES
+  static unsigned long long* dbg = nullptr;
+  const bool times = MODE != me::MODE_FILTER && getenv("ME_B200_TIMES") && nchunks <= 64;
+  if (times) {
+    if (!dbg) cudaMalloc(&dbg, 64 * 4 * sizeof(unsigned long long));
+    unsigned long long init[64 * 4];
+    for (int i = 0; i < 64 * 4; i++) init[i] = (i & 1) ? 0ull : ~0ull;
+    cudaMemcpy(dbg, init, sizeof(init), cudaMemcpyHostToDevice);
+  }
+#endif
   long long c = 0;
   for (long long e0 = 0; e0 < a.nevt; e0 += chunk, c++) {
     const long long n = (a.nevt - e0 < chunk) ? (a.nevt - e0) : chunk;
-    const int hf = (int)(c & 1);
-    char* base = (char*)a.scratch + (px ? (size_t)hf * half : 0);
+    const int hf = (int)(c & 1), part = (int)(c % NPART);
+    char* base = (char*)a.scratch + (px ? (size_t)part * half : 0);
     p.a = a;
     p.a.nevt = n;
     p.a.mom = a.mom + e0 * (Grp::npar * 4);
@@ -125,26 +153,43 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     p.a.me = a.me ? a.me + e0 : nullptr;
     p.a.selhel = a.selhel ? a.selhel + e0 : nullptr;
     p.a.selcol = a.selcol ? a.selcol + e0 : nullptr;
+#ifdef ME_DEBUG_TIMES
+    p.dbg = times ? dbg + 4 * c : nullptr;
+#endif
     p.ev = base;
     p.xt = base + align_up((size_t)n * evb, 256);
     constexpr int PT = ((1 << N) + N + 6 <= 32) ? 32 : 64;
     cudaStream_t s1 = px ? (hf ? px->sb : px->sa) : st, s2 = px ? px->s2 : st;
-    if (px && c >= 2 && (err = cudaStreamWaitEvent(s1, px->k2[hf], 0)) != cudaSuccess) return (int)err;  // half free again
+    if (px && c >= NPART && (err = cudaStreamWaitEvent(s1, px->k2[part], 0)) != cudaSuccess) return (int)err;  // part free again
     k0<<<(unsigned)((n * PT + 127) / 128), 128, 0, s1>>>(p.a, (EV*)p.ev);
     k1<<<(unsigned)(n * nunit), 32, GE::SMEM, s1>>>(p);
     if (px) {
       if ((err = cudaEventRecord(px->k1[hf], s1)) != cudaSuccess) return (int)err;
       if ((err = cudaStreamWaitEvent(s2, px->k1[hf], 0)) != cudaSuccess) return (int)err;
     }
+    // colour kernel: WPS warps per SM (or one warp per event if that is fewer); the warps stride over the events
     long long b2 = (n + CG::WARPS - 1) / CG::WARPS;
-    if (b2 > (long long)sms * k2_per_sm) b2 = (long long)sms * k2_per_sm;
+    long long cap2 = (long long)sms * ((CG::WPS + CG::WARPS - 1) / CG::WARPS);
+    if (cap2 > (long long)sms * k2_per_sm) cap2 = (long long)sms * k2_per_sm;
+    if (b2 > cap2) b2 = cap2;
     k2<<<(unsigned)b2, CG::WARPS * 32, CG::SMEM, s2>>>(p);
-    if (px && (err = cudaEventRecord(px->k2[hf], s2)) != cudaSuccess) return (int)err;
+    if (px && (err = cudaEventRecord(px->k2[part], s2)) != cudaSuccess) return (int)err;
     err = cudaGetLastError();
     if (err != cudaSuccess) return (int)err;
   }
+#ifdef ME_DEBUG_TIMES
+  if (times) {
+    cudaDeviceSynchronize();
+    unsigned long long t[64 * 4];
+    cudaMemcpy(t, dbg, sizeof(t), cudaMemcpyDeviceToHost);
+    const unsigned long long t0 = t[0];
+    for (long long i = 0; i < nchunks; i++)
+      fprintf(stderr, "chunk %2lld  K1 %9.1f .. %9.1f us   K2 %9.1f .. %9.1f us\n", i, (t[4 * i] - t0) * 1e-3, (t[4 * i + 1] - t0) * 1e-3,
+              (t[4 * i + 2] - t0) * 1e-3, (t[4 * i + 3] - t0) * 1e-3);
+  }
+#endif
   if (px) {  // join: the caller's stream continues after the last colour kernel (s2 is in order, and follows sa / sb)
-    err = cudaStreamWaitEvent(st, px->k2[(int)((c - 1) & 1)], 0);
+    err = cudaStreamWaitEvent(st, px->k2[(int)((c - 1) % NPART)], 0);
     if (err != cudaSuccess) return (int)err;
   }
   return 0;
