@@ -2,20 +2,24 @@
 """bench.py -- MEs/s of the gg -> t tbar g g hot path on B200 (BASELINE.json metric), one JSON line.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--nevt E] [--precision fp64|fp32|mixed]
-                    [--process gg_ttgg] [--sweep] [--no-extras] [--impl reference]
+                    [--process gg_ttgg] [--no-sweep] [--no-extras] [--impl reference]
 
 A "step" is one pass of the whole hot path (me_compute: load, wavefunctions, diagrams, jamps, colour
 sum, helicity loop, helicity/colour selection, store) over one batch of seeded RAMBO events.
 `value` times the C-ABI call with inputs resident in HBM (CUDA events on the launch stream);
-`e2e` times me_compute_host with pinned HOST buffers (H2D + kernel + D2H inside the timed region).
-Multi-GPU (torchrun): events are independent, ranks run replicas on disjoint seeded batches, no
-collective on the data path ("scaling": "weak").  --impl reference times the CPU oracle.
+`e2e` times me_compute_host with pinned HOST buffers (H2D + kernels + D2H inside the timed region).
+The GPU arm makes its inputs on the device with me_generate (the product's own seeded RAMBO); only the
+cpu_baseline leg and --impl reference touch oracle/.
+Multi-GPU: events are independent, ranks run replicas on disjoint seeded ranges, no collective on the
+data path ("scaling": "weak").  `--gpus N` without a launcher re-executes itself under torchrun.
+--impl reference times the CPU oracle.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import re
 import subprocess
 import sys
 import threading
@@ -26,13 +30,8 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2503_21935_b200 import inputs as I  # noqa: E402
 from paper_2503_21935_b200.shard import max_over_ranks, rank_range  # noqa: E402
 
-# DRAM traffic per event of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full
-# capture, profiles/r1_ttgg_fp64_group_v2_ncu_full.txt: 14.24 MB for 65536 events); algorithmic bytes are
-# 6*4*8 + 8 + 16 + 16 = 232 B per event
-TRAFFIC_BYTES_PER_EVENT = {"gg_ttgg": 14.24256e6 / 65536}
 # SURVEY.md 8(d) accounting ("each distinct current once per helicity"): FLOPs of the one-event-per-thread code
 PER_HELICITY_ACCOUNTING = {"gg_ttgg": 30331 * 64 + 672}
 
@@ -40,35 +39,54 @@ METRIC = "matrix elements/sec (MEs/s) for gg->ttbar gg fp64 & fp32 on 1 B200; % 
 UNIT = "MEs/s"
 ALPHAS = {"ee_mumu": 0.118, "gg_tt": 0.118, "gg_ttg": 0.118, "gg_ttgg": None, "gg_ttggg": 0.118}
 DTYPE = {"fp64": "f64", "fp32": "f32", "mixed": "f64+f32"}
+GROUP = ("gg_ttgg", "gg_ttggg")   # lane-group pipeline: colour contraction on the tensor cores
 
 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--nevt", type=int, default=1 << 20, help="events per step (per GPU)")
     ap.add_argument("--process", default="gg_ttgg")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--no-sweep", action="store_true", help="skip the events-per-launch sweep 2^14..2^22")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the events-per-launch sweep 2^8..2^22")
     ap.add_argument("--no-extras", action="store_true", help="skip fp32/mixed lines, cpu_baseline and e2e")
     return ap.parse_args()
 
 
 def flops_per_me(process, ngood):
-    """Algorithmic FLOPs per ME of the generated code (FMA = 2), counted by the generator (gen/flops.json)."""
+    """Algorithmic FLOPs per ME of the generated code (FMA = 2), counted by the generator (gen/flops.json):
+    (all, the part that runs on the FMA pipes when the colour contraction is on the tensor cores, detail)."""
     path = os.path.join(ROOT, "paper_2503_21935_b200", "csrc", "gen", "flops.json")
     with open(path) as f:
         d = json.load(f)[process]
-    return d["per_event"] + ngood * d["per_helicity"], d
+    allf = d["per_event"] + ngood * d["per_helicity"]
+    return allf, d["per_event"] + ngood * d["amplitudes_per_helicity"], d
 
 
-def make_inputs(process, nevt, seed, start=0):
-    mom = I.make_momenta(process, nevt, seed=seed, start=start)
-    gs = I.make_gs(nevt, seed=seed, alphas=ALPHAS[process], start=start)
-    rh, rc = I.make_rnd(nevt, seed=seed, start=start)
-    return mom, gs, rh, rc
+def profile_traffic(process, precision):
+    """DRAM bytes per event of the dominant (amplitude) kernel from the committed ncu summary of this build, or None:
+    (dram__bytes_read.sum + dram__bytes_write.sum) / events of the captured launch."""
+    path = os.path.join(ROOT, "profiles", f"r2_{process}_{precision}_pipeline_ncu_full.txt")
+    if not os.path.exists(path):
+        return None, None
+    txt = open(path).read()
+    m = re.search(r"# events per captured amplitude launch: (\d+)", txt)
+    blocks = txt.split("\nKernel Name")
+    for b in blocks:
+        if "amp_kernel" not in b.split("\n")[0]:
+            continue
+        tot = 0.0
+        for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            mm = re.search(re.escape(key) + r" \[(\w+)\] = ([0-9.eE+-]+)", b)
+            if not mm:
+                return None, None
+            tot += float(mm.group(2)) * {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}[mm.group(1)]
+        if m:
+            return tot / int(m.group(1)), os.path.relpath(path, ROOT)
+    return None, None
 
 
 class ClockSampler:
@@ -120,34 +138,44 @@ def time_device(torch, m, bufs, steps, warmup, select=True):
     """ms per step of me_compute with device-resident inputs: CUDA events on the launch stream."""
     mom, gs, rh, rc, out, sh, sc = bufs
     stream = torch.cuda.current_stream()
+    kw = dict(out=out, selhel=sh if select else None, selcol=sc if select else None, stream=stream)
     for _ in range(warmup):
-        m.compute(mom, gs, rh if select else None, rc if select else None, out=out, selhel=sh if select else None,
-                  selcol=sc if select else None, stream=stream)
+        m.compute(mom, gs, rh if select else None, rc if select else None, **kw)
     torch.cuda.synchronize()
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
     ev[0].record(stream)
     for k in range(steps):
-        m.compute(mom, gs, rh if select else None, rc if select else None, out=out, selhel=sh if select else None,
-                  selcol=sc if select else None, stream=stream)
+        m.compute(mom, gs, rh if select else None, rc if select else None, **kw)
         ev[k + 1].record(stream)
     torch.cuda.synchronize()
     per = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
     return ev[0].elapsed_time(ev[steps]), per
 
 
+def oracle_inputs(process, nevt, seed=1, start=0):
+    from oracle import rambo as R
+    return (R.make_momenta(process, nevt, seed=seed, start=start), R.make_gs(nevt, seed=seed, alphas=ALPHAS[process], start=start))
+
+
 def cpu_baseline(process, seconds_target=15.0):
-    """The oracle as it stands, on this box's host cores, on a bounded sample of the same workload."""
+    """The oracle as it stands, on this box's host cores, on a bounded sample of the same workload, and the
+    oracle's own count of FLOPs per ME ("counted mode": the same source compiled with an operation-counting scalar)."""
     from oracle import oracle as O
     n0 = {"ee_mumu": 16384, "gg_tt": 16384, "gg_ttg": 4096, "gg_ttgg": 256, "gg_ttggg": 16}[process]
-    mom, gs, _, _ = make_inputs(process, n0, seed=1)
+    mom, gs = oracle_inputs(process, n0)
     O.me(process, mom[:8], gs[:8])
     t = time.perf_counter(); O.me(process, mom, gs); dt = time.perf_counter() - t
     n = int(max(n0, min(1 << 20, n0 * seconds_target / max(dt, 1e-3))))
-    mom, gs, _, _ = make_inputs(process, n, seed=1)
+    mom, gs = oracle_inputs(process, n)
     mask = O.good_helicities(process, mom[:n0], gs[:n0])
     t = time.perf_counter(); O.me(process, mom, gs, mask=mask); dt = time.perf_counter() - t
+    cnt = O.count_ops(process, mom[0], float(gs[0]), mask=mask)
     return {"value": n / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
-            "sample": f"first {n} events of the seeded {process} batch (seed 1), good helicities only, {dt:.1f} s"}
+            "sample": f"first {n} events of the seeded {process} stream (seed 1), good helicities only, {dt:.1f} s",
+            "flops_per_me_counted": cnt["flops"],
+            "flops_note": "oracle/me_oracle.cpp compiled with its operation-counting scalar (-DORC_COUNT): additions + "
+                          "multiplications + divisions + square roots of one event over the good helicities (every diagram, "
+                          "4x4 matrices, each distinct current once per helicity, colour sum as the plain double sum)"}
 
 
 def run_reference(a):
@@ -157,7 +185,7 @@ def run_reference(a):
     from oracle import oracle as O
     process = a.process
     n0 = {"ee_mumu": 16384, "gg_tt": 16384, "gg_ttg": 16384, "gg_ttgg": 8192, "gg_ttggg": 64}[process]
-    mom, gs, _, _ = make_inputs(process, n0, seed=1)
+    mom, gs = oracle_inputs(process, n0)
     mask = O.good_helicities(process, mom[: min(n0, 256)], gs[: min(n0, 256)])
     for _ in range(a.warmup):
         O.me(process, mom[: max(8, n0 // 8)], gs[: max(8, n0 // 8)], mask=mask)
@@ -166,7 +194,7 @@ def run_reference(a):
         O.me(process, mom, gs, mask=mask)
     dt = time.perf_counter() - t
     val = a.steps * n0 / dt
-    sample = f"each step = first {n0} events of the seeded {process} batch (bounded sample of the {a.nevt}-event workload)"
+    sample = f"each step = first {n0} events of the seeded {process} stream (bounded sample of the {a.nevt}-event workload)"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
         "warmup": a.warmup, "ms_per_step": 1e3 * dt / a.steps, "higher_is_better": True, "scaling": "weak",
@@ -178,8 +206,21 @@ def run_reference(a):
         "gpu_launches": 0}))
 
 
+def respawn_under_torchrun(a):
+    """`python bench.py --gpus N` without a launcher: run the same command as N ranks on this node."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={a.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    sys.exit(subprocess.call(cmd))
+
+
 def main():
     a = parse()
+    if a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return respawn_under_torchrun(a)
     if a.impl == "reference":
         return run_reference(a)
     import torch
@@ -195,73 +236,103 @@ def main():
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     process, nevt = a.process, a.nevt
+    extras = rank == 0 and not a.no_extras
 
-    def barrier():
-        if world > 1:
+    def barrier(sync_ranks):
+        if sync_ranks and world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # seeded inputs: rank r takes events [r*nevt, (r+1)*nevt) of the stream (disjoint shards, no exchange);
-    # rank 0 generates up to 2^22 events when it also runs the events-per-launch sweep
-    sweep = rank == 0 and not a.no_extras and not a.no_sweep and process == "gg_ttgg"
-    start, stop = rank_range(nevt, rank, world)
+    # seeded inputs made on the device: rank r takes events [r*nevt, (r+1)*nevt) of the stream (disjoint shards, no
+    # exchange); rank 0 makes up to 2^22 events when it also runs the events-per-launch sweep
+    sweep = extras and not a.no_sweep and process == "gg_ttgg"
+    start, _ = rank_range(nevt, rank, world)
     nmax = max(nevt, 1 << 22) if sweep else nevt
-    mom_all, gs_all, rh_all, rc_all = make_inputs(process, nmax, seed=1, start=start)
-    mom_h, gs_h, rh_h, rc_h = mom_all[:nevt], gs_all[:nevt], rh_all[:nevt], rc_all[:nevt]
-    t = lambda x: torch.from_numpy(x).to(dev)
-    bufs = (t(mom_h), t(gs_h), t(rh_h), t(rc_h), torch.empty(nevt, dtype=torch.float64, device=dev),
-            torch.empty(nevt, dtype=torch.int32, device=dev), torch.empty(nevt, dtype=torch.int32, device=dev))
+    gen = MatrixElement(process, "fp64", device=local)
+    alphas_dev = 0.0 if ALPHAS[process] is None else ALPHAS[process]
+    mom_all, gs_all, rh_all, rc_all = gen.generate(nmax, seed=1, start=start, alphas=alphas_dev)
+    torch.cuda.synchronize()
+    gen.close()
+    out_all = torch.empty(nmax, dtype=torch.float64, device=dev)
+    sh_all = torch.empty(nmax, dtype=torch.int32, device=dev)
+    sc_all = torch.empty(nmax, dtype=torch.int32, device=dev)
+    big = (mom_all, gs_all, rh_all, rc_all, out_all, sh_all, sc_all)
+    bufs = tuple(x[:nevt] for x in big)
 
-    def bench_precision(prec, steps, warmup, n=nevt):
+    def bench_precision(prec, steps, warmup, sync_ranks):
         m = MatrixElement(process, prec, device=local)
-        b = bufs if n == nevt else tuple(x[:n].contiguous() for x in bufs)
-        mask = m.filter_helicities(b[0], b[1])
-        barrier()
+        mask = m.filter_helicities(bufs[0], bufs[1])
+        barrier(sync_ranks)
         with ClockSampler(local) as cs:
-            total_ms, per = time_device(torch, m, b, steps, warmup)
-        barrier()
+            total_ms, per = time_device(torch, m, bufs, steps, warmup)
+        barrier(sync_ranks)
         info = m.launch_info()
         return m, mask, total_ms, per, cs.summary(), info
 
-    m, mask, total_ms, per, clocks, info = bench_precision(a.precision, a.steps, a.warmup)
+    m, mask, total_ms, per, clocks, info = bench_precision(a.precision, a.steps, a.warmup, True)
     total_ms = max_over_ranks(total_ms, dist if world > 1 else None, dev)
     ms_per_step = total_ms / a.steps
     value = world * nevt / (ms_per_step * 1e-3)
     ngood = int(mask.sum())
-    fl, fl_detail = flops_per_me(process, ngood)
+    fl_all, fl_fma, fl_detail = flops_per_me(process, ngood)
+    on_tensor = process in GROUP and a.precision != "fp64"   # colour contraction off the FMA pipes
+    bytes_per_event = m.npar * 32 + 8 + 16 + 16
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": DTYPE[a.precision], "data": "synthetic",
         "config": {"workload": process, "events_per_step_per_gpu": nevt, "precision": a.precision,
-                   "inputs": "seeded RAMBO sqrt(s)=1500 GeV, alpha_s~U[0.10,0.13], helicity+colour selection on",
-                   "l2": "momenta+randoms+outputs per step = %.0f MB %s the 126 MB L2" % (
-                       nevt * (m.npar * 32 + 40) / 1e6, ">" if nevt * (m.npar * 32 + 40) > 126e6 else "<"),
+                   "inputs": "seeded RAMBO sqrt(s)=1500 GeV made on the device (me_generate), alpha_s~U[0.10,0.13], "
+                             "helicity+colour selection on",
+                   "l2": "momenta+randoms+outputs per step = %.0f MB %s the 126 MB L2; the path is FMA-bound (%d B per "
+                         "event against ~%.2g FLOP), no flush applied" % (nevt * bytes_per_event / 1e6,
+                                                                           ">" if nevt * bytes_per_event > 126e6 else "<",
+                                                                           bytes_per_event, fl_all),
                    "good_helicities": ngood, "launch": info, "parallelism": f"replicas x{world}"},
-        "clocks": clocks, "gpu_launches": a.steps,
+        "clocks": clocks, "gpu_launches": a.steps * max(1, info.get("launches", 1)),
     }
     if rank == 0:
         prec_peak = "fp32" if a.precision == "fp32" else "fp64"
-        peak = fma_peak(prec_peak, local)
-        kernel_ms = float(np.mean(per))
-        achieved = fl * nevt / (kernel_ms * 1e-3) * 1e-12
+        with ClockSampler(local) as cs_peak:
+            peak = fma_peak(prec_peak, local)
+            for _ in range(3):   # a few more runs so that the sampler sees the microbenchmark under load
+                peak = max(peak, fma_peak(prec_peak, local))
+        props = torch.cuda.get_device_properties(local)
+        max_mhz = clocks.get("sm_max_mhz") or 1965.0
+        nominal = props.multi_processor_count * (64 if prec_peak == "fp64" else 128) * 2 * max_mhz * 1e-6
+        step_ms = float(np.mean(per))
+        fl = fl_fma if on_tensor else fl_all
+        achieved = fl * nevt / (step_ms * 1e-3) * 1e-12
+        tr, tr_src = profile_traffic(process, a.precision)
         line["roofline"] = {
             "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-            "traffic": (TRAFFIC_BYTES_PER_EVENT[process] * nevt if process in TRAFFIC_BYTES_PER_EVENT else None),
-            "traffic_note": "DRAM bytes per launch scaled from one ncu capture (profiles/); the path is FMA-bound, not HBM-bound",
-            "frac_per_helicity_accounting": (PER_HELICITY_ACCOUNTING[process] * nevt / (kernel_ms * 1e-3) * 1e-12 / peak
-                                             if process in PER_HELICITY_ACCOUNTING else None),
-            "flops_per_me": fl, "flops_source": "generator count of the operations this kernel executes (FMA = 2, "
-            f"DESIGN.md section 5): {fl_detail['per_helicity']} per helicity x {ngood} good helicities + {fl_detail['per_event']} per event",
-            "peak_source": f"me_fma_peak({prec_peak}): register-resident FMA chain measured on this GPU in this run",
-            "nominal_peak": 148 * (64 if prec_peak == "fp64" else 128) * 2 * 1.965e-3,
-            "kernel_ms": kernel_ms,
+            "frac_nominal": achieved / nominal, "nominal_peak": nominal,
+            "nominal_peak_source": f"{props.multi_processor_count} SMs x {64 if prec_peak == 'fp64' else 128} lanes x 2 x "
+                                   f"{max_mhz:.0f} MHz (device properties, nvidia-smi clocks.max.sm)",
+            "kernel": ("the whole step (setup + amplitude + colour kernels of every chunk); the amplitude kernel is the "
+                       "dominant one, its share of the step is in profiles/ (ncu launch list)") if process in GROUP else "event_kernel",
+            "step_ms": step_ms, "flops_per_me": fl,
+            "flops_source": "generator count of the operations the kernels execute (FMA = 2, DESIGN.md section 5): "
+                            f"{fl_detail['amplitudes_per_helicity']} (amplitudes) + {fl_detail['colour_per_helicity']} (colour sum, "
+                            f"symmetric half) per helicity x {ngood} good helicities + {fl_detail['per_event']} per event"
+                            + ("; the colour contraction of this build runs on the TF32 tensor cores, so only the "
+                               "amplitude part is credited against the FMA peak" if on_tensor else ""),
+            "frac_all_flops": fl_all * nevt / (step_ms * 1e-3) * 1e-12 / peak,
+            "tensor_flops_per_me": (fl_all - fl_fma) if on_tensor else 0,
+            "peak_source": f"me_fma_peak({prec_peak}): register-resident FMA chains measured on this GPU in this run (best of 4)",
+            "peak_clocks": cs_peak.summary(),
+            "traffic": (tr * nevt if tr is not None else None),
+            "traffic_source": tr_src,
+            "traffic_note": "DRAM bytes of the amplitude kernel per step, scaled per event from the ncu capture named in "
+                            "traffic_source; the path is FMA-bound, not HBM-bound",
+            "frac_per_helicity_accounting": (PER_HELICITY_ACCOUNTING[process] * nevt / (step_ms * 1e-3) * 1e-12 / peak
+                                             if process in PER_HELICITY_ACCOUNTING and not on_tensor else None),
         }
     m.close()
-    if rank == 0 and not a.no_extras:
+    if extras:
         # e2e: host buffers (pinned) -> me_compute_host -> host results
-        pin = lambda x: torch.from_numpy(x).pin_memory()
-        hm, hg, hr, hc = pin(mom_h), pin(gs_h), pin(rh_h), pin(rc_h)
+        pin = lambda x: x.cpu().pin_memory()
+        hm, hg, hr, hc = (pin(x) for x in bufs[:4])
         ho = torch.empty(nevt, dtype=torch.float64).pin_memory()
         hsh = torch.empty(nevt, dtype=torch.int32).pin_memory()
         hsc = torch.empty(nevt, dtype=torch.int32).pin_memory()
@@ -275,42 +346,42 @@ def main():
         dt = time.perf_counter() - t0
         m.close()
         line["e2e"] = {"value": a.steps * nevt / dt, "unit": UNIT,
-                       "h2d_bytes_per_step": int(mom_h.nbytes + gs_h.nbytes + rh_h.nbytes + rc_h.nbytes),
-                       "d2h_bytes_per_step": int(nevt * 16), "api": "me_compute_host (pinned host buffers)"}
+                       "h2d_bytes_per_step": int(sum(x.numel() * x.element_size() for x in (hm, hg, hr, hc))),
+                       "d2h_bytes_per_step": int(nevt * 16),
+                       "api": "me_compute_host (pinned host buffers; chunks double-buffered over copy-in / compute / copy-out streams)"}
+        del hm, hg, hr, hc, ho, hsh, hsc
         others = {}
         for prec in ("fp64", "fp32", "mixed"):
             if prec == a.precision:
                 continue
-            m2, mk2, tot2, per2, clk2, info2 = bench_precision(prec, max(2, a.steps // 2), a.warmup)
-            ms2 = tot2 / max(2, a.steps // 2)
+            m2, mk2, tot2, per2, clk2, info2 = bench_precision(prec, a.steps, a.warmup, False)
+            ms2 = float(np.mean(per2))
             pk = fma_peak("fp32" if prec == "fp32" else "fp64", local)
-            ach = fl * nevt / (ms2 * 1e-3) * 1e-12
+            ot = process in GROUP and prec != "fp64"
+            ach = (fl_fma if ot else fl_all) * nevt / (ms2 * 1e-3) * 1e-12
             others[prec] = {"value": nevt / (ms2 * 1e-3), "unit": UNIT, "ms_per_step": ms2, "launch": info2,
-                            "roofline_frac": ach / pk, "peak_tflops": pk, "clocks": clk2}
+                            "roofline_frac": ach / pk, "roofline_frac_all_flops": fl_all * nevt / (ms2 * 1e-3) * 1e-12 / pk,
+                            "peak_tflops": pk, "clocks": clk2}
             m2.close()
         line["other_precisions"] = others
         if sweep:
-            big = tuple(torch.from_numpy(x).to(dev) for x in (mom_all, gs_all, rh_all, rc_all)) + (
-                torch.empty(nmax, dtype=torch.float64, device=dev), torch.empty(nmax, dtype=torch.int32, device=dev),
-                torch.empty(nmax, dtype=torch.int32, device=dev))
             sw = {}
             for prec in ("fp64", "fp32", "mixed"):
                 m3 = MatrixElement(process, prec, device=local)
                 m3.set_good_helicities(mask)
-                for lg in range(14, 23):
+                for lg in range(8, 23):
                     n = 1 << lg
                     b3 = tuple(x[:n] for x in big)
-                    tot3, per3 = time_device(torch, m3, b3, 5, 3)
+                    tot3, per3 = time_device(torch, m3, b3, 10, 3)
                     sw[f"{prec}:{n}"] = n / (float(np.median(per3)) * 1e-3)
                 m3.close()
             line["sweep_mes_per_s"] = sw
-            best = max((v, k) for k, v in sw.items() if k.startswith("fp64"))
-            line["sweep_best"] = {"fp64": best[1], "fp32": max((v, k) for k, v in sw.items() if k.startswith("fp32"))[1]}
+            line["sweep_note"] = "median of 10 launches per point, events per launch 2^8 .. 2^22"
+            line["sweep_best"] = {p: max((v, k) for k, v in sw.items() if k.startswith(p))[1] for p in ("fp64", "fp32", "mixed")}
         # self-contained step: inputs made on the device by me_generate, then me_compute
         m4 = MatrixElement(process, a.precision, device=local)
         m4.set_good_helicities(mask)
         stream = torch.cuda.current_stream()
-        alphas_dev = 0.0 if ALPHAS[process] is None else ALPHAS[process]
         for _ in range(a.warmup):
             g = m4.generate(nevt, seed=1, alphas=alphas_dev)
             m4.compute(*g, out=bufs[4], selhel=bufs[5], selcol=bufs[6])
@@ -329,10 +400,14 @@ def main():
                                  "generate_plus_compute_mes_per_s": a.steps * nevt / (e1.elapsed_time(e2) * 1e-3),
                                  "api": "me_generate (seeded RAMBO on the device) + me_compute"}
         m4.close()
-        line["cpu_baseline"] = cpu_baseline(process)
+        cb = cpu_baseline(process)
+        line["roofline"]["flops_per_me_oracle"] = cb.pop("flops_per_me_counted")
+        line["roofline"]["flops_per_me_oracle_note"] = cb.pop("flops_note")
+        line["cpu_baseline"] = cb
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
+        dist.barrier()
         dist.destroy_process_group()
 
 

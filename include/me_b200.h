@@ -97,7 +97,9 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
                const double* d_rndcol, int64_t nevt, double* d_me, int32_t* d_selhel, int32_t* d_selcol,
                void* stream);
 
-/* Same call with HOST buffers (pinned or pageable): copies in, computes, copies out and synchronises.
+/* Same call with HOST buffers (pinned or pageable): copies in, computes, copies out and synchronises.  The batch
+ * flows in chunks through two device staging slots on three internal streams, so that the copies of neighbouring
+ * chunks overlap the kernels (pinned host memory needed for that; pageable memory still works, serially).
  * This is the end-to-end path bench.py times as `e2e`. */
 int me_compute_host(me_handle* h, const double* momenta, const double* gs, const double* rndhel,
                     const double* rndcol, int64_t nevt, double* me, int32_t* selhel, int32_t* selcol);
@@ -108,8 +110,8 @@ int me_compute_host(me_handle* h, const double* momenta, const double* gs, const
  * E = sqrts/2; final state from RAMBO flat phase space with the process' masses) and, where the pointer is not
  * NULL, d_gs[nevt] (alphas > 0: g_s = sqrt(4 pi alphas) fixed; alphas <= 0: alpha_s ~ U[0.10, 0.13] per event),
  * d_rndhel[nevt], d_rndcol[nevt] (uniforms in (0,1)) and d_weight[nevt] (the RAMBO phase-space weight).  The
- * numbers are those of paper_2503_21935_b200/inputs.py (same counter-based generator, fp64) up to the rounding of
- * the device math library.  Enqueues on `stream`, does not synchronise. */
+ * generator is counter-based (splitmix64 steps on (seed, stream, event index): event e of a stream is the same
+ * whatever the batch it is made in); its numpy oracle is oracle/rambo.py (tests/test_gpu_rambo.py).  Enqueues on `stream`, does not synchronise. */
 int me_generate(me_handle* h, uint64_t seed, int64_t start, int64_t nevt, double sqrts, double alphas,
                 double* d_momenta, double* d_gs, double* d_rndhel, double* d_rndcol, double* d_weight, void* stream);
 

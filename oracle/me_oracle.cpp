@@ -800,10 +800,14 @@ int orc_me_helicities(int proc, const double* params, const double* mom, const d
   if (!P) return -1;
   Params par = params_from(params);
   const int npar = P->npar, ncomb = P->ncomb, ncol = P->ncol;
+  // threads of THIS call only (no omp_set_num_threads: it would change the process-wide setting)
 #ifdef _OPENMP
-  if (nthreads > 0) omp_set_num_threads(nthreads);
+  const int nt = (nthreads > 0) ? nthreads : omp_get_max_threads();
+#else
+  const int nt = 1;
 #endif
-#pragma omp parallel for schedule(dynamic, 1)
+  (void)nt;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nt)
   for (int64_t e = 0; e < nevt; e++) {
     const double* pm = mom + (size_t)e * npar * 4;
     std::vector<cd> J;

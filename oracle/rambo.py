@@ -1,10 +1,16 @@
-"""Seeded synthetic inputs: counter-based PRNG + RAMBO flat phase space.
+"""ORACLE (test infrastructure, NOT the product): seeded synthetic inputs, counter-based PRNG + RAMBO flat phase space.
 
-This module is the *harness* (the role of the paper's standalone application, steps 1-2 of the
-MC chain: "random numbers are drawn ... converted into particle momenta using a phase space
-sampling algorithm").  It holds none of the matrix-element arithmetic and is the
-only module shared by the oracle tests and the CUDA tests/bench (both sides read the buffers it
-writes).  numpy only; no torch, no CUDA.
+Plain numpy restatement of steps 1-2 of the MC chain ("random numbers are drawn ... converted into particle
+momenta using a phase space sampling algorithm"; the paper's standalone application does both
+data-parallel).  Two roles:
+  * it writes the seeded input buffers (momenta, g_s, r_hel, r_col) that the oracle tests and the GPU parity tests
+    feed to both sides; it holds none of the matrix-element arithmetic;
+  * it is the oracle of the product's device-side generator me_generate (csrc/me_rambo.cu):
+    tests/test_gpu_rambo.py compares the two (uniforms bit-exact, momenta and weights to rounding).  Each side
+    implements the same counter-based generator on its own (splitmix64 steps); they share no code.
+Pinned by tests/test_inputs.py (P15: closed-form weights, N = 2 and N = 3 phase-space volumes, momentum conservation,
+mass shells, stream independence).  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / reference legs
+import it; bench.py's GPU arm makes its inputs with me_generate.  numpy only; no torch, no CUDA.
 
 Recipe: sqrt(s) = 1500 GeV, incoming p0 = (E,0,0,+E),
 p1 = (E,0,0,-E), final state from RAMBO (massless generation -> conformal boost to the CM frame ->

@@ -62,7 +62,8 @@ struct me_handle {
   // staging for me_compute_host
   void* d_stage;
   size_t stage_bytes;
-  cudaStream_t own_stream;
+  cudaStream_t own_stream, s_in, s_out;   // me_compute_host: compute, copy-in and copy-out streams
+  cudaEvent_t ev_in[2], ev_comp[2], ev_out[2];
   me::LaunchInfo last;
   mutable std::string err;
 };
@@ -184,7 +185,8 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
   h->d_cum = nullptr; h->cum_bytes = 0; h->d_frac = nullptr; h->d_stage = nullptr; h->stage_bytes = 0;
   h->d_scratch = nullptr; h->scratch_bytes = 0; h->have_pipe = false;
   memset(&h->pipe, 0, sizeof(h->pipe));
-  h->own_stream = nullptr;
+  h->own_stream = nullptr; h->s_in = nullptr; h->s_out = nullptr;
+  for (int i = 0; i < 2; i++) { h->ev_in[i] = nullptr; h->ev_comp[i] = nullptr; h->ev_out[i] = nullptr; }
   memset(&h->last, 0, sizeof(h->last));
   DeviceGuard guard(device);
   if ((e = guard.err) != cudaSuccess || (e = cudaMalloc(&h->d_frac, 128 * sizeof(unsigned long long))) != cudaSuccess) {
@@ -252,7 +254,16 @@ int me_destroy(me_handle* h) {
   if (h->d_cum) cudaFree(h->d_cum);
   if (h->d_frac) cudaFree(h->d_frac);
   if (h->d_stage) cudaFree(h->d_stage);
-  if (h->own_stream) cudaStreamDestroy(h->own_stream);
+  if (h->own_stream) {
+    cudaStreamDestroy(h->own_stream);
+    if (h->s_in) cudaStreamDestroy(h->s_in);
+    if (h->s_out) cudaStreamDestroy(h->s_out);
+    for (int i = 0; i < 2; i++) {
+      if (h->ev_in[i]) cudaEventDestroy(h->ev_in[i]);
+      if (h->ev_comp[i]) cudaEventDestroy(h->ev_comp[i]);
+      if (h->ev_out[i]) cudaEventDestroy(h->ev_out[i]);
+    }
+  }
   delete h;
   return ME_OK;
 }
@@ -427,34 +438,67 @@ int me_compute_host(me_handle* h, const double* momenta, const double* gs, const
   DeviceGuard guard(h->device);
   cudaError_t e = guard.err;
   if (e != cudaSuccess) return cuda_fail(h, e, "me_compute_host");
-  if (!h->own_stream && (e = cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking)) != cudaSuccess)
-    return cuda_fail(h, e, "me_compute_host: stream");
-  const size_t n = (size_t)nevt, bm = n * h->npar * 4 * 8, b8 = n * 8, b4 = n * 4;
-  // layout of the staging buffer: momenta | gs | rndhel | rndcol | me | selhel | selcol
-  const size_t want = bm + 4 * b8 + 2 * b4 + 64;
-  int rc = ensure(h, &h->d_stage, &h->stage_bytes, want);
+  if (!h->own_stream) {
+    // three internal streams (copy in, compute, copy out) and the events that chain them, made once
+    if ((e = cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking)) != cudaSuccess ||
+        (e = cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking)) != cudaSuccess ||
+        (e = cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking)) != cudaSuccess)
+      return cuda_fail(h, e, "me_compute_host: stream");
+    for (int i = 0; i < 2; i++)
+      if ((e = cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming)) != cudaSuccess ||
+          (e = cudaEventCreateWithFlags(&h->ev_comp[i], cudaEventDisableTiming)) != cudaSuccess ||
+          (e = cudaEventCreateWithFlags(&h->ev_out[i], cudaEventDisableTiming)) != cudaSuccess)
+        return cuda_fail(h, e, "me_compute_host: event");
+  }
+  // Chunks of the batch flow through two staging slots: while chunk k is computed, chunk k + 1 is copied in and the
+  // results of chunk k - 1 are copied out (one cudaMemcpyAsync per array and chunk).
+  int64_t chunk = (nevt + 7) / 8;
+  if (chunk < 16384) chunk = 16384;
+  if (chunk > 262144) chunk = 262144;
+  if (chunk > nevt) chunk = nevt;
+  const size_t c = (size_t)chunk, bm = c * h->npar * 4 * 8, b8 = c * 8, b4 = c * 4;
+  // layout of one staging slot: momenta | gs | rndhel | rndcol | me | selhel | selcol
+  const size_t slot = ((bm + 4 * b8 + 2 * b4 + 255) / 256) * 256;
+  int rc = ensure(h, &h->d_stage, &h->stage_bytes, 2 * slot);
   if (rc) return rc;
-  char* base = (char*)h->d_stage;
-  double* d_mom = (double*)base;
-  double* d_gs = (double*)(base + bm);
-  double* d_rh = (double*)(base + bm + b8);
-  double* d_rc = (double*)(base + bm + 2 * b8);
-  double* d_me = (double*)(base + bm + 3 * b8);
-  int32_t* d_sh = (int32_t*)(base + bm + 4 * b8);
-  int32_t* d_sc = (int32_t*)(base + bm + 4 * b8 + b4);
-  cudaStream_t st = h->own_stream;
-  if ((e = cudaMemcpyAsync(d_mom, momenta, bm, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(h, e, "H2D momenta");
-  if (gs && (e = cudaMemcpyAsync(d_gs, gs, b8, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(h, e, "H2D gs");
   const bool sh = selhel && rndhel, sc = selcol && rndcol;
-  if (sh && (e = cudaMemcpyAsync(d_rh, rndhel, b8, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(h, e, "H2D rndhel");
-  if (sc && (e = cudaMemcpyAsync(d_rc, rndcol, b8, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(h, e, "H2D rndcol");
-  rc = me_compute(h, d_mom, gs ? d_gs : nullptr, sh ? d_rh : nullptr, sc ? d_rc : nullptr, nevt, d_me,
-                  sh ? d_sh : nullptr, sc ? d_sc : nullptr, st);
-  if (rc) return rc;
-  if ((e = cudaMemcpyAsync(me_out, d_me, b8, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(h, e, "D2H me");
-  if (sh && (e = cudaMemcpyAsync(selhel, d_sh, b4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(h, e, "D2H selhel");
-  if (sc && (e = cudaMemcpyAsync(selcol, d_sc, b4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(h, e, "D2H selcol");
-  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: synchronize");
+  int64_t k = 0;
+  for (int64_t e0 = 0; e0 < nevt; e0 += chunk, k++) {
+    const int64_t n = (nevt - e0 < chunk) ? (nevt - e0) : chunk;
+    const int b = (int)(k & 1);
+    char* base = (char*)h->d_stage + (size_t)b * slot;
+    double* d_mom = (double*)base;
+    double* d_gs = (double*)(base + bm);
+    double* d_rh = (double*)(base + bm + b8);
+    double* d_rc = (double*)(base + bm + 2 * b8);
+    double* d_me = (double*)(base + bm + 3 * b8);
+    int32_t* d_sh = (int32_t*)(base + bm + 4 * b8);
+    int32_t* d_sc = (int32_t*)(base + bm + 4 * b8 + b4);
+    const size_t nn = (size_t)n;
+    // copy in (the slot's inputs are free once the compute of chunk k - 2 has finished)
+    if (k >= 2 && (e = cudaStreamWaitEvent(h->s_in, h->ev_comp[b], 0)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: wait");
+    if ((e = cudaMemcpyAsync(d_mom, momenta + (size_t)e0 * h->npar * 4, nn * h->npar * 32, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return cuda_fail(h, e, "H2D momenta");
+    if (gs && (e = cudaMemcpyAsync(d_gs, gs + e0, nn * 8, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return cuda_fail(h, e, "H2D gs");
+    if (sh && (e = cudaMemcpyAsync(d_rh, rndhel + e0, nn * 8, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return cuda_fail(h, e, "H2D rndhel");
+    if (sc && (e = cudaMemcpyAsync(d_rc, rndcol + e0, nn * 8, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return cuda_fail(h, e, "H2D rndcol");
+    if ((e = cudaEventRecord(h->ev_in[b], h->s_in)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: record");
+    // compute (the slot's outputs are free once the copy-out of chunk k - 2 has finished)
+    if ((e = cudaStreamWaitEvent(h->own_stream, h->ev_in[b], 0)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: wait");
+    if (k >= 2 && (e = cudaStreamWaitEvent(h->own_stream, h->ev_out[b], 0)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: wait");
+    rc = me_compute(h, d_mom, gs ? d_gs : nullptr, sh ? d_rh : nullptr, sc ? d_rc : nullptr, n, d_me,
+                    sh ? d_sh : nullptr, sc ? d_sc : nullptr, h->own_stream);
+    if (rc) return rc;
+    if ((e = cudaEventRecord(h->ev_comp[b], h->own_stream)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: record");
+    // copy out
+    if ((e = cudaStreamWaitEvent(h->s_out, h->ev_comp[b], 0)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: wait");
+    if ((e = cudaMemcpyAsync(me_out + e0, d_me, nn * 8, cudaMemcpyDeviceToHost, h->s_out)) != cudaSuccess) return cuda_fail(h, e, "D2H me");
+    if (sh && (e = cudaMemcpyAsync(selhel + e0, d_sh, nn * 4, cudaMemcpyDeviceToHost, h->s_out)) != cudaSuccess) return cuda_fail(h, e, "D2H selhel");
+    if (sc && (e = cudaMemcpyAsync(selcol + e0, d_sc, nn * 4, cudaMemcpyDeviceToHost, h->s_out)) != cudaSuccess) return cuda_fail(h, e, "D2H selcol");
+    if ((e = cudaEventRecord(h->ev_out[b], h->s_out)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: record");
+  }
+  if ((e = cudaStreamSynchronize(h->s_out)) != cudaSuccess || (e = cudaStreamSynchronize(h->own_stream)) != cudaSuccess ||
+      (e = cudaStreamSynchronize(h->s_in)) != cudaSuccess)
+    return cuda_fail(h, e, "me_compute_host: synchronize");
   return ME_OK;
 }
 

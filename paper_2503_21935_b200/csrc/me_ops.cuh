@@ -175,7 +175,8 @@ template <typename T> ME_HD spinbasis<T> make_spinbasis(mom4<T> p, T m) {
   if (pp == T(0)) {  // at rest: quantise along +z
     s.xp[0] = mk<T>(T(1), T(0)); s.xp[1] = mk<T>(T(0), T(0));
     s.xm[0] = mk<T>(T(0), T(0)); s.xm[1] = mk<T>(T(1), T(0));
-  } else if (pt2 == T(0) && pz < T(0)) {
+  } else if ((pt2 == T(0) && pz < T(0)) || ((pz >= T(0)) ? pp + pz : pt2 / (pp - pz)) == T(0)) {
+    // exactly backward, or so close to it that |p| + pz underflows (fp32): the -z limit of the formulas below
     s.xp[0] = mk<T>(T(0), T(0)); s.xp[1] = mk<T>(T(1), T(0));
     s.xm[0] = mk<T>(T(-1), T(0)); s.xm[1] = mk<T>(T(0), T(0));
   } else {

@@ -2,8 +2,9 @@
 // application, "random numbers are drawn ... converted into particle momenta using a phase space sampling
 // algorithm"): counter-based uniforms -> RAMBO flat phase space -> momenta[nevt][npar][4], plus the
 // per-event g_s and the two selection randoms, written straight into HBM so that a batch never touches the host.
-// The numbers are those of paper_2503_21935_b200/inputs.py (same generator, same algorithm, fp64): the harness'
-// numpy version is the reference this kernel is tested against (tests/test_gpu_rambo.py).  One event per thread.
+// Checked against the numpy oracle oracle/rambo.py, which implements the same counter-based generator and the same
+// RAMBO steps on its own (tests/test_gpu_rambo.py: uniforms bit-exact, momenta and weights to rounding); no code is
+// shared.  One event per thread.
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>

@@ -66,12 +66,14 @@ def load_library(path: str = LIB_PATH):
     return L
 
 
-def _ptr(t, dtype=None):
-    """Device pointer of a contiguous CUDA tensor (or None)."""
+def _ptr(t, dtype=None, device=None):
+    """Device pointer of a contiguous CUDA tensor (or None); with `device`, the tensor must live on that ordinal."""
     if t is None:
         return None
     if not t.is_cuda or not t.is_contiguous():
         raise MEError("expected a contiguous CUDA tensor")
+    if device is not None and t.device.index != device:
+        raise MEError(f"tensor on cuda:{t.device.index}, but this handle was created for cuda:{device}")
     if dtype is not None and t.dtype != dtype:
         raise MEError(f"expected dtype {dtype}, got {t.dtype}")
     return ctypes.c_void_p(t.data_ptr())
@@ -109,6 +111,10 @@ class MatrixElement:
             msg = self._L.me_last_error(self._h)
             raise MEError(f"error {rc}: {msg.decode() if msg else ''}")
 
+    def _same_device(self, stream):
+        if getattr(stream, "device", None) is not None and stream.device.index != self.device:
+            raise MEError(f"stream on cuda:{stream.device.index}, but this handle was created for cuda:{self.device}")
+
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
             self._L.me_destroy(self._h)
@@ -141,7 +147,8 @@ class MatrixElement:
         import torch
         nevt = momenta.shape[0]
         s = stream if stream is not None else torch.cuda.current_stream(momenta.device)
-        self._check(self._L.me_filter_helicities(self._h, _ptr(momenta, torch.float64), _ptr(gs, torch.float64), nevt,
+        self._same_device(s)
+        self._check(self._L.me_filter_helicities(self._h, _ptr(momenta, torch.float64, self.device), _ptr(gs, torch.float64, self.device), nevt,
                                                  ctypes.c_void_p(s.cuda_stream)))
         return self.get_good_helicities()
 
@@ -176,9 +183,10 @@ class MatrixElement:
         if rndcol is not None and selcol is None:
             selcol = torch.empty(nevt, dtype=torch.int32, device=dev)
         s = stream if stream is not None else torch.cuda.current_stream(dev)
-        f64 = torch.float64
-        self._check(self._L.me_compute(self._h, _ptr(momenta, f64), _ptr(gs, f64), _ptr(rndhel, f64), _ptr(rndcol, f64),
-                                       nevt, _ptr(out, f64), _ptr(selhel, torch.int32), _ptr(selcol, torch.int32),
+        f64, d = torch.float64, self.device
+        self._same_device(s)
+        self._check(self._L.me_compute(self._h, _ptr(momenta, f64, d), _ptr(gs, f64, d), _ptr(rndhel, f64, d), _ptr(rndcol, f64, d),
+                                       nevt, _ptr(out, f64, d), _ptr(selhel, torch.int32, d), _ptr(selcol, torch.int32, d),
                                        ctypes.c_void_p(s.cuda_stream)))
         return out, selhel, selcol
 
@@ -207,6 +215,9 @@ class MatrixElement:
         gs, rh, rc = (torch.empty(nevt, dtype=f64, device=dev) for _ in range(3))
         wt = torch.empty(nevt, dtype=f64, device=dev) if want_weight else None
         s = stream if stream is not None else torch.cuda.current_stream(dev)
+        if dev.index != self.device:
+            raise MEError(f"device cuda:{dev.index} requested, but this handle was created for cuda:{self.device}")
+        self._same_device(s)
         self._check(self._L.me_generate(self._h, int(seed), int(start), int(nevt), float(sqrts), float(alphas), _ptr(mom, f64),
                                         _ptr(gs, f64), _ptr(rh, f64), _ptr(rc, f64), _ptr(wt, f64), ctypes.c_void_p(s.cuda_stream)))
         return (mom, gs, rh, rc, wt) if want_weight else (mom, gs, rh, rc)

@@ -4,7 +4,7 @@ size (finite, positive, selections inside the good set / colour range, independe
 import numpy as np
 import pytest
 
-from paper_2503_21935_b200 import inputs as I
+from oracle import rambo as I
 
 pytestmark = pytest.mark.gpu
 

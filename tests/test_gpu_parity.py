@@ -6,7 +6,7 @@ where the oracle's cumulative weight lies within tolerance of the random number.
 import numpy as np
 import pytest
 
-from paper_2503_21935_b200 import inputs as I
+from oracle import rambo as I
 
 pytestmark = pytest.mark.gpu
 
@@ -236,4 +236,34 @@ def test_group_kernel_edge_batches(torch_cuda):
     me_h, sh, sc = m.compute_host(case["mom"], case["gs"], case["rh"], case["rc"])
     assert np.allclose(me_h, case["sel"]["me"], rtol=1e-10, atol=0)
     assert np.mean(sh == case["sel"]["selhel"]) > 0.999 and np.mean(sc == case["sel"]["selcol"]) > 0.999
+    m.close()
+
+
+@pytest.mark.parametrize("process,precision,n", [("gg_ttgg", "fp64", 2 * 4736 + 1234), ("gg_ttgg", "fp32", 2 * 4736 + 1234),
+                                                 ("gg_ttggg", "fp64", 900), ("gg_ttggg", "mixed", 900)])
+def test_lane_group_pipeline_is_deterministic_and_chunk_independent(torch_cuda, process, precision, n):
+    """The lane-group pipeline is warp-synchronous shared-memory code whose scratch is reused from chunk to chunk
+    (compute-sanitizer is closed on this pool): a race or a wrong chunk offset would show as
+    run-to-run or split-dependent differences.  Two runs of the same batch are bit-identical, and so are the results
+    of the batch done in one call (several internal chunks on two streams) and in two calls of unequal size."""
+    from paper_2503_21935_b200.me import MatrixElement
+    dev = torch_cuda.device("cuda:0")
+    mom = torch_cuda.from_numpy(I.make_momenta(process, n, seed=5)).to(dev)
+    gs = torch_cuda.from_numpy(I.make_gs(n, seed=5, alphas=ALPHAS[process])).to(dev)
+    rh, rc = (torch_cuda.from_numpy(x).to(dev) for x in I.make_rnd(n, seed=5))
+    m = MatrixElement(process, precision)
+    m.filter_helicities(mom, gs)
+    runs = []
+    for _ in range(3):
+        me, sh, sc = m.compute(mom, gs, rh, rc)
+        torch_cuda.cuda.synchronize()
+        runs.append((me.clone(), sh.clone(), sc.clone()))
+    for r in runs[1:]:
+        assert all(torch_cuda.equal(x, y) for x, y in zip(r, runs[0]))
+    k = n // 3 + 1
+    a = m.compute(mom[:k].contiguous(), gs[:k].contiguous(), rh[:k].contiguous(), rc[:k].contiguous())
+    b = m.compute(mom[k:].contiguous(), gs[k:].contiguous(), rh[k:].contiguous(), rc[k:].contiguous())
+    torch_cuda.cuda.synchronize()
+    for i in range(3):
+        assert torch_cuda.equal(torch_cuda.cat([a[i], b[i]]), runs[0][i])
     m.close()

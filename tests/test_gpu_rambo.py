@@ -1,11 +1,10 @@
-"""me_generate (device-side seeded inputs) against the harness generator
-paper_2503_21935_b200/inputs.py: same counter-based uniforms (bit-exact), same RAMBO algorithm (fp64; equal up to
-the rounding of the device math library), physical momenta, and an ME computed from device-made inputs equal to
-the ME from host-made inputs."""
+"""me_generate (device-side seeded inputs) against its numpy oracle oracle/rambo.py: same
+counter-based uniforms (bit-exact), same RAMBO algorithm (fp64; equal up to the rounding of the device math
+library), physical momenta, and an ME computed from device-made inputs equal to the ME from oracle-made inputs."""
 import numpy as np
 import pytest
 
-from paper_2503_21935_b200 import inputs as I
+from oracle import rambo as I
 
 pytestmark = pytest.mark.gpu
 

@@ -4,7 +4,7 @@ import math
 import numpy as np
 import pytest
 
-from paper_2503_21935_b200 import inputs as I
+from oracle import rambo as I
 
 
 def test_uniforms_are_counter_based_and_open_interval():

@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 from oracle import oracle as O
-from paper_2503_21935_b200 import inputs as I
+from oracle import rambo as I
 
 GG = ["gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg"]
 

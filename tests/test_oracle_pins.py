@@ -10,7 +10,7 @@ import numpy as np
 import pytest
 
 from oracle import oracle as O
-from paper_2503_21935_b200 import inputs as I
+from oracle import rambo as I
 from helpers import read_golden
 
 GOLD = read_golden("worked_points.txt")

@@ -5,7 +5,7 @@ import pytest
 
 from oracle import bg_numpy as B
 from oracle import oracle as O
-from paper_2503_21935_b200 import inputs as I
+from oracle import rambo as I
 
 
 @pytest.mark.parametrize("proc,nev", [("gg_tt", 3), ("gg_ttg", 3), ("gg_ttgg", 1), ("gg_ttggg", 1)])

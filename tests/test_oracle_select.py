@@ -15,7 +15,7 @@ import numpy as np
 import pytest
 
 from oracle import oracle as O
-from paper_2503_21935_b200 import inputs as I
+from oracle import rambo as I
 
 
 def _one_event(proc, seed=5):
