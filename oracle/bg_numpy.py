@@ -156,3 +156,76 @@ def ordered_amplitudes(momenta, gs, hel, mt=173.0, wt=0.0):
             amp += L(s[:a]) @ (1j * gs * slash(G(s[a:])[0])) @ v
         out[n] = amp
     return orders, out
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# Route B': ONE Feynman diagram from its structural key (multichannel pins, reading R17).
+# Key grammar (me_oracle.cpp build_channels): leaf = particle index; "(A,B)" three-gluon vertex; "[A,B,C]" four-gluon
+# vertex; blocks attached to the quark line from t to tbar separated by "|".  Literal Feynman rules as in the header,
+# colour stripped; a four-gluon vertex has three colour-structure terms, so a diagram with v of them has 3^v term
+# amplitudes.  Chiral representation, numpy: shares nothing with Route A except the statement of the rules.
+# ----------------------------------------------------------------------------------------------------------------
+def _parse_tree(s, pos):
+    if s[pos] in "([":
+        close = ")" if s[pos] == "(" else "]"
+        kids = []
+        pos += 1
+        while True:
+            kid, pos = _parse_tree(s, pos)
+            kids.append(kid)
+            if s[pos] == ",":
+                pos += 1
+            else:
+                assert s[pos] == close
+                return tuple(kids), pos + 1
+    end = pos
+    while end < len(s) and s[end].isdigit():
+        end += 1
+    return int(s[pos:end]), end
+
+
+def diagram_term_amplitudes(key, momenta, gs, hel, mt=173.0, wt=0.0):
+    """Amplitudes of the colour-structure terms of the diagram `key` for one event and helicity assignment."""
+    p = np.asarray(momenta, dtype=float)
+    k = {i: (p[i] if i < 2 else -p[i]) for i in range(p.shape[0])}
+
+    def tree(t):
+        """list of (current, momentum) over the term choices of the four-gluon vertices below t"""
+        if isinstance(t, int):
+            e = polvec(p[t], hel[t])
+            return [((e if t < 2 else e.conj()).astype(complex), k[t].astype(complex))]
+        subs = [tree(c) for c in t]
+        out = []
+        for combo in itertools.product(*subs):
+            K = sum(c[1] for c in combo)
+            prop = -1j / mdot(K, K)
+            if len(t) == 2:
+                (A, kA), (B, kB) = combo
+                k3 = -K
+                W = mdot(A, B) * (kA - kB) + B * mdot(kB - k3, A) + A * mdot(k3 - kA, B)
+                out.append((prop * gs * W, K))
+            else:
+                A, B, C = (c[0] for c in combo)
+                for W in (mdot(A, C) * B - mdot(B, C) * A, mdot(A, B) * C - mdot(B, C) * A, mdot(A, B) * C - mdot(A, C) * B):
+                    out.append((prop * (-1j * gs * gs) * W, K))
+        return out
+
+    blocks = []
+    for b in key.split("|"):
+        t, end = _parse_tree(b, 0)
+        assert end == len(b)
+        blocks.append(tree(t))
+    ub = bar(spinor_u(p[2], mt, hel[2]))
+    v = spinor_v(p[3], mt, hel[3])
+    amps = []
+    for combo in itertools.product(*blocks):
+        row = ub
+        q = p[2].astype(complex)
+        for j, (cur, K) in enumerate(combo):
+            row = row @ (1j * gs * slash(cur))
+            if j + 1 < len(combo):
+                q = q - K
+                den = mdot(q, q) - mt * mt + 1j * mt * wt
+                row = row @ (1j * (slash(q) + mt * np.eye(4)) / den)
+        amps.append(row @ v)
+    return np.array(amps)

@@ -32,6 +32,7 @@
 #include <cstring>
 #include <map>
 #include <mutex>
+#include <string>
 #include <vector>
 #ifdef _OPENMP
 #include <omp.h>
@@ -381,6 +382,9 @@ struct Process {
   std::map<std::vector<int>, int> flow_index;
   std::vector<double> C;  // colour matrix [ncol][ncol]
   long ndiag_counted;
+  // multichannel (reading R17): channel = Feynman diagram, numbered by its structural key
+  std::vector<std::string> chan_keys;  // [ndiag], sorted
+  std::vector<int> chan_of_sub;        // [nsub] channel of every sub-diagram (the terms of a four-gluon vertex share it)
 };
 
 static int lowbit(unsigned m) { return __builtin_ctz(m); }
@@ -590,6 +594,34 @@ static void build_color_matrix(Process& P) {
   P.C = acc;
 }
 
+// Structural key of a gluon tree and of a Feynman diagram (reading R17): a leaf is its particle index, a
+// three-gluon vertex "(A,B)" with the lowest leg in A, a four-gluon vertex "[A,B,C]" with the lowest leg in A and the
+// lowest of the rest in B; a diagram is the keys of the trees attached to the quark line from t to tbar joined by "|".
+// Channels are the distinct keys in increasing (byte-wise) order: the three colour-structure terms of a four-gluon
+// vertex belong to one diagram, hence to one channel.
+static std::string tree_key(const Process& P, int t) {
+  const Tree& T = P.trees[t];
+  if (T.kind == 0) return std::to_string(T.leg);
+  if (T.kind == 3) return "(" + tree_key(P, T.ch[0]) + "," + tree_key(P, T.ch[1]) + ")";
+  return "[" + tree_key(P, T.ch[0]) + "," + tree_key(P, T.ch[1]) + "," + tree_key(P, T.ch[2]) + "]";
+}
+static void build_channels(Process& P) {
+  std::vector<std::string> keys(P.sub.size());
+  for (size_t d = 0; d < P.sub.size(); d++) {
+    std::vector<int> blocks{P.sub[d].last};
+    for (int n = P.sub[d].prefix; n > 0; n = P.trie[n].parent) blocks.push_back(P.trie[n].tree);
+    std::string k;
+    for (size_t i = blocks.size(); i-- > 0;) { k += tree_key(P, blocks[i]); if (i) k += "|"; }
+    keys[d] = k;
+  }
+  P.chan_keys = keys;
+  std::sort(P.chan_keys.begin(), P.chan_keys.end());
+  P.chan_keys.erase(std::unique(P.chan_keys.begin(), P.chan_keys.end()), P.chan_keys.end());
+  P.chan_of_sub.resize(P.sub.size());
+  for (size_t d = 0; d < P.sub.size(); d++)
+    P.chan_of_sub[d] = (int)(std::lower_bound(P.chan_keys.begin(), P.chan_keys.end(), keys[d]) - P.chan_keys.begin());
+}
+
 static Process* build_process(int id) {
   Process* P = new Process();
   P->id = id;
@@ -626,6 +658,7 @@ static Process* build_process(int id) {
   enumerate_lines(*P, all, 0, unit, nd);
   P->ndiag = (int)nd;
   build_color_matrix(*P);
+  build_channels(*P);
   return P;
 }
 static Process* get_process(int id) {
@@ -872,6 +905,55 @@ int orc_count_ops(int proc, const double* params, const double* mom, double gs, 
   (void)proc; (void)params; (void)mom; (void)gs; (void)mask; (void)out4; (void)me_raw;
   return -2;
 #endif
+}
+
+// Multichannel weights ("events from different channels"; reading R17): for every
+// event and channel d (= Feynman diagram), num[e][d] = sum over the helicities of mask and over the colour-structure
+// terms t of the diagram of |A_{d,t}(h)|^2, with A the Feynman-rule value of the (sub)diagram evaluated by eval_jamps.
+// The single-diagram-enhancement weight of channel d is num[e][d] / sum_d' num[e][d'].
+int orc_multichannel(int proc, const double* params, const double* mom, const double* gs, int64_t nevt,
+                     const uint8_t* mask, double* num, int nthreads) {
+  Process* P = get_process(proc);
+  if (!P || proc == 0) return -1;
+  Params par = params_from(params);
+  const int npar = P->npar, ncomb = P->ncomb, nch = (int)P->chan_keys.size();
+#ifdef _OPENMP
+  const int nt = (nthreads > 0) ? nthreads : omp_get_max_threads();
+#else
+  const int nt = 1;
+#endif
+  (void)nt;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nt)
+  for (int64_t e = 0; e < nevt; e++) {
+    std::vector<cd> J, A;
+    double* out = num + (size_t)e * nch;
+    for (int d = 0; d < nch; d++) out[d] = 0.0;
+    for (int h = 0; h < ncomb; h++) {
+      if (mask && !mask[h]) continue;
+      eval_jamps(*P, par, mom + (size_t)e * npar * 4, gs[e], h, -1, J, &A, 0);
+      for (size_t d = 0; d < A.size(); d++) out[P->chan_of_sub[d]] += to_double(cnorm(A[d]));
+    }
+  }
+  return 0;
+}
+// number of channels, and (buf != NULL) their keys separated by newlines; returns the bytes needed
+int orc_channel_keys(int proc, char* buf, int cap) {
+  Process* P = get_process(proc);
+  if (!P || proc == 0) return -1;
+  std::string all;
+  for (auto& k : P->chan_keys) { all += k; all += "\n"; }
+  if (buf && cap > (int)all.size()) memcpy(buf, all.c_str(), all.size() + 1);
+  return (int)all.size() + 1;
+}
+// allowed[ndiag][ncol]: 1 iff the diagram contributes to the colour flow (some term has K != 0)
+int orc_channel_flows(int proc, uint8_t* allowed) {
+  Process* P = get_process(proc);
+  if (!P || proc == 0) return -1;
+  const int nch = (int)P->chan_keys.size();
+  memset(allowed, 0, (size_t)nch * P->ncol);
+  for (size_t d = 0; d < P->sub.size(); d++)
+    for (auto& kc : P->sub[d].K) allowed[(size_t)P->chan_of_sub[d] * P->ncol + kc.first] = 1;
+  return nch;
 }
 
 // operation census of ONE helicity: number of three-/four-gluon currents, quark-line chain steps,

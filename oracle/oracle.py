@@ -60,6 +60,9 @@ def lib():
         L.orc_brute_color.argtypes = [ctypes.c_int, dp, dp, ctypes.c_double, ctypes.c_int, dp]
         L.orc_wavefunction.argtypes = [ctypes.c_int, dp, ctypes.c_double, ctypes.c_int, dp]
         L.orc_slash.argtypes = [dp, dp]
+        L.orc_multichannel.argtypes = [ctypes.c_int, dp, dp, dp, ctypes.c_int64, ctypes.c_void_p, dp, ctypes.c_int]
+        L.orc_channel_keys.argtypes = [ctypes.c_int, ctypes.c_char_p, ctypes.c_int]
+        L.orc_channel_flows.argtypes = [ctypes.c_int, ctypes.c_void_p]
         L.orc_num_threads.restype = ctypes.c_int
         _lib = L
     return _lib
@@ -145,11 +148,46 @@ def me(process, momenta, gs, params=None, mask=None, nthreads=0) -> np.ndarray:
     return mh.sum(axis=1) / info(process)["denom"]
 
 
-def select(process, momenta, gs, rndhel, rndcol, params=None, mask=None, nthreads=0):
+def channel_keys(process) -> list:
+    """Structural keys of the channels (= Feynman diagrams) in channel order (reading R17; see me_oracle.cpp)."""
+    n = lib().orc_channel_keys(PROC_ID[process], None, 0)
+    assert n > 0
+    buf = ctypes.create_string_buffer(n + 1)
+    assert lib().orc_channel_keys(PROC_ID[process], buf, n + 1) == n
+    return buf.value.decode().split("\n")[:-1]
+
+
+def channel_flows(process) -> np.ndarray:
+    """allowed[ndiag][ncol] (bool): the colour flows a channel's diagram contributes to."""
+    i = info(process)
+    out = np.zeros((i["ndiag"], i["ncol"]), dtype=np.uint8)
+    assert lib().orc_channel_flows(PROC_ID[process], out.ctypes.data) == i["ndiag"]
+    return out.astype(bool)
+
+
+def multichannel(process, momenta, gs, params=None, mask=None, nthreads=0) -> np.ndarray:
+    """num[nevt][ndiag] = sum over (good) helicities and colour-structure terms of |A_d|^2 (reading R17); the
+    single-diagram-enhancement weight of channel d is num[:, d] / num.sum(axis=1)."""
+    i = info(process)
+    mom = np.ascontiguousarray(momenta, dtype=np.float64)
+    nevt = mom.shape[0]
+    g = np.ascontiguousarray(np.broadcast_to(np.asarray(gs, dtype=np.float64), (nevt,)))
+    num = np.zeros((nevt, i["ndiag"]), dtype=np.float64)
+    p = _params(params)
+    m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    rc = lib().orc_multichannel(PROC_ID[process], _dp(p), _dp(mom), _dp(g), nevt, None if m is None else m.ctypes.data,
+                                _dp(num), int(nthreads))
+    assert rc == 0
+    return num
+
+
+def select(process, momenta, gs, rndhel, rndcol, params=None, mask=None, nthreads=0, channel=None):
     """Reading R11.  Returns dict(me, selhel, selcol, cumhel [nevt][ncomb], cumcol [nevt][ncol]).
 
     helicity: scan helicities in table order, pick the first good h with r_hel * S < sum_{h'<=h} |M_h'|^2,
     fall back to the last good one; colour: weights w_c = sum_{h good} |J_c(h)|^2, same scan with r_col.
+    With channel[nevt] (reading R17) the colour weights of the flows the event's channel does not contribute to
+    are set to zero before the scan (fallback: the last allowed flow).
     """
     i = info(process)
     mh, j2 = me_helicities(process, momenta, gs, params, mask=mask, want_jamp2=True, nthreads=nthreads)
@@ -159,6 +197,10 @@ def select(process, momenta, gs, rndhel, rndcol, params=None, mask=None, nthread
     selcol = np.zeros(nevt, dtype=np.int32)
     cumhel = np.zeros_like(mh)
     wcol = j2.sum(axis=1)
+    allowed = None
+    if channel is not None:
+        allowed = channel_flows(process)[np.asarray(channel)]      # [nevt][ncol]
+        wcol = np.where(allowed, wcol, 0.0)
     cumcol = np.zeros_like(wcol)
     last_good = int(np.nonzero(good)[0][-1])
     for e in range(nevt):
@@ -177,9 +219,9 @@ def select(process, momenta, gs, rndhel, rndcol, params=None, mask=None, nthread
         for c in range(i["ncol"]):
             totc += wcol[e, c]
             cumcol[e, c] = totc
-        selc = i["ncol"] - 1
+        selc = i["ncol"] - 1 if allowed is None else int(np.nonzero(allowed[e])[0][-1])
         for c in range(i["ncol"]):
-            if rndcol[e] * totc < cumcol[e, c]:
+            if (allowed is None or allowed[e, c]) and rndcol[e] * totc < cumcol[e, c]:
                 selc = c
                 break
         selcol[e] = selc
