@@ -97,6 +97,26 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
                const double* d_rndcol, int64_t nevt, double* d_me, int32_t* d_selhel, int32_t* d_selcol,
                void* stream);
 
+/* Multichannel running ("events from different channels" in one launch).  Reading
+ * R17 of DESIGN.md (the paper gives no formula): a channel is a Feynman diagram of the process; channels are numbered
+ * 0 .. ndiag-1 in increasing byte order of the structural keys returned by me_channel_table.  d_channel[nevt] (device,
+ * int32, values outside 0 .. ndiag-1 are clamped for the colour selection and give num = 0) assigns a channel to every
+ * event; events of any mix of channels may share a call (a warp never works on two events at once in the kernels that
+ * look at the channel).  Outputs, beside those of me_compute:
+ *   d_num[nevt] = sum over the good helicities and the colour-structure terms of diagram d = channel[e] of |A_d|^2,
+ *   d_den[nevt] = the same summed over ALL diagrams   (fp64 in every build; both include g_s^(2n)),
+ * so that num/den is the single-diagram-enhancement weight of the event's channel; and the colour selection
+ * (d_selcol) only picks flows that diagram d contributes to.  d_me is the plain ME (multiply by num/den yourself).
+ * gg processes only (ME_ERR_PROCESS for ee_mumu).  The first call allocates the kernel's per-event scratch
+ * (3.6 KB x min(nevt, 65536) at most); later calls with no more events do not allocate.  Enqueues on `stream`. */
+int me_compute_multichannel(me_handle* h, const double* d_momenta, const double* d_gs, const double* d_rndhel,
+                            const double* d_rndcol, const int32_t* d_channel, int64_t nevt, double* d_me,
+                            int32_t* d_selhel, int32_t* d_selcol, double* d_num, double* d_den, void* stream);
+/* Channel keys, one per line in channel order, NUL terminated: the trees attached to the quark line from t to tbar
+ * separated by "|"; a leaf is its particle index, "(A,B)" a three-gluon vertex, "[A,B,C]" a four-gluon vertex.
+ * Returns the bytes needed (call with out = NULL first), or a negative error code. */
+int me_channel_table(const me_handle* h, char* out, int cap);
+
 /* Same call with HOST buffers (pinned or pageable): copies in, computes, copies out and synchronises.  The batch
  * flows in chunks through two device staging slots on three internal streams, so that the copies of neighbouring
  * chunks overlap the kernels (pinned host memory needed for that; pageable memory still works, serially).

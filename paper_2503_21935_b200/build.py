@@ -42,6 +42,8 @@ def _units():
                 defs.append("-DME_IS_EE_MUMU")
             src = "me_proc_group.cu" if p in GROUP_LAYOUT else "me_proc.cu"
             yield f"{p}_p{prec}", os.path.join(CSRC, src), defs
+    for p in PROCS[1:]:
+        yield f"{p}_diag", os.path.join(CSRC, "me_proc_diag.cu"), [f"-DME_PROC={p}"]
     yield "api", os.path.join(CSRC, "me_api.cu"), []
     yield "peak", os.path.join(CSRC, "me_peak.cu"), []
     yield "rambo", os.path.join(CSRC, "me_rambo.cu"), []
@@ -53,8 +55,9 @@ def _deps_hash(defs):
         for f in sorted(files):
             if f.endswith((".cu", ".cuh", ".h")):
                 # a unit depends on the shared headers and on its own generated header only
-                if f.startswith(("proc_", "grp_", "cmat_")) and not any(
-                        f in (f"proc_{d.split('=')[1]}.cuh", f"grp_{d.split('=')[1]}.cuh", f"cmat_{d.split('=')[1]}.h")
+                if f.startswith(("proc_", "grp_", "cmat_", "diag_")) and not any(
+                        f in (f"proc_{d.split('=')[1]}.cuh", f"grp_{d.split('=')[1]}.cuh", f"cmat_{d.split('=')[1]}.h",
+                              f"diag_{d.split('=')[1]}.cuh")
                         for d in defs if d.startswith("-DME_PROC=")):
                     continue
                 if f == "me_tables.h" and defs:

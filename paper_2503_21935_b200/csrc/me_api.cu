@@ -25,17 +25,38 @@ ME_DECL(gg_ttg)
 ME_DECL(gg_ttgg)
 ME_DECL(gg_ttggg)
 
+// multichannel (me_proc_diag.cu), gg processes only
+typedef int (*diag_fn)(const me::LaunchArgs&, const int*, double*, double*, void*, void*);
+typedef int (*chanflows_fn)(const unsigned**, int*);
+typedef size_t (*diag_scratch_fn)();
+#define ME_DECL_DIAG(name)                                                                          \
+  int me_launch_diag_##name(const me::LaunchArgs&, const int*, double*, double*, void*, void*);    \
+  int me_chanflows_##name(const unsigned**, int*);                                                  \
+  size_t me_diag_scratch_##name();
+ME_DECL_DIAG(gg_tt)
+ME_DECL_DIAG(gg_ttg)
+ME_DECL_DIAG(gg_ttgg)
+ME_DECL_DIAG(gg_ttggg)
+
+#include "gen/me_tables.h"
+
 namespace {
 
 struct ProcDesc {
   const char* name;
   int npar, ngl, ndiag;
   launch_fn fn[3];
+  diag_fn diag;
+  chanflows_fn chanflows;
+  diag_scratch_fn diag_scratch;
+  const char* chan_keys;
 };
 #define ME_ROW(name, npar, ngl, ndiag) \
-  { #name, npar, ngl, ndiag, { me_launch_##name##_p0, me_launch_##name##_p1, me_launch_##name##_p2 } }
+  { #name, npar, ngl, ndiag, { me_launch_##name##_p0, me_launch_##name##_p1, me_launch_##name##_p2 }, \
+    me_launch_diag_##name, me_chanflows_##name, me_diag_scratch_##name, kChanKeys_##name }
 const ProcDesc kProcs[] = {
-    ME_ROW(ee_mumu, 4, 0, 2), ME_ROW(gg_tt, 4, 2, 3), ME_ROW(gg_ttg, 5, 3, 16),
+    { "ee_mumu", 4, 0, 2, { me_launch_ee_mumu_p0, me_launch_ee_mumu_p1, me_launch_ee_mumu_p2 }, nullptr, nullptr, nullptr, kChanKeys_ee_mumu },
+    ME_ROW(gg_tt, 4, 2, 3), ME_ROW(gg_ttg, 5, 3, 16),
     ME_ROW(gg_ttgg, 6, 4, 123), ME_ROW(gg_ttggg, 7, 5, 1240),
 };
 
@@ -57,6 +78,8 @@ struct me_handle {
   // lane-group pipeline (gg_ttgg, gg_ttggg): per-event data and jamps between its kernels, one chunk of events
   void* d_scratch;
   size_t scratch_bytes;
+  void* d_mc;         // multichannel: per-event data of the diagram kernel (grows on first use)
+  size_t mc_bytes;
   me::PipeCtx pipe;   // internal streams / events of the pipeline (valid iff d_scratch)
   bool have_pipe;
   // staging for me_compute_host
@@ -183,7 +206,7 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
   }
   h->have_good = false; h->good.n = 0;
   h->d_cum = nullptr; h->cum_bytes = 0; h->d_frac = nullptr; h->d_stage = nullptr; h->stage_bytes = 0;
-  h->d_scratch = nullptr; h->scratch_bytes = 0; h->have_pipe = false;
+  h->d_scratch = nullptr; h->scratch_bytes = 0; h->have_pipe = false; h->d_mc = nullptr; h->mc_bytes = 0;
   memset(&h->pipe, 0, sizeof(h->pipe));
   h->own_stream = nullptr; h->s_in = nullptr; h->s_out = nullptr;
   for (int i = 0; i < 2; i++) { h->ev_in[i] = nullptr; h->ev_comp[i] = nullptr; h->ev_out[i] = nullptr; }
@@ -250,6 +273,7 @@ int me_destroy(me_handle* h) {
     for (int i = 0; i < 2; i++) cudaEventDestroy(h->pipe.k1[i]);
     for (int i = 0; i < 4; i++) cudaEventDestroy(h->pipe.k2[i]);
   }
+  if (h->d_mc) cudaFree(h->d_mc);
   if (h->d_scratch) cudaFree(h->d_scratch);
   if (h->d_cum) cudaFree(h->d_cum);
   if (h->d_frac) cudaFree(h->d_frac);
@@ -300,7 +324,6 @@ int me_color_table(const me_handle* h, int8_t* out) {
 // ------------------------------------------------------------------------------------------------
 // colour matrix, helicity filter, compute
 // ------------------------------------------------------------------------------------------------
-#include "gen/me_tables.h"
 
 namespace {
 
@@ -390,9 +413,9 @@ int me_set_good_helicities(me_handle* h, const uint8_t* mask) {
   return size_cum(h);
 }
 
-int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const double* d_rndhel,
-               const double* d_rndcol, int64_t nevt, double* d_me, int32_t* d_selhel, int32_t* d_selcol,
-               void* stream) {
+static int compute_core(me_handle* h, const double* d_momenta, const double* d_gs, const double* d_rndhel,
+                        const double* d_rndcol, int64_t nevt, double* d_me, int32_t* d_selhel, int32_t* d_selcol,
+                        void* stream, const int32_t* d_channel, const unsigned* d_chanflows, int nchan) {
   int rc = check_inputs(h, d_momenta, d_gs, nevt, "me_compute");
   if (rc) return rc;
   if (!h->have_good) return fail(h, ME_ERR_NO_HELICITIES, "me_compute: call me_filter_helicities or me_set_good_helicities first");
@@ -409,6 +432,7 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
   a.mom = d_momenta; a.gs = d_gs; a.rndhel = d_rndhel; a.rndcol = d_rndcol; a.nevt = nevt;
   a.me = d_me; a.selhel = d_selhel; a.selcol = d_selcol; a.par = h->par; a.good = h->good;
   a.scratch = h->d_scratch; a.scratch_bytes = h->scratch_bytes; a.pipe = h->have_pipe ? &h->pipe : nullptr;
+  a.channel = d_channel; a.chanflows = d_chanflows; a.nchan = nchan;
   a.good.mask[0] = a.good.mask[1] = 0ull;
   for (int i = 0; i < a.good.n; i++) a.good.mask[a.good.h[i] >> 6] |= 1ull << (a.good.h[i] & 63);
   const int mode = (d_selhel || d_selcol) ? me::MODE_SELECT : me::MODE_ME;
@@ -427,6 +451,55 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
   if (ce) return cuda_fail(h, (cudaError_t)ce, "me_compute: launch");
   h->last = info;
   return ME_OK;
+}
+
+int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const double* d_rndhel,
+               const double* d_rndcol, int64_t nevt, double* d_me, int32_t* d_selhel, int32_t* d_selcol,
+               void* stream) {
+  return compute_core(h, d_momenta, d_gs, d_rndhel, d_rndcol, nevt, d_me, d_selhel, d_selcol, stream, nullptr, nullptr, 0);
+}
+
+int me_compute_multichannel(me_handle* h, const double* d_momenta, const double* d_gs, const double* d_rndhel,
+                            const double* d_rndcol, const int32_t* d_channel, int64_t nevt, double* d_me,
+                            int32_t* d_selhel, int32_t* d_selcol, double* d_num, double* d_den, void* stream) {
+  if (!h) return ME_ERR_ARG;
+  if (!h->proc->diag) return fail(h, ME_ERR_PROCESS, "me_compute_multichannel: no channels for this process");
+  if (nevt > 0 && (!d_channel || !d_num || !d_den)) return fail(h, ME_ERR_ARG, "me_compute_multichannel: null channel / num / den pointer");
+  if (misaligned(d_channel, 4) || misaligned(d_num, 8) || misaligned(d_den, 8)) return fail(h, ME_ERR_ARG, "me_compute_multichannel: misaligned pointer");
+  DeviceGuard guard(h->device);
+  if (guard.err != cudaSuccess) return cuda_fail(h, guard.err, "me_compute_multichannel");
+  const unsigned* cfl = nullptr;
+  int nchan = 0;
+  int ce = h->proc->chanflows(&cfl, &nchan);
+  if (ce) return cuda_fail(h, (cudaError_t)ce, "me_compute_multichannel: channel table");
+  // the matrix element, with the colour selection restricted to the flows of each event's channel
+  int rc = compute_core(h, d_momenta, d_gs, d_rndhel, d_rndcol, nevt, d_me, d_selhel, d_selcol, stream, d_channel, cfl, nchan);
+  if (rc || nevt == 0) return rc;
+  // the single-diagram-enhancement weights: diagram-by-diagram kernel, fp64 whatever the build, in chunks that fit its scratch
+  const size_t per = h->proc->diag_scratch();
+  int64_t chunk = nevt < 65536 ? nevt : 65536;
+  void* p = h->d_mc;
+  rc = ensure(h, &p, &h->mc_bytes, per * (size_t)chunk);
+  h->d_mc = p;
+  if (rc) return rc;
+  me::LaunchArgs a;
+  memset(&a, 0, sizeof(a));
+  a.par = h->par; a.good = h->good;
+  for (int64_t e0 = 0; e0 < nevt; e0 += chunk) {
+    a.nevt = (nevt - e0 < chunk) ? (nevt - e0) : chunk;
+    a.mom = d_momenta + e0 * h->npar * 4; a.gs = d_gs + e0;
+    ce = h->proc->diag(a, d_channel + e0, d_num + e0, d_den + e0, h->d_mc, stream);
+    if (ce) return cuda_fail(h, (cudaError_t)ce, "me_compute_multichannel: launch");
+  }
+  return ME_OK;
+}
+
+int me_channel_table(const me_handle* h, char* out, int cap) {
+  if (!h) return ME_ERR_ARG;
+  const int need = (int)strlen(h->proc->chan_keys) + 1;
+  if (out && cap >= need) memcpy(out, h->proc->chan_keys, (size_t)need);
+  else if (out) return fail(h, ME_ERR_ARG, "me_channel_table: buffer too small");
+  return need;
 }
 
 int me_compute_host(me_handle* h, const double* momenta, const double* gs, const double* rndhel,

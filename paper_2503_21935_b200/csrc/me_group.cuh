@@ -1040,13 +1040,15 @@ __global__ void __launch_bounds__(ColGeom<G, TC>::WARPS * 32) colour_kernel(cons
           if (lane < 4) wcs[4 * i + lane] = (double)w;
         }
         __syncwarp();
+        // multichannel (reading R17): flows the event's channel does not contribute to are not selectable
+        const unsigned* cfl = a.channel ? a.chanflows + 4 * min(max(a.channel[e], 0), a.nchan - 1) : nullptr;
         constexpr int PER = (NCOL + 31) / 32;
         double val[PER];
         bool ok[PER];
 #pragma unroll
         for (int i = 0; i < PER; i++) {
           const int c = lane * PER + i;
-          ok[i] = c < NCOL;
+          ok[i] = c < NCOL && (!cfl || ((cfl[c >> 5] >> (c & 31)) & 1u));
           val[i] = ok[i] ? wcs[c] : 0.0;
         }
         double total;

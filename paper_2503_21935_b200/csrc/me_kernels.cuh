@@ -35,6 +35,9 @@ struct LaunchArgs {
   void* scratch;               // lane-group pipeline: per-event data and jamps between its kernels (owned by the handle)
   size_t scratch_bytes;
   const struct PipeCtx* pipe;  // lane-group pipeline: the handle's internal streams and events (host side only)
+  const int* channel;          // multichannel: [nevt] channel (diagram) of every event, or nullptr
+  int nchan;                   // multichannel: number of channels (channel ids are clamped to 0 .. nchan-1)
+  const unsigned* chanflows;   // multichannel: [nchan][4] bit c set iff colour flow c is allowed for the channel
   DevParams par;
   GoodList good;
 };
@@ -158,17 +161,22 @@ __global__ void __launch_bounds__(NT, MINB) event_kernel(const LaunchArgs a) {
         a.selhel[e] = sel;
       }
       if (a.selcol) {
+        // multichannel (reading R17): flows the event's channel does not contribute to get weight zero
+        const unsigned* cfl = a.channel ? a.chanflows + 4 * min(max(a.channel[e], 0), a.nchan - 1) : nullptr;
+        auto allowed = [&](int c) { return !cfl || ((cfl[c >> 5] >> (c & 31)) & 1u); };
         double tot = 0.0;
 #pragma unroll
-        for (int c = 0; c < P::ncol; c++) tot += (double)wc[c];
+        for (int c = 0; c < P::ncol; c++) tot += allowed(c) ? (double)wc[c] : 0.0;
         const double target = a.rndcol[e] * tot;
         int sel = P::ncol - 1;
         double run = 0.0;
         bool found = false;
 #pragma unroll
         for (int c = 0; c < P::ncol; c++) {
-          run += (double)wc[c];
-          if (!found && target < run) { sel = c; found = true; }
+          if (allowed(c)) {
+            run += (double)wc[c];
+            if (!found) { sel = c; found = target < run; }   // ends on the first hit, else on the last allowed flow
+          }
         }
         a.selcol[e] = sel;
       }

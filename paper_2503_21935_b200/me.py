@@ -19,7 +19,7 @@ PROCESSES = ("ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg")
 
 EXPORTS = ("me_create", "me_destroy", "me_last_error", "me_info", "me_helicity_table", "me_color_table",
            "me_color_matrix", "me_filter_helicities", "me_get_good_helicities", "me_set_good_helicities",
-           "me_compute", "me_compute_host", "me_generate", "me_launch_info", "me_launch_stats", "me_fma_peak")
+           "me_compute", "me_compute_multichannel", "me_channel_table", "me_compute_host", "me_generate", "me_launch_info", "me_launch_stats", "me_fma_peak")
 
 
 class MEError(RuntimeError):
@@ -54,6 +54,8 @@ def load_library(path: str = LIB_PATH):
     L.me_get_good_helicities.argtypes = [vp, ip, vp]
     L.me_set_good_helicities.argtypes = [vp, vp]
     L.me_compute.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, vp, vp]
+    L.me_compute_multichannel.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, vp]
+    L.me_channel_table.argtypes = [vp, ctypes.c_char_p, ctypes.c_int]
     L.me_compute_host.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, vp]
     L.me_generate.argtypes = [vp, ctypes.c_uint64, i64, i64, ctypes.c_double, ctypes.c_double, vp, vp, vp, vp, vp, vp]
     L.me_launch_info.argtypes = [vp, ip, ip, ip, ip]
@@ -189,6 +191,31 @@ class MatrixElement:
                                        nevt, _ptr(out, f64, d), _ptr(selhel, torch.int32, d), _ptr(selcol, torch.int32, d),
                                        ctypes.c_void_p(s.cuda_stream)))
         return out, selhel, selcol
+
+    def compute_multichannel(self, momenta, gs, channel, rndhel=None, rndcol=None, stream=None):
+        """me_compute_multichannel: returns (me, selhel, selcol, num, den); channel: cuda int32 [nevt]."""
+        import torch
+        nevt = momenta.shape[0]
+        dev, d = momenta.device, self.device
+        f64 = torch.float64
+        out, num, den = (torch.empty(nevt, dtype=f64, device=dev) for _ in range(3))
+        selhel = torch.empty(nevt, dtype=torch.int32, device=dev) if rndhel is not None else None
+        selcol = torch.empty(nevt, dtype=torch.int32, device=dev) if rndcol is not None else None
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        self._same_device(s)
+        self._check(self._L.me_compute_multichannel(
+            self._h, _ptr(momenta, f64, d), _ptr(gs, f64, d), _ptr(rndhel, f64, d), _ptr(rndcol, f64, d),
+            _ptr(channel, torch.int32, d), nevt, _ptr(out, f64, d), _ptr(selhel, torch.int32, d), _ptr(selcol, torch.int32, d),
+            _ptr(num, f64, d), _ptr(den, f64, d), ctypes.c_void_p(s.cuda_stream)))
+        return out, selhel, selcol, num, den
+
+    def channel_table(self) -> list:
+        n = self._L.me_channel_table(self._h, None, 0)
+        if n < 0:
+            self._check(n)
+        buf = ctypes.create_string_buffer(n)
+        self._check(min(0, self._L.me_channel_table(self._h, buf, n)))
+        return buf.value.decode().split("\n")[:-1]
 
     def compute_host(self, momenta, gs=None, rndhel=None, rndcol=None, out=None, selhel=None, selcol=None):
         """Host buffers in, host buffers out (numpy arrays or pinned CPU tensors viewed as numpy); synchronous."""
