@@ -95,8 +95,10 @@ def test_generated_sources_are_deterministic(tmp_path):
     from paper_2503_21935_b200.codegen.generate import generate_all
     a = generate_all(str(tmp_path / "a"), only=["gg_ttg"])
     b = generate_all(str(tmp_path / "b"), only=["gg_ttg"])
-    assert open(a[0]).read() == open(b[0]).read()
-    txt = open(a[0]).read()
+    assert [os.path.basename(x) for x in a] == [os.path.basename(x) for x in b]
+    for x, y in zip(a, b):
+        assert open(x).read() == open(y).read()
+    txt = open([x for x in a if os.path.basename(x) == "proc_gg_ttg.cuh"][0]).read()
     assert "vvv_current" in txt and "vvvv_currents" in txt and "row_prop" in txt and txt.count("J[") == 6
 
 
@@ -182,3 +184,20 @@ def test_group_layout_tables_are_consistent():
         assert sorted(leaves) == list(range(len(g.flows)))
         fl = g.flops()
         assert fl["per_gluon_combination"] == fl["tree"] + fl["walk"] + fl["colour"]
+
+
+def test_diagram_tables_cover_every_channel_and_flow():
+    """codegen/emit_diag.py (multichannel tables): one channel per Feynman diagram, every closure has a channel, every
+    colour flow is reached by some diagram, and the sizes are those of the diagram counts 3 / 16 / 123 / 1240."""
+    from paper_2503_21935_b200.codegen import diagrams, emit_diag
+    for name, ngl, ndiag in (("gg_tt", 2, 3), ("gg_ttg", 3, 16), ("gg_ttgg", 4, 123)):
+        st = diagrams.build(ngl)
+        dg = emit_diag.Diagrams(name, st)
+        assert len(dg.keys) == ndiag == st.ndiag and dg.keys == sorted(set(dg.keys))
+        assert {dg.chan[c[2]] for c in dg.closures} == set(range(ndiag))
+        reached = [any(row[c] for row in dg.allowed) for c in range(len(st.flows))]
+        assert all(reached)
+        # a diagram made of single gluons on the quark line feeds exactly one flow (the order of attachment)
+        for k, row in zip(dg.keys, dg.allowed):
+            if "(" not in k and "[" not in k:
+                assert sum(row) == 1 and st.flows[row.index(1)] == tuple(int(x) for x in k.split("|"))
