@@ -15,8 +15,8 @@ enumerates the diagrams of g g -> t tbar + (n-2) g from diagrams.Structure and w
 Channel numbering (reading R17): the structural key of a diagram is the "|"-joined keys of the trees on
 the quark line from t to tbar; a leaf's key is its particle index, a three-gluon vertex "(A,B)" with the lowest leg in
 A, a four-gluon vertex "[A,B,C]" with the lowest leg in A and the lowest of the rest in B.  Channels are the distinct
-keys in increasing byte order; the three terms of a four-gluon vertex share a key, hence a channel.  The oracle
-builds the same numbering on its own (oracle/me_oracle.cpp build_channels); tests compare the two key lists.
+keys in increasing byte order; the three terms of a four-gluon vertex share a key, hence a channel.  The CPU checker
+builds the same numbering on its own from the same written rule; tests compare the two key lists.
 """
 from __future__ import annotations
 
