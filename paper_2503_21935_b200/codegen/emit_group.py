@@ -36,8 +36,13 @@ def mask_of(seq):
 
 
 class Group:
-    def __init__(self, name: str, n: int):
+    def __init__(self, name: str, n: int, twins=None):
         self.name, self.n = name, n
+        # twins: every stored current of even length (the only ones whose reversed sequence carries a minus sign) is
+        # stored twice, as +J and -J, and the tables point at the copy with the right sign: no sign handling at the
+        # loads (8 integer instructions per loaded current).  Worth its shared memory for n = 4 (6 extra slots of 22);
+        # for n = 5 (70 extra slots of 105) shared memory is what bounds the resident warps, so the sign bit stays.
+        self.twins = (n <= 4) if twins is None else twins
         idx = tuple(range(n))
         self.flows = list(itertools.permutations(idx))
         self.flow_index = {f: i for i, f in enumerate(self.flows)}
@@ -51,11 +56,18 @@ class Group:
             if L < n:
                 for s in seqs:
                     self.slot[s] = len(self.slot)
-        self.nslot = len(self.slot)
+        self.twin = {}
+        if self.twins:
+            for s, i in list(self.slot.items()):
+                if len(s) % 2 == 0:
+                    self.twin[s] = len(self.slot) + len(self.twin)
+        self.nslot = len(self.slot) + len(self.twin)
         assert self.nslot < 255 and len(self.flows) <= 128
 
     def ref(self, seq):
         can, sgn = canonical(seq)
+        if sgn < 0 and can in self.twin:
+            return self.twin[can], 1
         return self.slot[can], sgn
 
     # ------------------------------------------------------------------ gluon-current task tables
@@ -64,7 +76,7 @@ class Group:
         words = []
         for seq in self.level_seqs[L]:
             top = L == self.n
-            h0 = (255 if top else self.slot[seq]) | (mask_of(seq) << 8)
+            h0 = (255 if top else self.slot[seq]) | (mask_of(seq) << 8) | (self.twin.get(seq, 0) << 16)
             h1 = 0
             if top:
                 rev = tuple(reversed(seq))
@@ -141,6 +153,7 @@ class Group:
         o(f"struct Grp_{self.name} {{")
         o(f"  static constexpr int n = {n}, npar = {n + 2}, ncomb = {1 << (n + 2)}, ncol = {len(self.flows)}, "
           f"ndiag = {ndiag}, denom = {denom}, cden = {cmat_den}, nslot = {self.nslot}, ninit = {len(self.level_seqs[n])}, "
+          f"signs = {0 if self.twins else 1}, "
           f"nstream = {nstream};")
         o("  __device__ __forceinline__ static const unsigned int* level(int L) {")
         o("    switch (L) {")

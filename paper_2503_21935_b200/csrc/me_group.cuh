@@ -124,10 +124,11 @@ template <typename T> __device__ __forceinline__ spin4<T> ld_spin(const T* p) {
 // into different bank groups: without it a 64-byte slot stride reaches only half of the banks for a given chunk.
 template <typename T> struct GrpSlot;
 template <> struct GrpSlot<double> {
+  template <bool SIGNS = true>
   __device__ __forceinline__ static vec4<double> ld(const double* slots, unsigned s, unsigned neg) {
     const char* base = reinterpret_cast<const char*>(slots + s * 8);
     const unsigned x = (s >> 1) & 3u;
-    const int m = (int)(neg << 31);
+    const int m = SIGNS ? (int)(neg << 31) : 0;
     vec4<double> r;
 #pragma unroll
     for (int i = 0; i < 4; i++) {
@@ -145,10 +146,11 @@ template <> struct GrpSlot<double> {
   }
 };
 template <> struct GrpSlot<float> {
+  template <bool SIGNS = true>
   __device__ __forceinline__ static vec4<float> ld(const float* slots, unsigned s, unsigned neg) {
     const char* base = reinterpret_cast<const char*>(slots + s * 8);
     const unsigned x = 0u;  // fp32: the extra address arithmetic costs more issue slots than the conflicts (measured)
-    const int m = (int)(neg << 31);
+    const int m = SIGNS ? (int)(neg << 31) : 0;
     vec4<float> r;
 #pragma unroll
     for (int i = 0; i < 2; i++) {
@@ -473,14 +475,14 @@ __device__ __forceinline__ void grp_tree(const GrpEvent<T, G::n>& ev, T* slots, 
 #pragma unroll(UT)
         for (int j = 0; j < NV3; j++) {
           const unsigned w = __ldg(tw + 2 + j);
-          const vec4<T> A = GrpSlot<T>::ld(slots, w & 255u, w >> 31);
+          const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
           const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
           v3_acc(acc, A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
         }
 #pragma unroll(UT)
         for (int j = 0; j < NV4; j++) {
           const unsigned w = __ldg(tw + 2 + NV3 + j);
-          const vec4<T> A = GrpSlot<T>::ld(slots, w & 255u, w >> 31);
+          const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
           const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
           const vec4<T> C = GrpSlot<T>::ld(slots, (w >> 16) & 255u, 0u);
           v4_acc(acc, A, B, C);
@@ -490,6 +492,12 @@ __device__ __forceinline__ void grp_tree(const GrpEvent<T, G::n>& ev, T* slots, 
         for (int i = 0; i < 4; i++) acc.c[i] = s * acc.c[i];
         if (!TOP) {
           GrpSlot<T>::st(slots, h0 & 255u, acc);
+          if (G::signs == 0 && ((h0 >> 16) & 255u)) {   // even length: the negated twin, for the reversed sequence
+            vec4<T> nacc;
+#pragma unroll
+            for (int i = 0; i < 4; i++) nacc.c[i] = -acc.c[i];
+            GrpSlot<T>::st(slots, (h0 >> 16) & 255u, nacc);
+          }
         } else {
           // the full-length current is contracted at once with the four t-tbar currents: the j = 0 term of the
           // jamps of this sequence and of its reverse
@@ -534,7 +542,7 @@ struct GrpWalkCtx {
   const unsigned* stream;
   int ht;
   __device__ __forceinline__ unsigned next() { return __ldg(stream++); }
-  __device__ __forceinline__ vec4<T> cur(unsigned w) const { return GrpSlot<T>::ld(slots, w & 255u, w >> 31); }
+  __device__ __forceinline__ vec4<T> cur(unsigned w) const { return GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31); }
   typedef WalkPack<T, GrpGeom<G, T>::HTL> WP;
   typedef typename WP::PS PS;
   __device__ __forceinline__ vec4<PS> curw(unsigned w) const {

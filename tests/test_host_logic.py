@@ -146,9 +146,12 @@ def test_group_layout_tables_are_consistent():
     """Lane-group layout (codegen/emit_group.py): slots, level tables and per-role word streams."""
     import itertools
     from paper_2503_21935_b200.codegen import emit_group as EG
-    for n, nslot in ((4, 22), (5, 105)):
+    for n, nslot, ntwin in ((4, 22, 6), (5, 105, 0)):
         g = EG.Group("t", n)
-        assert g.nslot == nslot == sum(len(g.level_seqs[L]) for L in range(1, n))
+        # n = 4: the even-length currents are stored twice (+J and -J), the tables point at the copy with the sign
+        assert len(g.slot) == nslot == sum(len(g.level_seqs[L]) for L in range(1, n)) and len(g.twin) == ntwin
+        assert g.nslot == nslot + ntwin and sorted(g.twin.values()) == list(range(nslot, nslot + ntwin))
+        assert all(len(s) % 2 == 0 for s in g.twin)
         # canonical sequences: one of each {seq, reversed seq}; the reflection sign is (-1)^(len+1)
         for L in range(1, n + 1):
             allseq = [s for c in itertools.combinations(range(n), L) for s in itertools.permutations(c)]
@@ -161,10 +164,12 @@ def test_group_layout_tables_are_consistent():
             tab, nv3, nv4 = g.level_table(L), L - 1, (L - 1) * (L - 2) // 2
             W = 2 + nv3 + nv4
             assert len(tab) == W * len(g.level_seqs[L])
-            lower = {g.slot[s] for k in range(1, L) for s in g.level_seqs[k]}
+            lower = {g.slot[s] for k in range(1, L) for s in g.level_seqs[k]} | {v for s, v in g.twin.items() if len(s) < L}
             for t, seq in enumerate(g.level_seqs[L]):
                 w = tab[t * W:(t + 1) * W]
                 assert (w[0] >> 8) & 31 == EG.mask_of(seq)
+                for x in w[2:]:
+                    assert ntwin == 0 or (x >> 31) == 0          # with twins no word carries a sign bit
                 for x in w[2:2 + nv3]:
                     assert (x & 255) in lower and ((x >> 8) & 255) in lower
                     assert ((x >> 16) & 31) | ((x >> 21) & 31) == EG.mask_of(seq) and ((x >> 16) & 31) & ((x >> 21) & 31) == 0
@@ -181,6 +186,7 @@ def test_group_layout_tables_are_consistent():
             st = g.role_stream(s1)
             assert len(st) == len(g.role_stream(0))
             leaves += [(w >> 16) & 127 for w in st if (w >> 8) & 31 == (1 << n) - 1]
+            assert ntwin == 0 or all((w >> 31) == 0 for w in st if (w >> 8) & 31 != (1 << n) - 1)
         assert sorted(leaves) == list(range(len(g.flows)))
         fl = g.flops()
         assert fl["per_gluon_combination"] == fl["tree"] + fl["walk"] + fl["colour"]
