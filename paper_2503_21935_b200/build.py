@@ -31,6 +31,14 @@ TUNE = {
     ("gg_ttgg", 0): (32, 8), ("gg_ttgg", 1): (32, 16), ("gg_ttgg", 2): (32, 8),
 }
 DEFAULT_TUNE = (128, 1)
+# extra nvcc flags for experiments, e.g. ME_B200_NVCC_FLAGS="-DME_UNROLL_T=2" (part of the units' hashes)
+# for the units whose name starts with one of ME_B200_NVCC_UNITS (comma separated; default: all)
+EXTRA = os.environ.get("ME_B200_NVCC_FLAGS", "").split()
+EXTRA_UNITS = [u for u in os.environ.get("ME_B200_NVCC_UNITS", "").split(",") if u]
+
+
+def _extra(name):
+    return EXTRA if (not EXTRA_UNITS or any(name.startswith(u) for u in EXTRA_UNITS)) else []
 
 
 def _units():
@@ -49,7 +57,7 @@ def _units():
     yield "rambo", os.path.join(CSRC, "me_rambo.cu"), []
 
 
-def _deps_hash(defs):
+def _deps_hash(defs, extra=()):
     h = hashlib.sha256()
     for root, _, files in sorted(os.walk(CSRC)):
         for f in sorted(files):
@@ -66,7 +74,7 @@ def _deps_hash(defs):
                     h.update(f.encode() + fh.read())
     with open(os.path.join(os.path.dirname(HERE), "include", "me_b200.h"), "rb") as fh:
         h.update(fh.read())
-    h.update(" ".join(NVCC_BASE + defs).encode())
+    h.update(" ".join(NVCC_BASE + defs + list(extra)).encode())
     return h.hexdigest()
 
 
@@ -74,10 +82,10 @@ def _compile(unit, force, verbose):
     name, src, defs = unit
     obj = os.path.join(OBJ, name + ".o")
     stamp = obj + ".hash"
-    want = _deps_hash(defs)
+    want = _deps_hash(defs, _extra(name))
     if not force and os.path.exists(obj) and os.path.exists(stamp) and open(stamp).read() == want:
         return name, "cached", ""
-    cmd = NVCC_BASE + defs + ["-c", src, "-o", obj]
+    cmd = NVCC_BASE + defs + _extra(name) + ["-c", src, "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     log = r.stdout + r.stderr
     with open(os.path.join(OBJ, name + ".ptxas.txt"), "w") as f:

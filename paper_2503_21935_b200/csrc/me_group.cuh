@@ -456,79 +456,111 @@ template <class G, typename T, typename TC> struct GrpWalkCtx;
 // Colour-ordered gluon currents of one group, level by level (|seq| = 2 .. n).  One copy of the vertex code: the
 // levels, the tasks of a level and the terms of a task are run-time loops over the generated tables (keeps the
 // kernel small enough for the instruction cache; the loop bodies are ~100 FMA-pipe instructions each).
-template <class G, typename T, typename TC>
-__device__ __forceinline__ void grp_tree(const GrpEvent<T, G::n>& ev, T* slots, TC* X, int r, bool active) {
+template <class G, typename T, typename TC, int LS>
+__device__ __forceinline__ void grp_tree_level(const GrpEvent<T, G::n>& ev, T* slots, TC* X, int r, bool active, int Lrt) {
+  // LS > 0: the level is a compile-time constant and the term loops are unrolled (straight-line task body: the
+  // loads of later terms move above the arithmetic of earlier ones); LS == 0: run-time level Lrt, one copy of the code
   constexpr int LPG = GrpGeom<G, T>::LPG, UT = ME_UNROLL_T;
+  const int L = LS ? LS : Lrt;
+  const int NV3 = L - 1, NV4 = (L - 1) * (L - 2) / 2, W = 2 + NV3 + NV4;
+  const bool TOP = (L == G::n);
+  const unsigned* tab = G::level(L);
+  const int nt = G::ntask(L);
 #pragma unroll 1
-  for (int L = 2; L <= G::n; L++) {
-    const int NV3 = L - 1, NV4 = (L - 1) * (L - 2) / 2, W = 2 + NV3 + NV4;
-    const bool TOP = (L == G::n);
-    const unsigned* tab = G::level(L);
-    const int nt = G::ntask(L);
-#pragma unroll 1
-    for (int t0 = 0; t0 < nt; t0 += LPG) {
-      const int t = t0 + r;
-      if (active && t < nt) {
-        const unsigned* tw = tab + t * W;
-        const unsigned h0 = __ldg(tw);
-        vec4<T> acc = zero_vec4<T>();
-#pragma unroll(UT)
-        for (int j = 0; j < NV3; j++) {
-          const unsigned w = __ldg(tw + 2 + j);
-          const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
-          const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
-          v3_acc(acc, A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
-        }
-#pragma unroll(UT)
-        for (int j = 0; j < NV4; j++) {
-          const unsigned w = __ldg(tw + 2 + NV3 + j);
-          const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
-          const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
-          const vec4<T> C = GrpSlot<T>::ld(slots, (w >> 16) & 255u, 0u);
-          v4_acc(acc, A, B, C);
-        }
-        const T s = ev.ik[(h0 >> 8) & 31u];
+  for (int t0 = 0; t0 < nt; t0 += LPG) {
+    const int t = t0 + r;
+    if (active && t < nt) {
+      const unsigned* tw = tab + t * W;
+      const unsigned h0 = __ldg(tw);
+      vec4<T> acc = zero_vec4<T>();
+      auto term3 = [&](int j) {
+        const unsigned w = __ldg(tw + 2 + j);
+        const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
+        const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
+        v3_acc(acc, A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
+      };
+      auto term4 = [&](int j) {
+        const unsigned w = __ldg(tw + 2 + NV3 + j);
+        const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
+        const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
+        const vec4<T> C = GrpSlot<T>::ld(slots, (w >> 16) & 255u, 0u);
+        v4_acc(acc, A, B, C);
+      };
+      if constexpr (LS > 0) {
 #pragma unroll
-        for (int i = 0; i < 4; i++) acc.c[i] = s * acc.c[i];
-        if (!TOP) {
-          GrpSlot<T>::st(slots, h0 & 255u, acc);
-          if (G::signs == 0 && ((h0 >> 16) & 255u)) {   // even length: the negated twin, for the reversed sequence
-            vec4<T> nacc;
+        for (int j = 0; j < LS - 1; j++) term3(j);
 #pragma unroll
-            for (int i = 0; i < 4; i++) nacc.c[i] = -acc.c[i];
-            GrpSlot<T>::st(slots, (h0 >> 16) & 255u, nacc);
+        for (int j = 0; j < (LS - 1) * (LS - 2) / 2; j++) term4(j);
+      } else {
+#pragma unroll(UT)
+        for (int j = 0; j < NV3; j++) term3(j);
+#pragma unroll(UT)
+        for (int j = 0; j < NV4; j++) term4(j);
+      }
+      const T s = ev.ik[(h0 >> 8) & 31u];
+#pragma unroll
+      for (int i = 0; i < 4; i++) acc.c[i] = s * acc.c[i];
+      if (!TOP) {
+        GrpSlot<T>::st(slots, h0 & 255u, acc);
+        if (G::signs == 0 && ((h0 >> 16) & 255u)) {   // even length: the negated twin, for the reversed sequence
+          vec4<T> nacc;
+#pragma unroll
+          for (int i = 0; i < 4; i++) nacc.c[i] = -acc.c[i];
+          GrpSlot<T>::st(slots, (h0 >> 16) & 255u, nacc);
+        }
+      } else {
+        // the full-length current is contracted at once with the four t-tbar currents: the j = 0 term of the
+        // jamps of this sequence and of its reverse
+        if constexpr (GrpInit<G>::GLOBAL) {
+          // ... parked in the jamp buffer itself (rows of the two flows), where the leaves of the walk pick it
+          // up: it stays in L2 until the leaf overwrites it with the finished jamp
+          const unsigned h1 = __ldg(tw + 1);
+          TC* ja = X + (h1 & 127u) * 8;
+          TC* jb = X + ((h1 >> 8) & 127u) * 8;
+          const T sb = (h1 >> 31) ? T(-1) : T(1);
+#pragma unroll
+          for (int v = 0; v < 4; v++) {
+            const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
+            const cx<T> a = mdot(q, acc);
+            GrpWalkCtx<G, T, TC>::st2(ja + 2 * v, TC(a.re), TC(a.im));
+            GrpWalkCtx<G, T, TC>::st2(jb + 2 * v, TC(sb * a.re), TC(sb * a.im));
           }
         } else {
-          // the full-length current is contracted at once with the four t-tbar currents: the j = 0 term of the
-          // jamps of this sequence and of its reverse
-          if constexpr (GrpInit<G>::GLOBAL) {
-            // ... parked in the jamp buffer itself (rows of the two flows), where the leaves of the walk pick it
-            // up: it stays in L2 until the leaf overwrites it with the finished jamp
-            const unsigned h1 = __ldg(tw + 1);
-            TC* ja = X + (h1 & 127u) * 8;
-            TC* jb = X + ((h1 >> 8) & 127u) * 8;
-            const T sb = (h1 >> 31) ? T(-1) : T(1);
+          // ... in "init" slot t of shared memory, read by the leaves of the walk
+          T* ji = slots + (G::nslot + t) * 8;
 #pragma unroll
-            for (int v = 0; v < 4; v++) {
-              const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
-              const cx<T> a = mdot(q, acc);
-              GrpWalkCtx<G, T, TC>::st2(ja + 2 * v, TC(a.re), TC(a.im));
-              GrpWalkCtx<G, T, TC>::st2(jb + 2 * v, TC(sb * a.re), TC(sb * a.im));
-            }
-          } else {
-            // ... in "init" slot t of shared memory, read by the leaves of the walk
-            T* ji = slots + (G::nslot + t) * 8;
-#pragma unroll
-            for (int v = 0; v < 4; v++) {
-              const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
-              const cx<T> a = mdot(q, acc);
-              ji[2 * v] = a.re; ji[2 * v + 1] = a.im;
-            }
+          for (int v = 0; v < 4; v++) {
+            const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
+            const cx<T> a = mdot(q, acc);
+            ji[2 * v] = a.re; ji[2 * v + 1] = a.im;
           }
         }
       }
     }
-    __syncwarp();
+  }
+  __syncwarp();
+}
+
+template <class G, typename T, typename TC, int LS>
+__device__ __forceinline__ void grp_tree_static(const GrpEvent<T, G::n>& ev, T* slots, TC* X, int r, bool active) {
+  grp_tree_level<G, T, TC, LS>(ev, slots, X, r, active, LS);
+  if constexpr (LS < G::n) grp_tree_static<G, T, TC, LS + 1>(ev, slots, X, r, active);
+}
+
+template <class G, typename T, typename TC>
+__device__ __forceinline__ void grp_tree(const GrpEvent<T, G::n>& ev, T* slots, TC* X, int r, bool active) {
+  // one copy of the tree code per level with the term loops unrolled (n = 4: +2 % fp64, +5 % fp32, measured), or one
+  // copy for all levels with run-time loops
+#ifdef ME_TREE_STATIC
+  constexpr bool STATIC = (ME_TREE_STATIC != 0);
+#else
+  constexpr bool STATIC = (G::n <= 4);
+#endif
+  if constexpr (STATIC) {
+    grp_tree_static<G, T, TC, 2>(ev, slots, X, r, active);
+  } else {
+#pragma unroll 1
+    for (int L = 2; L <= G::n; L++) grp_tree_level<G, T, TC, 0>(ev, slots, X, r, active, L);
   }
 }
 
@@ -571,6 +603,10 @@ struct GrpWalkCtx {
   // J_flow(h_t, b) = init + a  ->  X[flow][2 (2 h_t + b) + re/im]; stores bypass L1 (the table words live there)
   __device__ __forceinline__ static void st2(double* q, double x, double y) { __stcg(reinterpret_cast<double2*>(q), make_double2(x, y)); }
   __device__ __forceinline__ static void st2(float* q, float x, float y) { __stcg(reinterpret_cast<float2*>(q), make_float2(x, y)); }
+  // finished jamps: read once by the colour kernel, so they leave L2 first (the per-event data of K0 and the parked
+  // full-length currents stay)
+  __device__ __forceinline__ static void stf(double* q, double x, double y) { __stcs(reinterpret_cast<double2*>(q), make_double2(x, y)); }
+  __device__ __forceinline__ static void stf(float* q, float x, float y) { __stcs(reinterpret_cast<float2*>(q), make_float2(x, y)); }
   __device__ __forceinline__ static void ld2(const double* q, double& x, double& y) { const double2 t = __ldcg(reinterpret_cast<const double2*>(q)); x = t.x; y = t.y; }
   __device__ __forceinline__ static void ld2(const float* q, float& x, float& y) { const float2 t = __ldcg(reinterpret_cast<const float2*>(q)); x = t.x; y = t.y; }
   __device__ __forceinline__ void leaf(const spin4<PS> (&Xs)[WP::NCH], unsigned w) const {
@@ -604,13 +640,13 @@ struct GrpWalkCtx {
   }
   // finished jamp(s) of (chain c, b): packed pair = both h_t at once
   __device__ __forceinline__ static void fin(TC* q, const T (&ini)[GrpGeom<G, T>::HTL ? 4 : 2][2], int c, int b, f2 re, f2 im) {
-    st2(q + 2 * b, TC(ini[b][0] + re.v.x), TC(ini[b][1] + im.v.x));                  // h_t = 0: v = b
-    st2(q + 4 + 2 * b, TC(ini[2 + b][0] + re.v.y), TC(ini[2 + b][1] + im.v.y));      // h_t = 1: v = 2 + b
+    stf(q + 2 * b, TC(ini[b][0] + re.v.x), TC(ini[b][1] + im.v.x));                  // h_t = 0: v = b
+    stf(q + 4 + 2 * b, TC(ini[2 + b][0] + re.v.y), TC(ini[2 + b][1] + im.v.y));      // h_t = 1: v = 2 + b
   }
   template <typename S>
   __device__ __forceinline__ static void fin(TC* q, const T (&ini)[GrpGeom<G, T>::HTL ? 4 : 2][2], int c, int b, S re, S im) {
     const int k = 2 * c + b;   // HTL: c = h_t; otherwise c = 0 and q already points at the lane's h_t
-    st2(q + 2 * k, TC(ini[k][0] + re), TC(ini[k][1] + im));
+    stf(q + 2 * k, TC(ini[k][0] + re), TC(ini[k][1] + im));
   }
 };
 
@@ -696,10 +732,14 @@ __global__ void __launch_bounds__(32, MINB) amp_kernel(const PipeArgs p) {
     const int unit = (int)(blockIdx.x - e * nunit);
     {
       // ---- a1: the event's helicity-independent data (K0), HBM -> shared memory past L1 (the table words live there)
-      const int4* src = reinterpret_cast<const int4*>(reinterpret_cast<const EV*>(p.ev) + e);
-      int4* dst = reinterpret_cast<int4*>(&ev);
-#pragma unroll 4
-      for (int i = lane; i < (int)(sizeof(EV) / 16); i += 32) dst[i] = __ldcg(src + i);
+      // (asynchronous 16-byte copies, all in flight at once: one round trip to L2 / HBM instead of one per loop pass)
+      const char* src = reinterpret_cast<const char*>(reinterpret_cast<const EV*>(p.ev) + e);
+      const unsigned dst = (unsigned)__cvta_generic_to_shared(&ev);
+      static_assert(sizeof(EV) % 16 == 0, "GrpEvent is copied in 16-byte pieces");
+#pragma unroll
+      for (int i = lane; i < (int)(sizeof(EV) / 16); i += 32)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * (unsigned)i), "l"(src + 16 * i) : "memory");
+      asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
     }
     __syncwarp();
     const int ci = unit * GPW + gi;                       // position in the list of combinations
@@ -808,7 +848,7 @@ template <int NCOL> struct ColFrag<NCOL, double> {
   __device__ __forceinline__ void load(const double* X, int lane) {
     const double* p = X + (lane & 3) * 8 + (lane >> 2);
 #pragma unroll
-    for (int i = 0; i < NW; i++) a[i] = __ldcg(p + 32 * i);
+    for (int i = 0; i < NW; i++) a[i] = __ldcs(p + 32 * i);
   }
   // cf: [pair(I,J)][k-step s][lane]: B[k = lane % 4][n = lane / 4] = C'[8 I + 4 s + k][8 J + perm(n)]
   // returns the thread's part of q_m (m = lane / 4); the quad sum and the re + im sum are the caller's
@@ -857,8 +897,8 @@ template <int NCOL> struct ColFrag<NCOL, float> {
     const float* p = X + (g >> 2) * (NCOL * 8) + (lane & 3) * 8 + 2 * (g & 3);
 #pragma unroll
     for (int I = 0; I < NT; I++) {
-      const float2 u = __ldcg(reinterpret_cast<const float2*>(p + 64 * I));
-      const float2 w = __ldcg(reinterpret_cast<const float2*>(p + 64 * I + 32));
+      const float2 u = __ldcs(reinterpret_cast<const float2*>(p + 64 * I));
+      const float2 w = __ldcs(reinterpret_cast<const float2*>(p + 64 * I + 32));
       x[I][0] = u.x; x[I][1] = u.y; x[I][2] = w.x; x[I][3] = w.y;
     }
   }

@@ -106,7 +106,9 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
   // shared memory: what ME_MINB amplitude warps need and no more (the rest of the 256 KB stays L1 for the table words)
   int carve = (int)((size_t)ME_MINB * (GE::SMEM + 1024) * 100 / (228 * 1024)) + 1;
   if (carve > 100) carve = 100;
-  err = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, GE::SMEM);
+  int k1_smem = GE::SMEM;
+  if (const char* pad = getenv("ME_B200_AMP_PAD_KB")) { k1_smem += atoi(pad) * 1024; carve = 100; }   // experiments: fewer resident warps
+  err = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, k1_smem);
   if (err == cudaSuccess) err = cudaFuncSetAttribute(k1, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
   if (err == cudaSuccess) err = cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, CG::SMEM);
   int k2_per_sm = 1;
@@ -162,7 +164,7 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     cudaStream_t s1 = px ? (hf ? px->sb : px->sa) : st, s2 = px ? px->s2 : st;
     if (px && c >= NPART && (err = cudaStreamWaitEvent(s1, px->k2[part], 0)) != cudaSuccess) return (int)err;  // part free again
     k0<<<(unsigned)((n * PT + 127) / 128), 128, 0, s1>>>(p.a, (EV*)p.ev);
-    k1<<<(unsigned)(n * nunit), 32, GE::SMEM, s1>>>(p);
+    k1<<<(unsigned)(n * nunit), 32, k1_smem, s1>>>(p);
     if (px) {
       if ((err = cudaEventRecord(px->k1[hf], s1)) != cudaSuccess) return (int)err;
       if ((err = cudaStreamWaitEvent(s2, px->k1[hf], 0)) != cudaSuccess) return (int)err;
