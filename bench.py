@@ -226,7 +226,7 @@ def main():
     import torch
     import torch.distributed as dist
 
-    from paper_2503_21935_b200.me import MatrixElement, fma_peak
+    from paper_2503_21935_b200.me import MatrixElement, fma_peak, mma_peak
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -325,6 +325,10 @@ def main():
             "traffic_source": tr_src,
             "traffic_note": "DRAM bytes of the amplitude kernel per step, scaled per event from the ncu capture named in "
                             "traffic_source; the path is FMA-bound, not HBM-bound",
+            "tensor_peaks": ({"dmma_m8n8k4_f64": mma_peak("dmma", local), "tf32_m16n8k8": mma_peak("tf32", local),
+                              "note": "me_mma_peak, measured in this run; the colour contraction (K2) uses DMMA in the fp64 build "
+                                      "(same FP64 units as DFMA: fewer issue slots, no extra throughput) and 2xTF32 in fp32/mixed"}
+                             if process in GROUP else None),
             "frac_per_helicity_accounting": (PER_HELICITY_ACCOUNTING[process] * nevt / (step_ms * 1e-3) * 1e-12 / peak
                                              if process in PER_HELICITY_ACCOUNTING and not on_tensor else None),
         }

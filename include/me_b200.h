@@ -148,6 +148,13 @@ int me_launch_stats(const me_handle* h, int* launches, int64_t* chunk_events, in
  * FMA = 2 FLOP.  This is the denominator of the roofline fractions. */
 int me_fma_peak(int precision, int device, double* tflops);
 
+/* Measured peak of the tensor-core instructions the colour contraction uses (same kind of microbenchmark):
+ * kind 0 = mma.sync m8n8k4 f64 (DMMA: on B200 it runs on the FP64 units, so it buys no throughput over DFMA, only
+ * issue slots), kind 1 = mma.sync m16n8k8 tf32 with fp32 accumulation (a pipe of its own).  *tflops: 2 m n k FLOP
+ * per warp-wide MMA.  Context for the roofline of bench.py (north_star (d): tensor cores "only where it
+ * genuinely batches"). */
+int me_mma_peak(int kind, int device, double* tflops);
+
 #ifdef __cplusplus
 }
 #endif

@@ -40,6 +40,17 @@
 #define ME_UNROLL_T 1   // unroll factor of the term loops of the tree (loads of term j + 1 overlap the arithmetic of term j)
 #endif
 
+// -DME_CHECK=1: the build of the self-checks (compute-sanitizer is not available on the pool):
+// every slot index read from a table is bounds-checked, the shared memory of a warp and the pipeline scratch of a
+// chunk are filled with NaN before use, so that a read of anything not written in this unit / chunk shows up as a
+// NaN matrix element in the parity tests
+#if defined(ME_CHECK) && ME_CHECK
+#include <cassert>
+#define ME_ASSERT(x) assert(x)
+#else
+#define ME_ASSERT(x) ((void)0)
+#endif
+
 namespace me {
 
 // Packed pair of floats: lane-local SIMD over the two t helicities of the quark-line walk in the fp32 build
@@ -475,12 +486,14 @@ __device__ __forceinline__ void grp_tree_level(const GrpEvent<T, G::n>& ev, T* s
       vec4<T> acc = zero_vec4<T>();
       auto term3 = [&](int j) {
         const unsigned w = __ldg(tw + 2 + j);
+        ME_ASSERT((w & 255u) < (unsigned)G::nslot && ((w >> 8) & 255u) < (unsigned)G::nslot);
         const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
         const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
         v3_acc(acc, A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
       };
       auto term4 = [&](int j) {
         const unsigned w = __ldg(tw + 2 + NV3 + j);
+        ME_ASSERT((w & 255u) < (unsigned)G::nslot && ((w >> 8) & 255u) < (unsigned)G::nslot && ((w >> 16) & 255u) < (unsigned)G::nslot);
         const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
         const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
         const vec4<T> C = GrpSlot<T>::ld(slots, (w >> 16) & 255u, 0u);
@@ -501,6 +514,7 @@ __device__ __forceinline__ void grp_tree_level(const GrpEvent<T, G::n>& ev, T* s
 #pragma unroll
       for (int i = 0; i < 4; i++) acc.c[i] = s * acc.c[i];
       if (!TOP) {
+        ME_ASSERT((h0 & 255u) < (unsigned)G::nslot && ((h0 >> 16) & 255u) < (unsigned)G::nslot);
         GrpSlot<T>::st(slots, h0 & 255u, acc);
         if (G::signs == 0 && ((h0 >> 16) & 255u)) {   // even length: the negated twin, for the reversed sequence
           vec4<T> nacc;
@@ -574,7 +588,7 @@ struct GrpWalkCtx {
   const unsigned* stream;
   int ht;
   __device__ __forceinline__ unsigned next() { return __ldg(stream++); }
-  __device__ __forceinline__ vec4<T> cur(unsigned w) const { return GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31); }
+  __device__ __forceinline__ vec4<T> cur(unsigned w) const { ME_ASSERT((w & 255u) < (unsigned)G::nslot); return GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31); }
   typedef WalkPack<T, GrpGeom<G, T>::HTL> WP;
   typedef typename WP::PS PS;
   __device__ __forceinline__ vec4<PS> curw(unsigned w) const {
@@ -613,6 +627,7 @@ struct GrpWalkCtx {
     constexpr bool HTL = GrpGeom<G, T>::HTL;
     constexpr int NV = HTL ? 4 : 2;          // (h_t, b) values this lane completes: v = v0 + k
     const int f = (w >> 16) & 127;
+    ME_ASSERT(f < G::ncol);
     const int v0 = HTL ? 0 : 2 * ht;
     TC* q = X + f * 8 + 2 * v0;
     T ini[NV][2];
@@ -620,6 +635,7 @@ struct GrpWalkCtx {
 #pragma unroll
       for (int k = 0; k < NV; k++) { TC x, y; ld2(q + 2 * k, x, y); ini[k][0] = T(x); ini[k][1] = T(y); }
     } else {
+      ME_ASSERT((w & 255u) >= (unsigned)G::nslot && (w & 255u) < (unsigned)(G::nslot + G::ninit));
       const T* ji = slots + (w & 255u) * 8 + 2 * v0;
       const T sg = (w >> 31) ? T(-1) : T(1);
 #pragma unroll
@@ -725,6 +741,10 @@ __global__ void __launch_bounds__(32, MINB) amp_kernel(const PipeArgs p) {
   const int gi = lane / LPG, r = lane - gi * LPG;
   const int nunit = (p.ncombo + GPW - 1) / GPW;
   T* slots = gbase + (size_t)((gi < GPW) ? gi : 0) * GE::GS;
+#if defined(ME_CHECK) && ME_CHECK
+  for (int i = lane; i < GPW * GE::GS; i += 32) gbase[i] = T(__longlong_as_double(0x7ff8000000000000ll));
+  __syncwarp();
+#endif
   // One warp per (event, unit).  (Persistent warps over a range of units measured 0-12 % slower: warps that start at
   // different times mix their tree and walk phases on the FP64 pipe, persistent ones run them in step.)
   {

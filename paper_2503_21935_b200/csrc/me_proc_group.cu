@@ -163,6 +163,10 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     constexpr int PT = ((1 << N) + N + 6 <= 32) ? 32 : 64;
     cudaStream_t s1 = px ? (hf ? px->sb : px->sa) : st, s2 = px ? px->s2 : st;
     if (px && c >= NPART && (err = cudaStreamWaitEvent(s1, px->k2[part], 0)) != cudaSuccess) return (int)err;  // part free again
+#if defined(ME_CHECK) && ME_CHECK
+    // self-check build: the part of the scratch this chunk uses starts as NaN
+    if ((err = cudaMemsetAsync(base, 0xff, align_up((size_t)n * evb, 256) + (size_t)n * p.ncombo * grpb + slack, s1)) != cudaSuccess) return (int)err;
+#endif
     k0<<<(unsigned)((n * PT + 127) / 128), 128, 0, s1>>>(p.a, (EV*)p.ev);
     k1<<<(unsigned)(n * nunit), 32, k1_smem, s1>>>(p);
     if (px) {

@@ -19,7 +19,7 @@ PROCESSES = ("ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg")
 
 EXPORTS = ("me_create", "me_destroy", "me_last_error", "me_info", "me_helicity_table", "me_color_table",
            "me_color_matrix", "me_filter_helicities", "me_get_good_helicities", "me_set_good_helicities",
-           "me_compute", "me_compute_multichannel", "me_channel_table", "me_compute_host", "me_generate", "me_launch_info", "me_launch_stats", "me_fma_peak")
+           "me_compute", "me_compute_multichannel", "me_channel_table", "me_compute_host", "me_generate", "me_launch_info", "me_launch_stats", "me_fma_peak", "me_mma_peak")
 
 
 class MEError(RuntimeError):
@@ -61,6 +61,7 @@ def load_library(path: str = LIB_PATH):
     L.me_launch_info.argtypes = [vp, ip, ip, ip, ip]
     L.me_launch_stats.argtypes = [vp, ip, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
     L.me_fma_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+    L.me_mma_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
     for n in EXPORTS:
         if n != "me_last_error":
             getattr(L, n).restype = ctypes.c_int
@@ -265,6 +266,15 @@ def fma_peak(precision: str = "fp64", device: int = 0) -> float:
     rc = load_library().me_fma_peak(PRECISIONS[precision], device, ctypes.byref(v))
     if rc != 0:
         raise MEError(f"me_fma_peak failed ({rc})")
+    return v.value
+
+
+def mma_peak(kind: str = "dmma", device: int = 0) -> float:
+    """Measured tensor-pipe peak in TFLOP/s (me_mma_peak): kind "dmma" (m8n8k4 f64) or "tf32" (m16n8k8)."""
+    v = ctypes.c_double()
+    rc = load_library().me_mma_peak({"dmma": 0, "tf32": 1}[kind], device, ctypes.byref(v))
+    if rc != 0:
+        raise MEError(f"me_mma_peak failed ({rc})")
     return v.value
 
 

@@ -175,6 +175,18 @@ def test_group_layout_tables_are_consistent():
                     assert ((x >> 16) & 31) | ((x >> 21) & 31) == EG.mask_of(seq) and ((x >> 16) & 31) & ((x >> 21) & 31) == 0
                 for x in w[2 + nv3:]:
                     assert {x & 255, (x >> 8) & 255, (x >> 16) & 255} <= lower
+        # race freedom of the warp-synchronous tree: the leaves occupy slots 0..n-1 (lane i writes slot i), every other
+        # slot (and twin) has exactly ONE writing task, and (checked above) every reader sits at a higher level, i.e.
+        # behind the __syncwarp() that closes the writer's level
+        assert [g.slot[(i,)] for i in range(n)] == list(range(n))
+        writers = list(range(n))
+        for L in range(2, n):
+            tab, W = g.level_table(L), 2 + (L - 1) + (L - 1) * (L - 2) // 2
+            for t in range(len(g.level_seqs[L])):
+                writers.append(tab[t * W] & 255)
+                if (tab[t * W] >> 16) & 255:
+                    writers.append((tab[t * W] >> 16) & 255)
+        assert sorted(writers) == list(range(g.nslot))
         # top level: every flow is initialised exactly once (as a canonical sequence or as its reverse)
         W = 2 + (n - 1) + (n - 1) * (n - 2) // 2
         top = g.level_table(n)
