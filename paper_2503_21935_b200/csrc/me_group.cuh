@@ -286,6 +286,93 @@ __device__ __forceinline__ void v4_acc(vec4<float>& acc, const vec4<float>& A, c
 }
 
 
+// Accumulator of one tree task.  fp64: the current itself.  fp32: the sum is kept as TWO packed accumulators per
+// component, acc_i = P_i + i Q_i with P_i, Q_i complex pairs: a complex product c * v adds c.re * v to P and c.im * v
+// to Q, i.e. two FFMA2 whose first operand is a broadcast scalar and whose second is the pair as loaded -- no
+// swapped / sign-flipped copies of either factor (they cost 17 moves and 6 negations per three-gluon term in the
+// single-accumulator form; measured).  P + i Q is folded once per task in finish().
+template <typename T> struct TreeAcc {
+  vec4<T> acc;
+  __device__ __forceinline__ void zero() { acc = zero_vec4<T>(); }
+  __device__ __forceinline__ void v3(const vec4<T>& A, const vec4<T>& B, const T* kA, const T* kB) { v3_acc(acc, A, B, kA, kB); }
+  __device__ __forceinline__ void v4(const vec4<T>& A, const vec4<T>& B, const vec4<T>& C) { v4_acc(acc, A, B, C); }
+  __device__ __forceinline__ vec4<T> finish(T s) const {
+    vec4<T> r;
+#pragma unroll
+    for (int i = 0; i < 4; i++) r.c[i] = s * acc.c[i];
+    return r;
+  }
+};
+// Minkowski product of two complex vectors as (P, Q): a.b = P + i Q, P = sum g_i a_i.re b_i, Q = sum g_i a_i.im b_i
+__device__ __forceinline__ float2 fold_pq(float2 P, float2 Q) { return make_float2(P.x - Q.y, P.y + Q.x); }
+__device__ __forceinline__ float2 mdot_pq(const float2 (&A)[4], const float2 (&B)[4]) {
+  float2 P = __fmul2_rn(make_float2(A[0].x, A[0].x), B[0]);
+  float2 Q = __fmul2_rn(make_float2(A[0].y, A[0].y), B[0]);
+#pragma unroll
+  for (int i = 1; i < 4; i++) {
+    P = __ffma2_rn(make_float2(-A[i].x, -A[i].x), B[i], P);
+    Q = __ffma2_rn(make_float2(-A[i].y, -A[i].y), B[i], Q);
+  }
+  return fold_pq(P, Q);
+}
+template <> struct TreeAcc<float> {
+  float2 P[4], Q[4];
+  __device__ __forceinline__ void zero() {
+#pragma unroll
+    for (int i = 0; i < 4; i++) P[i] = Q[i] = make_float2(0.f, 0.f);
+  }
+  // += c * v   /   -= c * v
+  __device__ __forceinline__ void mac(int i, float2 c, float2 v) {
+    P[i] = __ffma2_rn(make_float2(c.x, c.x), v, P[i]);
+    Q[i] = __ffma2_rn(make_float2(c.y, c.y), v, Q[i]);
+  }
+  __device__ __forceinline__ void msc(int i, float2 c, float2 v) {
+    P[i] = __ffma2_rn(make_float2(-c.x, -c.x), v, P[i]);
+    Q[i] = __ffma2_rn(make_float2(-c.y, -c.y), v, Q[i]);
+  }
+  __device__ __forceinline__ void v3(const vec4<float>& A, const vec4<float>& B, const float* kA, const float* kB) {
+    float2 a[4], b[4];
+    float kab[4], k1[4], k2[4];
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      a[i] = pk(A.c[i]); b[i] = pk(B.c[i]);
+      kab[i] = kA[i] - kB[i];
+      k1[i] = kA[i] + 2.f * kB[i];
+      k2[i] = -(2.f * kA[i] + kB[i]);
+    }
+    const float2 ab = mdot_pq(a, b), ca = mdot2(k1, a), cb = mdot2(k2, b);
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      P[i] = rmac2(P[i], kab[i], ab);
+      mac(i, ca, b[i]);
+      mac(i, cb, a[i]);
+    }
+  }
+  __device__ __forceinline__ void v4(const vec4<float>& A, const vec4<float>& B, const vec4<float>& C) {
+    float2 a[4], b[4], c[4];
+#pragma unroll
+    for (int i = 0; i < 4; i++) { a[i] = pk(A.c[i]); b[i] = pk(B.c[i]); c[i] = pk(C.c[i]); }
+    float2 ac = mdot_pq(a, c);
+    ac = __fadd2_rn(ac, ac);
+    const float2 bc = mdot_pq(b, c), ab = mdot_pq(a, b);
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      mac(i, ac, b[i]);
+      msc(i, bc, a[i]);
+      msc(i, ab, c[i]);
+    }
+  }
+  __device__ __forceinline__ vec4<float> finish(float s) const {
+    vec4<float> r;
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      const float2 t = __fmul2_rn(make_float2(s, s), fold_pq(P[i], Q[i]));
+      r.c[i].re = t.x; r.c[i].im = t.y;
+    }
+    return r;
+  }
+};
+
 // Helicity-independent data of one event: written by setup_kernel (K0) to HBM, staged in shared memory by the warp
 // that evaluates a unit of the event (K1).
 template <typename T, int N>
@@ -483,13 +570,14 @@ __device__ __forceinline__ void grp_tree_level(const GrpEvent<T, G::n>& ev, T* s
     if (active && t < nt) {
       const unsigned* tw = tab + t * W;
       const unsigned h0 = __ldg(tw);
-      vec4<T> acc = zero_vec4<T>();
+      TreeAcc<T> tacc;
+      tacc.zero();
       auto term3 = [&](int j) {
         const unsigned w = __ldg(tw + 2 + j);
         ME_ASSERT((w & 255u) < (unsigned)G::nslot && ((w >> 8) & 255u) < (unsigned)G::nslot);
         const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
         const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
-        v3_acc(acc, A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
+        tacc.v3(A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
       };
       auto term4 = [&](int j) {
         const unsigned w = __ldg(tw + 2 + NV3 + j);
@@ -497,7 +585,7 @@ __device__ __forceinline__ void grp_tree_level(const GrpEvent<T, G::n>& ev, T* s
         const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
         const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
         const vec4<T> C = GrpSlot<T>::ld(slots, (w >> 16) & 255u, 0u);
-        v4_acc(acc, A, B, C);
+        tacc.v4(A, B, C);
       };
       if constexpr (LS > 0) {
 #pragma unroll
@@ -510,9 +598,7 @@ __device__ __forceinline__ void grp_tree_level(const GrpEvent<T, G::n>& ev, T* s
 #pragma unroll(UT)
         for (int j = 0; j < NV4; j++) term4(j);
       }
-      const T s = ev.ik[(h0 >> 8) & 31u];
-#pragma unroll
-      for (int i = 0; i < 4; i++) acc.c[i] = s * acc.c[i];
+      const vec4<T> acc = tacc.finish(ev.ik[(h0 >> 8) & 31u]);
       if (!TOP) {
         ME_ASSERT((h0 & 255u) < (unsigned)G::nslot && ((h0 >> 16) & 255u) < (unsigned)G::nslot);
         GrpSlot<T>::st(slots, h0 & 255u, acc);
