@@ -6,6 +6,8 @@
 // "different helicity combinations of the particles from each event") for
 //     e+ e- -> mu+ mu-      (photon + Z, 2 diagrams)                       BASELINE.json configs[0]
 //     g g -> t tbar + (n-2) g,  n = 2..5 gluons (3/16/123/1240 diagrams)   BASELINE.json configs[1..4]
+//     g ubar -> tau+ tau- + (n-1) g + ubar, n = 1..3 gluons (photon + Z)    SURVEY.md 8(f) NEXT #4: the mixed
+//        EW+QCD workload class of the paper's Table 4 ("g u~ -> tau+ tau- g g u~" is n = 3)
 // The paper prints no formula; the definition written out here is the textbook one
 // (Route A): literal Feynman rules (Peskin & Schroeder conventions), explicit 4x4
 // Dirac matrices in the DIRAC representation, every diagram enumerated and evaluated one by one,
@@ -353,8 +355,8 @@ static ColExp col_comm(const ColExp& a, const ColExp& b, ci f) {  // f * [a, b]
 }
 
 struct Tree {
-  int kind;       // 0 leaf, 3 three-gluon vertex, 4 four-gluon vertex
-  int term;       // four-gluon vertex: which of the three f.f terms (0,1,2)
+  int kind;       // 0 leaf, 3 three-gluon vertex, 4 four-gluon vertex, 5 electroweak boson decaying to the lepton pair
+  int term;       // four-gluon vertex: which of the three f.f terms (0,1,2); boson: 0 photon, 1 Z
   int ch[3];      // child tree ids
   int leg;        // leaf: particle index
   unsigned mask;  // set of particle indices below this tree
@@ -373,6 +375,12 @@ struct SubDiagram {
 };
 struct Process {
   int id, npar, ngl, ncomb, ncol, ndiag, denom;
+  // fermion line: the row spinor sits at the END of the fermion arrow, the column spinor at its start.
+  //   gg -> t tbar + gluons : row = ubar(t) (particle 2, outgoing quark), column = v(tbar) (particle 3), mass m_t
+  //   g ubar -> tau+ tau- + gluons + ubar : row = vbar(ubar in) (particle 1, incoming antiquark), column = v(ubar out)
+  //   (the last particle), massless; ew = true: one photon / Z -> tau- (3) tau+ (2) is attached to the line
+  int row_leg, col_leg, lep_m, lep_p;
+  bool ew;
   std::vector<int> gl;  // gluon particle indices
   std::vector<Tree> trees;
   std::map<unsigned, std::vector<int>> trees_of;  // leg set -> tree ids
@@ -459,13 +467,40 @@ static long count_tree_diagrams(Process& P, int t) {
   return c;
 }
 
-static void enumerate_lines(Process& P, unsigned remaining, int node, const ColExp& prefix_col, long& ndiag) {
-  // choose the next block (any non-empty subset of the remaining gluons) and its tree
-  for (unsigned B = remaining; B; B = (B - 1) & remaining) {
-    const std::vector<int> ts = build_trees(P, B);
-    for (int t : ts) {
+// the electroweak "trees" of a process with ew = true: the photon and the Z attached to the lepton pair; they carry
+// no colour (unit string), their leg set is the lepton pair
+static std::vector<int> boson_trees(Process& P) {
+  const unsigned lm = (1u << P.lep_m) | (1u << P.lep_p);
+  auto it = P.trees_of.find(lm);
+  if (it != P.trees_of.end()) return it->second;
+  std::vector<int> out;
+  for (int b = 0; b < 2; b++) {
+    Tree t;
+    t.kind = 5; t.term = b; t.leg = -1; t.mask = lm; t.ch[0] = t.ch[1] = t.ch[2] = -1;
+    t.col[std::vector<int>()] = ci(1, 0);
+    P.trees.push_back(t);
+    out.push_back((int)P.trees.size() - 1);
+  }
+  P.trees_of[lm] = out;
+  return out;
+}
+
+// remaining: gluon legs not yet attached; boson_left: the electroweak boson is still to be attached
+static void enumerate_lines(Process& P, unsigned remaining, bool boson_left, int node, const ColExp& prefix_col, long& ndiag) {
+  // choose the next block: any non-empty subset of the remaining gluons with one of its trees, or the boson
+  std::vector<std::pair<unsigned, int>> choices;  // (gluon legs used, tree)
+  for (unsigned B = remaining; B; B = (B - 1) & remaining)
+    for (int t : build_trees(P, B)) choices.push_back(std::make_pair(B, t));
+  if (boson_left)
+    for (int t : boson_trees(P)) choices.push_back(std::make_pair(0u, t));
+  for (auto& ch : choices) {
+    const unsigned B = ch.first;
+    const int t = ch.second;
+    const bool is_boson = (P.trees[t].kind == 5);
+    const bool left_after = boson_left && !is_boson;
+    {
       ColExp col = col_mul(prefix_col, P.trees[t].col, ci(1, 0));
-      if (B == remaining) {  // last block: a complete (sub)diagram
+      if (B == remaining && !left_after) {  // last block: a complete (sub)diagram
         SubDiagram d;
         d.prefix = node;
         d.last = t;
@@ -491,9 +526,9 @@ static void enumerate_lines(Process& P, unsigned remaining, int node, const ColE
         P.sub.push_back(d);
       } else {
         TrieNode nd;
-        nd.parent = node; nd.tree = t; nd.mask = (node >= 0 ? P.trie[node].mask : 0u) | B;
+        nd.parent = node; nd.tree = t; nd.mask = (node >= 0 ? P.trie[node].mask : 0u) | P.trees[t].mask;
         P.trie.push_back(nd);
-        enumerate_lines(P, remaining ^ B, (int)P.trie.size() - 1, col, ndiag);
+        enumerate_lines(P, remaining ^ B, left_after, (int)P.trie.size() - 1, col, ndiag);
       }
     }
   }
@@ -602,6 +637,7 @@ static void build_color_matrix(Process& P) {
 static std::string tree_key(const Process& P, int t) {
   const Tree& T = P.trees[t];
   if (T.kind == 0) return std::to_string(T.leg);
+  if (T.kind == 5) return T.term == 0 ? "a" : "z";
   if (T.kind == 3) return "(" + tree_key(P, T.ch[0]) + "," + tree_key(P, T.ch[1]) + ")";
   return "[" + tree_key(P, T.ch[0]) + "," + tree_key(P, T.ch[1]) + "," + tree_key(P, T.ch[2]) + "]";
 }
@@ -631,10 +667,21 @@ static Process* build_process(int id) {
     P->flows.push_back(std::vector<int>());
     return P;
   }
-  int n = id + 1;  // gluons
-  P->ngl = n; P->npar = n + 2; P->ncomb = 1 << P->npar;
-  P->gl.push_back(0); P->gl.push_back(1);
-  for (int k = 4; k < P->npar; k++) P->gl.push_back(k);
+  int n;  // gluons
+  if (id <= 4) {
+    n = id + 1;
+    P->ngl = n; P->npar = n + 2; P->ncomb = 1 << P->npar;
+    P->gl.push_back(0); P->gl.push_back(1);
+    for (int k = 4; k < P->npar; k++) P->gl.push_back(k);
+    P->row_leg = 2; P->col_leg = 3; P->lep_m = P->lep_p = -1; P->ew = false;
+  } else {
+    // g ubar -> tau+ tau- + (n-1) g + ubar: 0 = g, 1 = ubar (in), 2 = tau+, 3 = tau-, 4.. = g, last = ubar (out)
+    n = id - 4;
+    P->ngl = n; P->npar = n + 4; P->ncomb = 1 << P->npar;
+    P->gl.push_back(0);
+    for (int k = 4; k < P->npar - 1; k++) P->gl.push_back(k);
+    P->row_leg = 1; P->col_leg = P->npar - 1; P->lep_p = 2; P->lep_m = 3; P->ew = true;
+  }
   // colour flows: permutations of the gluon particle indices in lexicographic order
   std::vector<int> perm = P->gl;
   std::sort(perm.begin(), perm.end());
@@ -643,10 +690,17 @@ static Process* build_process(int id) {
     P->flows.push_back(perm);
   } while (std::next_permutation(perm.begin(), perm.end()));
   P->ncol = (int)P->flows.size();
-  // denominators: 2*2 gluon spins, 8*8 gluon colours, (n-2)! identical final-state gluons
-  int fact = 1;
-  for (int k = 2; k <= n - 2; k++) fact *= k;
-  P->denom = 4 * 64 * fact;
+  if (id <= 4) {
+    // denominators: 2*2 gluon spins, 8*8 gluon colours, (n-2)! identical final-state gluons
+    int fact = 1;
+    for (int k = 2; k <= n - 2; k++) fact *= k;
+    P->denom = 4 * 64 * fact;
+  } else {
+    // 2*2 initial spins, 8*3 initial colours, (n-1)! identical final-state gluons
+    int fact = 1;
+    for (int k = 2; k <= n - 1; k++) fact *= k;
+    P->denom = 4 * 24 * fact;
+  }
   unsigned all = 0;
   for (int g : P->gl) all |= 1u << g;
   TrieNode root;
@@ -655,16 +709,16 @@ static Process* build_process(int id) {
   ColExp unit;
   unit[std::vector<int>()] = ci(1, 0);
   long nd = 0;
-  enumerate_lines(*P, all, 0, unit, nd);
+  enumerate_lines(*P, all, P->ew, 0, unit, nd);
   P->ndiag = (int)nd;
   build_color_matrix(*P);
   build_channels(*P);
   return P;
 }
 static Process* get_process(int id) {
-  static Process* cache[5] = {0, 0, 0, 0, 0};
+  static Process* cache[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   static std::mutex mtx;
-  if (id < 0 || id > 4) return 0;
+  if (id < 0 || id > 7) return 0;
   std::lock_guard<std::mutex> lock(mtx);
   if (!cache[id]) cache[id] = build_process(id);
   return cache[id];
@@ -683,8 +737,16 @@ static inline int hel_of(int h, int k, int npar) { return ((h >> (npar - 1 - k))
 //   four-gluon vertex    -i g_s^2 [ f^{abe}f^{cde}(g^{mu rho}g^{nu sigma} - g^{mu sigma}g^{nu rho})
 //                                 + f^{ace}f^{bde}(g^{mu nu}g^{rho sigma} - g^{mu sigma}g^{nu rho})
 //                                 + f^{ade}f^{bce}(g^{mu nu}g^{rho sigma} - g^{mu rho}g^{nu sigma}) ]
-// external: incoming g eps, outgoing g eps^*, outgoing t ubar, outgoing tbar v.
-// ward_leg >= 0 replaces that gluon's polarisation by its momentum (gauge test).
+//   fermion-photon vertex  i e Q_f gamma^mu              fermion-Z vertex  i gamma^mu (gL_f P_L + gR_f P_R),
+//                          gL_f = e (T3_f - Q_f sw^2)/(sw cw), gR_f = -e Q_f sw^2/(sw cw)   (u: Q = 2/3, T3 = 1/2;
+//                          tau: Q = -1, T3 = -1/2; (alpha, G_F, M_Z) scheme, reading R5)
+//   photon propagator      -i g_{mu nu} / q^2           Z propagator  -i g_{mu nu} / (q^2 - MZ^2 + i MZ GZ)
+//                          (the q_mu q_nu term vanishes on the massless lepton current, reading R6)
+// external: incoming g eps, outgoing g eps^*, outgoing quark ubar, outgoing antiquark v, incoming antiquark vbar.
+// The electroweak boson with its lepton pair enters the quark line like a colourless gluon tree whose "current" is
+//   V_B^mu = [ubar(tau-) i gamma^mu c_B^tau v(tau+)] (-i / D_B),   attached with the vertex i gamma_mu c_B^u
+// ward_leg >= 0 replaces that gluon's polarisation by its momentum (gauge test); ward_leg = -2 replaces the lepton
+// current by the boson momentum (conservation of the quark current, vector and axial for a massless line).
 // ----------------------------------------------------------------------------------------------
 struct Census {
   long v3, v4, chain, closure, jamp_terms;
@@ -718,6 +780,26 @@ static void eval_jamps(const Process& P, const Params& par, const double* mom, r
       }
       continue;
     }
+    if (T.kind == 5) {
+      // lepton current of boson B = T.term with its propagator (see the header of this function)
+      real_t e, gLl, gRl;
+      ew_couplings(par, e, gLl, gRl);
+      Sp ubl = bar(spinor_u(mom + 4 * P.lep_m, 0.0, hel_of(h, P.lep_m, npar)));
+      Sp vl = spinor_v(mom + 4 * P.lep_p, 0.0, hel_of(h, P.lep_p, npar));
+      M4 cl = (T.term == 0) ? chiral_coupling(-e, -e) : chiral_coupling(gLl, gRl);   // Q_tau = -1
+      cd s = mdot(K, K);
+      cd D = (T.term == 0) ? s : s - par.mz * par.mz + I_ * par.mz * par.wz;
+      V4 L;
+      for (int mu = 0; mu < 4; mu++) {
+        V4 unit;
+        for (int i = 0; i < 4; i++) unit.c[i] = 0.0;
+        unit.c[mu] = (mu == 0) ? 1.0 : -1.0;  // slash(unit) = gamma^mu (upper index)
+        L.c[mu] = I_ * row_col(ubl, times_col(mmul(slash(unit), cl), vl));
+      }
+      if (ward_leg == -2) L = K;
+      cur[t] = vscale(cdiv(-I_, D), L);
+      continue;
+    }
     V4 k3 = vscale(cd(-1.0), K);  // parent line momentum, incoming to this vertex
     cd k2 = mdot(K, K);
     cd prop = cdiv(-I_, k2);  // -i g_{mu nu} / k^2
@@ -740,27 +822,50 @@ static void eval_jamps(const Process& P, const Params& par, const double* mom, r
     }
   }
   // quark line
-  int lt = hel_of(h, 2, npar), ltb = hel_of(h, 3, npar);
-  Sp ub = bar(spinor_u(mom + 8, par.mt, lt));
-  Sp v = spinor_v(mom + 12, par.mt, ltb);
+  const real_t mq = P.ew ? real_t(0.0) : par.mt, wq = P.ew ? real_t(0.0) : par.wt;
+  const int lrow = hel_of(h, P.row_leg, npar), lcol = hel_of(h, P.col_leg, npar);
+  Sp ub = P.ew ? bar(spinor_v(mom + 4 * P.row_leg, mq, lrow))   // incoming antiquark: vbar
+               : bar(spinor_u(mom + 4 * P.row_leg, mq, lrow));  // outgoing quark: ubar
+  Sp v = spinor_v(mom + 4 * P.col_leg, mq, lcol);               // outgoing antiquark: v
+  // vertex of an attached block: i g_s gamma_mu J^mu for a gluon tree, i gamma_mu V^mu c_B^u for the boson
+  real_t e_, gLl_, gRl_, gLu = 0.0, gRu = 0.0, eQu = 0.0;
+  if (P.ew) {
+    ew_couplings(par, e_, gLl_, gRl_);
+    // gL_tau = e(-1/2 + sw^2)/(sw cw), gR_tau = e sw^2/(sw cw)  ->  e/(sw cw) = 2 (gR_tau - gL_tau), sw^2 = gR_tau / (e/(sw cw))
+    real_t eosc = 2.0 * (gRl_ - gLl_), sw2 = gRl_ / eosc;
+    eQu = e_ * (2.0 / 3.0);
+    gLu = eosc * (0.5 - (2.0 / 3.0) * sw2);
+    gRu = eosc * (-(2.0 / 3.0) * sw2);
+  }
+  auto attach = [&](const Sp& r, int tree) {
+    const Tree& T = P.trees[tree];
+    Sp x;
+    if (T.kind == 5) {
+      M4 cq = (T.term == 0) ? chiral_coupling(eQu, eQu) : chiral_coupling(gLu, gRu);
+      x = row_times(r, mmul(slash(cur[tree]), cq));
+      for (int i = 0; i < 4; i++) x.c[i] *= I_;
+    } else {
+      x = row_times(r, slash(cur[tree]));
+      for (int i = 0; i < 4; i++) x.c[i] *= I_ * gs;
+    }
+    return x;
+  };
   size_t nn = P.trie.size();
   std::vector<Sp> chain(nn);
   chain[0] = ub;
   for (size_t n = 1; n < nn; n++) {
     const TrieNode& N = P.trie[n];
-    // vertex i g_s gamma_mu J^mu of the attached tree
-    Sp x = row_times(chain[N.parent], slash(cur[N.tree]));
-    for (int i = 0; i < 4; i++) x.c[i] *= I_ * gs;
-    // propagator: fermion-arrow momentum q = p_t - (momentum injected so far) = -(k_t + sum_prefix k)
+    Sp x = attach(chain[N.parent], N.tree);
+    // propagator: fermion-arrow momentum q = -(k_row + sum_prefix k) (k: incoming convention)
     V4 q;
     for (int m = 0; m < 4; m++) {
-      real_t s = k[2][m];
+      real_t s = k[P.row_leg][m];
       for (int i = 0; i < npar; i++)
         if (N.mask & (1u << i)) s += k[i][m];
       q.c[m] = -s;
     }
-    cd den = mdot(q, q) - par.mt * par.mt + I_ * par.mt * par.wt;
-    Sp y = row_times(x, madd_mass(slash(q), par.mt));
+    cd den = mdot(q, q) - mq * mq + I_ * mq * wq;
+    Sp y = row_times(x, madd_mass(slash(q), mq));
     for (int i = 0; i < 4; i++) y.c[i] *= cdiv(I_, den);
     chain[n] = y;
     if (census) census->chain++;
@@ -769,8 +874,7 @@ static void eval_jamps(const Process& P, const Params& par, const double* mom, r
   if (amps) amps->assign(P.sub.size(), cd(0, 0));
   for (size_t d = 0; d < P.sub.size(); d++) {
     const SubDiagram& D = P.sub[d];
-    Sp x = row_times(chain[D.prefix], slash(cur[D.last]));
-    cd A = I_ * gs * row_col(x, v);
+    cd A = row_col(attach(chain[D.prefix], D.last), v);
     if (amps) (*amps)[d] = A;
     if (census) { census->closure++; census->jamp_terms += (long)D.K.size(); }
     for (auto& kc : D.K) jamp[kc.first] += cd(kc.second.real(), kc.second.imag()) * A;
@@ -786,7 +890,7 @@ static real_t color_sum(const Process& P, const std::vector<cd>& J) {
 }
 
 // ----------------------------------------------------------------------------------------------
-// C interface (ctypes).  proc: 0 ee_mumu, 1 gg_tt, 2 gg_ttg, 3 gg_ttgg, 4 gg_ttggg.
+// C interface (ctypes).  proc: 0 ee_mumu, 1 gg_tt, 2 gg_ttg, 3 gg_ttgg, 4 gg_ttggg, 5/6/7 g ubar -> tau+ tau- ubar + 0/1/2 g.
 // ----------------------------------------------------------------------------------------------
 extern "C" {
 
@@ -978,7 +1082,7 @@ int orc_census(int proc, long* out5) {
 #ifndef ORC_COUNT
 int orc_brute_color(int proc, const double* params, const double* mom, double gs, int h, double* out) {
   Process* P = get_process(proc);
-  if (!P || proc == 0 || P->ngl > 4) return -1;
+  if (!P || proc == 0 || P->ngl > 4 || P->ew) return -1;
   const SU3& S = su3();
   Params par = params_from(params);
   std::vector<cd> J, A;

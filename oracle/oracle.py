@@ -25,7 +25,9 @@ _lock = threading.Lock()
 _lib = None
 _lib_count = None
 
-PROC_ID = {"ee_mumu": 0, "gg_tt": 1, "gg_ttg": 2, "gg_ttgg": 3, "gg_ttggg": 4}
+PROC_ID = {"ee_mumu": 0, "gg_tt": 1, "gg_ttg": 2, "gg_ttgg": 3, "gg_ttggg": 4,
+           "gux_taptamux": 5, "gux_taptamgux": 6, "gux_taptamggux": 7}
+NGLUON = {"ee_mumu": 0, "gg_tt": 2, "gg_ttg": 3, "gg_ttgg": 4, "gg_ttggg": 5, "gux_taptamux": 1, "gux_taptamgux": 2, "gux_taptamggux": 3}
 DEFAULT_PARAMS = dict(mt=173.0, wt=1.4915, mz=91.188, wz=2.441, aewm1=132.507, gf=1.16639e-5)
 
 
@@ -101,7 +103,7 @@ def helicity_table(process: str) -> np.ndarray:
 
 def color_table(process: str) -> np.ndarray:
     i = info(process)
-    n = max(i["npar"] - 2, 0) if process != "ee_mumu" else 0
+    n = NGLUON[process]
     out = np.zeros((i["ncol"], n), dtype=np.int8)
     if n:
         assert lib().orc_color_table(PROC_ID[process], out.ctypes.data) == 0

@@ -36,6 +36,10 @@ PROCESSES = {
     "gg_ttg": dict(npar=5, final_top=(1, 1, 0), ngluon=3),
     "gg_ttgg": dict(npar=6, final_top=(1, 1, 0, 0), ngluon=4),
     "gg_ttggg": dict(npar=7, final_top=(1, 1, 0, 0, 0), ngluon=5),
+    # g ubar -> tau+ tau- + (n-1) g + ubar, all massless (Table 4 is n = 3)
+    "gux_taptamux": dict(npar=5, final_top=(0, 0, 0), ngluon=1),
+    "gux_taptamgux": dict(npar=6, final_top=(0, 0, 0, 0), ngluon=2),
+    "gux_taptamggux": dict(npar=7, final_top=(0, 0, 0, 0, 0), ngluon=3),
 }
 
 _M64 = np.uint64(0xFFFFFFFFFFFFFFFF)
