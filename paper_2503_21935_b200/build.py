@@ -20,7 +20,8 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libme_b200.so")
 
-PROCS = ["ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg"]
+PROCS = ["ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg", "gux_taptamggux"]
+DIAG_PROCS = ["gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg"]   # multichannel (diagram-by-diagram) kernels
 NVCC_BASE = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
              "--expt-relaxed-constexpr", "--extended-lambda", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -50,7 +51,7 @@ def _units():
                 defs.append("-DME_IS_EE_MUMU")
             src = "me_proc_group.cu" if p in GROUP_LAYOUT else "me_proc.cu"
             yield f"{p}_p{prec}", os.path.join(CSRC, src), defs
-    for p in PROCS[1:]:
+    for p in DIAG_PROCS:
         yield f"{p}_diag", os.path.join(CSRC, "me_proc_diag.cu"), [f"-DME_PROC={p}"]
     yield "api", os.path.join(CSRC, "me_api.cu"), []
     yield "peak", os.path.join(CSRC, "me_peak.cu"), []

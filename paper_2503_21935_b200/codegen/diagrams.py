@@ -77,9 +77,12 @@ def canonical(seq):
     return tuple(reversed(seq)), (-1) ** (len(seq) + 1)
 
 
-def build(ngl: int) -> Structure:
-    gluons = (0, 1) + tuple(range(4, ngl + 2))
-    npar = ngl + 2
+def build(ngl: int, gluons=None, npar=None, denom=None, ndiag_factor=None) -> Structure:
+    """gg -> t tbar + (ngl-2) g by default.  Other quark-line processes with the same colour structure pass their own
+    gluon particle indices, particle count, averaging factor and a function ndiag(count over ordered block
+    partitions) -> number of Feynman diagrams (see build_dy)."""
+    gluons = (0, 1) + tuple(range(4, ngl + 2)) if gluons is None else tuple(gluons)
+    npar = ngl + 2 if npar is None else npar
     trees, trees_on = [], {}
 
     def new_tree(**kw):
@@ -149,6 +152,18 @@ def build(ngl: int) -> Structure:
         return total
 
     ndiag = count(gluons)
+    if ndiag_factor is not None:
+        # an extra colourless attachment on the quark line (one of nb bosons): a diagram with k blocks has k + 1 places
+        def count_k(rem, k):
+            if not rem:
+                return k + 1
+            total = 0
+            for r in range(1, len(rem) + 1):
+                for blk in itertools.combinations(rem, r):
+                    rest = tuple(x for x in rem if x not in blk)
+                    total += ntop[blk] * count_k(rest, k + 1)
+            return total
+        ndiag = ndiag_factor * count_k(gluons, 0)
     flows = colour.flows_of(gluons)
     cm = colour.colour_matrix(flows)
     den = 1
@@ -161,7 +176,19 @@ def build(ngl: int) -> Structure:
     for k in range(2, ngl - 1):
         fact *= k
     return Structure(ngl=ngl, gluons=gluons, npar=npar, trees=trees, trees_on=trees_on, flows=flows,
-                     ordered=ordered, ndiag=ndiag, cmat_num=num, cmat_den=den, denom=4 * 64 * fact)
+                     ordered=ordered, ndiag=ndiag, cmat_num=num, cmat_den=den,
+                     denom=(4 * 64 * fact) if denom is None else denom)
+
+
+def build_dy(ngl: int = 3) -> Structure:
+    """g ubar -> tau+ tau- + (ngl-1) g + ubar (Table 4 for ngl = 3):
+    particles 0 = g, 1 = ubar (in), 2 = tau+, 3 = tau-, 4.. = g, last = ubar (out); one quark line with ngl gluons and one
+    photon / Z -> tau pair attached: the colour structure is that of a quark line with ngl gluons."""
+    gluons = (0,) + tuple(range(4, ngl + 3))
+    fact = 1
+    for k in range(2, ngl):
+        fact *= k
+    return build(ngl, gluons=gluons, npar=ngl + 4, denom=4 * 24 * fact, ndiag_factor=2)
 
 
 def _gcd(a, b):

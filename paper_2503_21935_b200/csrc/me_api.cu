@@ -24,6 +24,7 @@ ME_DECL(gg_tt)
 ME_DECL(gg_ttg)
 ME_DECL(gg_ttgg)
 ME_DECL(gg_ttggg)
+ME_DECL(gux_taptamggux)
 
 // multichannel (me_proc_diag.cu), gg processes only
 typedef int (*diag_fn)(const me::LaunchArgs&, const int*, double*, double*, void*, void*);
@@ -45,19 +46,25 @@ namespace {
 struct ProcDesc {
   const char* name;
   int npar, ngl, ndiag;
+  int denom;          // spin and colour average of the initial state x identical final-state particles
+  int gluons[8];      // particle indices of the gluons
+  int nmassive;       // the first nmassive final-state particles have the top mass (me_generate)
   launch_fn fn[3];
   diag_fn diag;
   chanflows_fn chanflows;
   diag_scratch_fn diag_scratch;
   const char* chan_keys;
 };
-#define ME_ROW(name, npar, ngl, ndiag) \
-  { #name, npar, ngl, ndiag, { me_launch_##name##_p0, me_launch_##name##_p1, me_launch_##name##_p2 }, \
+#define ME_ROW(name, npar, ngl, ndiag, denom, ...) \
+  { #name, npar, ngl, ndiag, denom, __VA_ARGS__, 2, { me_launch_##name##_p0, me_launch_##name##_p1, me_launch_##name##_p2 }, \
     me_launch_diag_##name, me_chanflows_##name, me_diag_scratch_##name, kChanKeys_##name }
 const ProcDesc kProcs[] = {
-    { "ee_mumu", 4, 0, 2, { me_launch_ee_mumu_p0, me_launch_ee_mumu_p1, me_launch_ee_mumu_p2 }, nullptr, nullptr, nullptr, kChanKeys_ee_mumu },
-    ME_ROW(gg_tt, 4, 2, 3), ME_ROW(gg_ttg, 5, 3, 16),
-    ME_ROW(gg_ttgg, 6, 4, 123), ME_ROW(gg_ttggg, 7, 5, 1240),
+    { "ee_mumu", 4, 0, 2, 4, {0}, 0, { me_launch_ee_mumu_p0, me_launch_ee_mumu_p1, me_launch_ee_mumu_p2 }, nullptr, nullptr, nullptr, kChanKeys_ee_mumu },
+    ME_ROW(gg_tt, 4, 2, 3, 256, {0, 1}), ME_ROW(gg_ttg, 5, 3, 16, 256, {0, 1, 4}),
+    ME_ROW(gg_ttgg, 6, 4, 123, 512, {0, 1, 4, 5}), ME_ROW(gg_ttggg, 7, 5, 1240, 1536, {0, 1, 4, 5, 6}),
+    // g ubar -> tau+ tau- g g ubar: 0 g, 1 ubar, 2 tau+, 3 tau-, 4 5 g, 6 ubar
+    { "gux_taptamggux", 7, 3, 100, 192, {0, 4, 5}, 0,
+      { me_launch_gux_taptamggux_p0, me_launch_gux_taptamggux_p1, me_launch_gux_taptamggux_p2 }, nullptr, nullptr, nullptr, kChanKeys_gux_taptamggux },
 };
 
 thread_local std::string g_create_error;
@@ -105,7 +112,7 @@ int factorial(int n) { int r = 1; for (int k = 2; k <= n; k++) r *= k; return r;
 // permutations of the gluon particle indices in lexicographic order (reading R8)
 void flows_of(const ProcDesc* p, int8_t* out) {
   int gl[8], n = p->ngl;
-  for (int k = 0; k < n; k++) gl[k] = (k < 2) ? k : k + 2;
+  for (int k = 0; k < n; k++) gl[k] = p->gluons[k];
   int idx[8];
   for (int k = 0; k < n; k++) idx[k] = k;
   int row = 0;
@@ -194,7 +201,7 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
   if (!h) return fail(nullptr, ME_ERR_NOMEM, "me_create: out of host memory");
   h->proc = pd; h->precision = precision; h->device = device;
   h->npar = pd->npar; h->ncomb = 1 << pd->npar; h->ncol = pd->ngl ? factorial(pd->ngl) : 1;
-  h->denom = pd->ngl ? 4 * 64 * factorial(pd->ngl - 2) : 4;
+  h->denom = pd->denom;
   me_params P = {173.0, 1.4915, 91.188, 2.441, 132.507, 1.16639e-5};
   if (params) P = *params;
   h->par.mt = P.mt; h->par.wt = P.wt; h->par.mz = P.mz; h->par.wz = P.wz;
@@ -203,6 +210,7 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
     const double mw2 = 0.5 * mz2 + std::sqrt(0.25 * mz2 * mz2 - pi * alpha * mz2 / (std::sqrt(2.0) * P.gf));
     const double sw2 = 1.0 - mw2 / mz2, sc = std::sqrt(sw2 * (1.0 - sw2)), ee = std::sqrt(4.0 * pi * alpha);
     h->par.ee2 = ee * ee; h->par.gl = ee / sc * (sw2 - 0.5); h->par.gr = ee / sc * sw2;
+    h->par.glu = ee / sc * (0.5 - (2.0 / 3.0) * sw2); h->par.gru = ee / sc * (-(2.0 / 3.0) * sw2);
   }
   h->have_good = false; h->good.n = 0;
   h->d_cum = nullptr; h->cum_bytes = 0; h->d_frac = nullptr; h->d_stage = nullptr; h->stage_bytes = 0;
@@ -333,6 +341,7 @@ void cmat_of(const me_handle* h, const int** num, int* den) {
   else if (!strcmp(n, "gg_tt")) { *num = kCmat_gg_tt; *den = kCden_gg_tt; }
   else if (!strcmp(n, "gg_ttg")) { *num = kCmat_gg_ttg; *den = kCden_gg_ttg; }
   else if (!strcmp(n, "gg_ttgg")) { *num = kCmat_gg_ttgg; *den = kCden_gg_ttgg; }
+  else if (!strcmp(n, "gux_taptamggux")) { *num = kCmat_gux_taptamggux; *den = kCden_gux_taptamggux; }
   else { *num = kCmat_gg_ttggg; *den = kCden_gg_ttggg; }
 }
 
@@ -589,7 +598,7 @@ int me_generate(me_handle* h, uint64_t seed, int64_t start, int64_t nevt, double
   a.mom = d_momenta; a.gs = d_gs; a.rndhel = d_rndhel; a.rndcol = d_rndcol; a.weight = d_weight;
   a.nevt = nevt; a.start = start; a.sqrts = sqrts; a.alphas = alphas;
   double msum = 0.0;
-  for (int i = 0; i < nfin; i++) { a.mass[i] = (h->proc->ngl && i < 2) ? h->par.mt : 0.0; msum += a.mass[i]; }
+  for (int i = 0; i < nfin; i++) { a.mass[i] = (i < h->proc->nmassive) ? h->par.mt : 0.0; msum += a.mass[i]; }
   if (!(msum < sqrts)) return fail(h, ME_ERR_ARG, "me_generate: sqrts below the mass threshold");
   DeviceGuard guard(h->device);
   if (guard.err != cudaSuccess) return cuda_fail(h, guard.err, "me_generate");

@@ -281,6 +281,15 @@ template <typename T> ME_HD spin4<T> row_slash_neg(const spin4<T>& R, const vec4
   for (int i = 0; i < 4; i++) o.c[i] = -o.c[i];
   return o;
 }
+// R (WLslash P_L + WRslash P_R): a vector boson with chirality-dependent couplings on a fermion line (the boson's
+// coupling-weighted current differs for the two chiralities).  In the chiral representation P_L keeps the upper two
+// components of the row R gamma^mu, P_R the lower two.
+template <typename T> ME_HD spin4<T> row_slash_chiral(const spin4<T>& R, const vec4<T>& WL, const vec4<T>& WR) {
+  const spin4<T> a = row_slash(R, WL), b = row_slash(R, WR);
+  spin4<T> o;
+  o.c[0] = a.c[0]; o.c[1] = a.c[1]; o.c[2] = b.c[2]; o.c[3] = b.c[3];
+  return o;
+}
 // X += R * Jslash
 template <typename T> ME_HD void row_slash_add(spin4<T>& X, const spin4<T>& R, const vec4<T>& J) {
   const cx<T> jp = J.c[0] + J.c[3], jm = J.c[0] - J.c[3];

@@ -3,6 +3,7 @@
 namespace me {
 struct DevParams {
   double mt, wt, mz, wz;
-  double ee2, gl, gr;  // e^2 and the Z couplings g_L, g_R of the charged leptons (ee_mumu only)
+  double ee2, gl, gr;  // e^2 and the Z couplings g_L, g_R of the charged leptons
+  double glu, gru;     // Z couplings of the up quark (Q = 2/3, T3 = 1/2)
 };
 }  // namespace me
