@@ -303,23 +303,22 @@ class EmitterDY(Emitter):
         st = self.st
         self.kdone = set()
         hb = lambda k: f"((h >> {st.npar - 1 - k}) & 1)"
-        self.w("// colour-flow amplitudes of helicity row h (particle 0 = most significant bit), g_s = 1")
-        self.w("template <typename T> ME_HD static void jamps(const Event<T>& ev, int h, me::cx<T>* J) {")
+        self.w("// colour-flow amplitudes of helicity row h (particle 0 = most significant bit), g_s = 1, for a quark line of")
+        self.w("// chirality CH (two-component form, me::wsp): CH = 0 the row spinor lives in components (2,3), CH = 1 in (0,1)")
+        self.w("template <int CH, typename T> ME_HD static void jamps_ch(const Event<T>& ev, int h, me::cx<T>* J) {")
         self.ind += 1
         for g in st.gluons:
             out = "false" if g < 2 else "true"
             self.w(f"const me::vec4<T> t{st.trees_on[(g,)][0]} = me::polvec(ev.pol[{g}], {hb(g)} ? 1 : -1, {out});")
-        self.w(f"const me::spin4<T> psi0 = me::select({hb(self.ROW)} != 0, ev.ub[1], ev.ub[0]);")
+        self.w(f"const me::wsp<T> psi0 = me::w_half<CH>(me::select({hb(self.ROW)} != 0, ev.ub[1], ev.ub[0]));")
         self.w(f"const me::spin4<T> vv = me::select({hb(self.col_leg())} != 0, ev.v[1], ev.v[0]);")
-        self.w("me::vec4<T> WL, WR;  // the electroweak insertion for a left- / right-handed quark line")
+        self.w("me::vec4<T> W;  // the electroweak insertion seen by this chirality of the quark line")
         self.w("{")
         self.w("  me::vec4<T> lR, lL;")
         self.w(f"  me::chiral_currents(me::select({hb(self.LEPM)} != 0, ev.lub[1], ev.lub[0]), "
                f"me::select({hb(self.LEPP)} != 0, ev.lv[1], ev.lv[0]), lR, lL);")
-        self.w("  for (int i = 0; i < 4; i++) {")
-        self.w("    WL.c[i] = me::fma(ev.aLR, lR.c[i], ev.aLL * lL.c[i]);")
-        self.w("    WR.c[i] = me::fma(ev.aRR, lR.c[i], ev.aRL * lL.c[i]);")
-        self.w("  }")
+        self.w("  const me::cx<T> aR = CH ? ev.aRR : ev.aLR, aL = CH ? ev.aRL : ev.aLL;")
+        self.w("  for (int i = 0; i < 4; i++) W.c[i] = me::fma(aR, lR.c[i], aL * lL.c[i]);")
         self.w("}")
         done_groups = set()
         for t in st.trees:
@@ -341,10 +340,14 @@ class EmitterDY(Emitter):
                 expr += (" + " if c > 0 else " - ") + f"t{tid}"
             expr = expr[3:] if expr.startswith(" + ") else "me::zero_vec4<T>()" + expr
             self.w(f"const me::vec4<T> {_nm('o', seq)} = {expr};")
-        self.w(f"const me::spin4<T> psi1 = me::row_prop(me::row_slash_chiral(psi0, WL, WR), {self.qexpr((), True)}, T(0), "
-               "me::mk<T>(ev.gd1_none, T(0)));")
+        self.w(f"const me::wsp<T> psi1 = me::w_prop<CH>(me::w_slash<CH>(psi0, W), {self.qexpr((), True)}, ev.gd1_none);")
         self.dfs_dy((), ["psi0"], ["psi1"])
         self.ind -= 1
+        self.w("}")
+        self.w("// an incoming antiquark of helicity +1 is carried by the components (2,3) of its row spinor vbar")
+        self.w("template <typename T> ME_HD static void jamps(const Event<T>& ev, int h, me::cx<T>* J) {")
+        self.w(f"  if ({hb(self.ROW)}) jamps_ch<0, T>(ev, h, J);")
+        self.w("  else jamps_ch<1, T>(ev, h, J);")
         self.w("}")
 
     def qexpr(self, legs, with_boson):
@@ -365,17 +368,17 @@ class EmitterDY(Emitter):
                 for j in range(len(seq)):
                     cur, sgn = self.ordered_ref(seq[j:])
                     if j == 0:
-                        self.w(f"me::spin4<T> {which} = me::row_slash{'' if sgn > 0 else '_neg'}({stack[0]}, {cur});")
+                        self.w(f"me::wsp<T> {which} = me::w_slash{'' if sgn > 0 else '_neg'}<CH>({stack[0]}, {cur});")
                     else:
-                        self.w(f"me::row_slash_{'add' if sgn > 0 else 'sub'}({which}, {stack[j]}, {cur});")
+                        self.w(f"me::w_slash_{'add' if sgn > 0 else 'sub'}<CH>({which}, {stack[j]}, {cur});")
             n0 = _nm("psi0", seq)
-            self.w(f"const me::spin4<T> {n0} = me::row_prop(X0, {self.qexpr(legs, False)}, T(0), me::mk<T>(ev.{_nm('gd0', legs)}, T(0)));")
-            self.w(f"X1 = X1 + me::row_slash_chiral({n0}, WL, WR);")
+            self.w(f"const me::wsp<T> {n0} = me::w_prop<CH>(X0, {self.qexpr(legs, False)}, ev.{_nm('gd0', legs)});")
+            self.w(f"X1 = X1 + me::w_slash<CH>({n0}, W);")
             if len(seq) == st.ngl:
-                self.w(f"J[{st.flows.index(seq)}] = me::row_col(X1, vv);")
+                self.w(f"J[{st.flows.index(seq)}] = me::w_col<CH>(X1, vv);")
             else:
                 n1 = _nm("psi1", seq)
-                self.w(f"const me::spin4<T> {n1} = me::row_prop(X1, {self.qexpr(legs, True)}, T(0), me::mk<T>(ev.{_nm('gd1', legs)}, T(0)));")
+                self.w(f"const me::wsp<T> {n1} = me::w_prop<CH>(X1, {self.qexpr(legs, True)}, ev.{_nm('gd1', legs)});")
                 self.dfs_dy(seq, s0 + [n0], s1 + [n1])
             self.ind -= 1
             self.w("}")

@@ -323,6 +323,67 @@ template <typename T> ME_HD spin4<T> row_prop(const spin4<T>& X, mom4<T> q, T m,
   for (int i = 0; i < 4; i++) o.c[i] = o.c[i] * gd;
   return o;
 }
+// ---------------------------------------------------------------------------------------------
+// Massless quark line of definite chirality: two-component (Weyl) form of the routines above.  In the chiral
+// representation a massless row spinor lives in one half (CH = 0: the lower two components, CH = 1: the upper two);
+// a vertex R Jslash moves it to the other half and the propagator numerator qslash moves it back, so a line costs half
+// the arithmetic and half the registers of the four-component form.
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+struct wsp {  // the two non-zero components
+  cx<T> c[2];
+};
+template <int CH, typename T> ME_HD wsp<T> w_half(const spin4<T>& R) {  // the half a CH line lives in
+  wsp<T> r;
+  r.c[0] = R.c[CH ? 0 : 2]; r.c[1] = R.c[CH ? 1 : 3];
+  return r;
+}
+// R Jslash: CH = 0 takes (R2, R3) and returns components (0, 1); CH = 1 takes (R0, R1) and returns (2, 3)
+template <int CH, typename T> ME_HD wsp<T> w_slash(const wsp<T>& R, const vec4<T>& J) {
+  const cx<T> jp = J.c[0] + J.c[3], jm = J.c[0] - J.c[3];
+  const cx<T> jt = J.c[1] + times_i(J.c[2]), jtb = J.c[1] - times_i(J.c[2]);
+  wsp<T> o;
+  if (CH == 0) { o.c[0] = fma(R.c[1], jt, R.c[0] * jp); o.c[1] = fma(R.c[1], jm, R.c[0] * jtb); }
+  else { o.c[0] = fnma(R.c[1], jt, R.c[0] * jm); o.c[1] = fnma(R.c[0], jtb, R.c[1] * jp); }
+  return o;
+}
+template <int CH, typename T> ME_HD wsp<T> w_slash_neg(const wsp<T>& R, const vec4<T>& J) {
+  wsp<T> o = w_slash<CH>(R, J);
+  o.c[0] = -o.c[0]; o.c[1] = -o.c[1];
+  return o;
+}
+template <int CH, typename T> ME_HD void w_slash_add(wsp<T>& X, const wsp<T>& R, const vec4<T>& J) {
+  const cx<T> jp = J.c[0] + J.c[3], jm = J.c[0] - J.c[3];
+  const cx<T> jt = J.c[1] + times_i(J.c[2]), jtb = J.c[1] - times_i(J.c[2]);
+  if (CH == 0) { X.c[0] = fma(R.c[1], jt, fma(R.c[0], jp, X.c[0])); X.c[1] = fma(R.c[1], jm, fma(R.c[0], jtb, X.c[1])); }
+  else { X.c[0] = fnma(R.c[1], jt, fma(R.c[0], jm, X.c[0])); X.c[1] = fnma(R.c[0], jtb, fma(R.c[1], jp, X.c[1])); }
+}
+template <int CH, typename T> ME_HD void w_slash_sub(wsp<T>& X, const wsp<T>& R, const vec4<T>& J) {
+  const cx<T> jp = J.c[0] + J.c[3], jm = J.c[0] - J.c[3];
+  const cx<T> jt = J.c[1] + times_i(J.c[2]), jtb = J.c[1] - times_i(J.c[2]);
+  if (CH == 0) { X.c[0] = fnma(R.c[1], jt, fnma(R.c[0], jp, X.c[0])); X.c[1] = fnma(R.c[1], jm, fnma(R.c[0], jtb, X.c[1])); }
+  else { X.c[0] = fma(R.c[1], jt, fnma(R.c[0], jm, X.c[0])); X.c[1] = fma(R.c[0], jtb, fnma(R.c[1], jp, X.c[1])); }
+}
+// X qslash / q^2 (massless propagator, gd = 1 / q^2 real): back to the half the line lives in
+template <int CH, typename T> ME_HD wsp<T> w_prop(const wsp<T>& X, mom4<T> q, T gd) {
+  const T qp = q.c[0] + q.c[3], qm = q.c[0] - q.c[3];
+  const cx<T> qt = mk<T>(q.c[1], q.c[2]), qtb = mk<T>(q.c[1], -q.c[2]);
+  wsp<T> o;
+  if (CH == 0) { o.c[0] = fnma(X.c[1], qt, qm * X.c[0]); o.c[1] = fnma(X.c[0], qtb, qp * X.c[1]); }   // (0,1) -> (2,3)
+  else { o.c[0] = fma(X.c[1], qt, qp * X.c[0]); o.c[1] = fma(X.c[0], qtb, qm * X.c[1]); }            // (2,3) -> (0,1)
+  o.c[0] = gd * o.c[0]; o.c[1] = gd * o.c[1];
+  return o;
+}
+template <typename T> ME_HD wsp<T> operator+(const wsp<T>& a, const wsp<T>& b) {
+  wsp<T> r;
+  r.c[0] = a.c[0] + b.c[0]; r.c[1] = a.c[1] + b.c[1];
+  return r;
+}
+// closure with a column spinor: X holds components (0,1) for CH = 0, (2,3) for CH = 1
+template <int CH, typename T> ME_HD cx<T> w_col(const wsp<T>& X, const spin4<T>& v) {
+  return fma(X.c[1], v.c[CH ? 3 : 1], X.c[0] * v.c[CH ? 2 : 0]);
+}
+
 // chiral vector currents of a fermion line, abar gamma^mu P_R b and abar gamma^mu P_L b (upper index):
 //   gamma^mu = [[0, sigma^mu], [sigmabar^mu, 0]], P_L = upper two components, P_R = lower two
 template <typename T>
