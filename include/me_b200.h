@@ -22,13 +22,16 @@
  *   - one handle serves one stream at a time: calls on the same handle from different streams must not overlap
  *     on the device (the scratch is per handle); use one handle per stream for concurrency.
  *   - momenta: [nevt][npar][4] doubles, (E, px, py, pz) in GeV, particle order = process string order,
- *     particles 0,1 incoming; for the gg processes 2 = t, 3 = tbar, 4.. = g; for ee_mumu
+ *     particles 0,1 incoming; for the gg processes 2 = t, 3 = tbar, 4.. = g; for gux_taptamggux
+ *     (g ubar -> tau+ tau- g g ubar through a photon or a Z, the mixed EW+QCD class of PAPER.md:110-122 Table 4)
+ *     0 = g, 1 = ubar, 2 = tau+, 3 = tau-, 4,5 = g, 6 = ubar; for ee_mumu
  *     0 = e+, 1 = e-, 2 = mu+, 3 = mu-.  No special frame is assumed.
  *   - gs: [nevt] doubles, g_s = sqrt(4 pi alpha_s) per event (ignored by ee_mumu, may be NULL there).
  *   - helicity index h (0-based): row of the table returned by me_helicity_table; row h has
  *     lambda_k = +1 if bit (npar-1-k) of h is set, else -1 (particle 0 slowest).
  *   - colour index c (0-based): row of me_color_table, the permutations of the gluon particle indices
- *     in lexicographic order (string from t to tbar).  ee_mumu: ncol = 1.
+ *     in lexicographic order (string from t to tbar; gux_taptamggux: from the incoming to the outgoing ubar).
+ *     ee_mumu: ncol = 1.
  *   - every function returns 0 on success or a negative ME_ERR_* code; me_last_error gives a
  *     NUL-terminated description of the last failure of that handle (or of me_create if h == NULL).
  *     No C++ exception crosses the boundary.  A handle may be used from one host thread at a time;
@@ -66,7 +69,7 @@ enum {
   ME_ERR_NOMEM = -5
 };
 
-/* process: "ee_mumu" | "gg_tt" | "gg_ttg" | "gg_ttgg" | "gg_ttggg"; precision: ME_FP64/ME_FP32/ME_MIXED
+/* process: "ee_mumu" | "gg_tt" | "gg_ttg" | "gg_ttgg" | "gg_ttggg" | "gux_taptamggux"; precision: ME_FP64/ME_FP32/ME_MIXED
  * (mixed = Feynman diagrams in fp64, colour quadratic form in fp32); device: CUDA ordinal. */
 int me_create(me_handle** out, const char* process, int precision, const me_params* params, int device);
 int me_destroy(me_handle* h);
@@ -107,7 +110,7 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
  *   d_den[nevt] = the same summed over ALL diagrams   (fp64 in every build; both include g_s^(2n)),
  * so that num/den is the single-diagram-enhancement weight of the event's channel; and the colour selection
  * (d_selcol) only picks flows that diagram d contributes to.  d_me is the plain ME (multiply by num/den yourself).
- * gg processes only (ME_ERR_PROCESS for ee_mumu).  The first call allocates the kernel's per-event scratch
+ * gg processes only (ME_ERR_PROCESS for ee_mumu and gux_taptamggux).  The first call allocates the kernel's per-event scratch
  * (3.6 KB x min(nevt, 65536) at most); later calls with no more events do not allocate.  Enqueues on `stream`. */
 int me_compute_multichannel(me_handle* h, const double* d_momenta, const double* d_gs, const double* d_rndhel,
                             const double* d_rndcol, const int32_t* d_channel, int64_t nevt, double* d_me,
