@@ -8,12 +8,13 @@ from oracle import rambo as I
 
 pytestmark = pytest.mark.gpu
 
-ALPHAS = {"ee_mumu": 0.118, "gg_tt": 0.118, "gg_ttg": 0.118, "gg_ttgg": None, "gg_ttggg": 0.118}
+ALPHAS = {"ee_mumu": 0.118, "gg_tt": 0.118, "gg_ttg": 0.118, "gg_ttgg": None, "gg_ttggg": 0.118, "gux_taptamggux": None}
 # (process, precision, events = BASELINE config size (gg_ttgg: bench.py's default step), oracle samples, tolerance)
 CASES = [("ee_mumu", "fp64", 16384, 256, 1e-10), ("gg_tt", "fp64", 524288, 256, 1e-10), ("gg_tt", "fp32", 524288, 256, 1e-3),
          ("gg_ttg", "fp64", 524288, 256, 1e-10), ("gg_ttg", "mixed", 524288, 256, 1e-5),
          ("gg_ttgg", "fp64", 1 << 20, 192, 1e-10), ("gg_ttgg", "fp32", 1 << 20, 192, 1e-3), ("gg_ttgg", "mixed", 1 << 20, 192, 1e-5),
-         ("gg_ttggg", "fp64", 262144, 24, 1e-10), ("gg_ttggg", "fp32", 262144, 24, 1e-3)]
+         ("gg_ttggg", "fp64", 262144, 24, 1e-10), ("gg_ttggg", "fp32", 262144, 24, 1e-3),
+         ("gux_taptamggux", "fp64", 524288, 256, 1e-10), ("gux_taptamggux", "fp32", 524288, 256, 1e-3)]
 
 
 @pytest.mark.parametrize("process,precision,nevt,nsample,tol", CASES)
@@ -52,7 +53,7 @@ def test_fullsize_sampled_against_oracle(process, precision, nevt, nsample, tol)
     m.close()
 
 
-@pytest.mark.parametrize("process,nevt", [("gg_ttg", 65536), ("gg_ttgg", 65536), ("gg_ttggg", 2048)])
+@pytest.mark.parametrize("process,nevt", [("gg_ttg", 65536), ("gg_ttgg", 65536), ("gg_ttggg", 2048), ("gux_taptamggux", 16384)])
 def test_accuracy_tail_every_event(process, nevt):
     """Every event of a larger batch against the oracle (flat RAMBO has a soft/collinear tail, no cuts): the
     BASELINE tolerances hold for the worst event, not only for sampled ones (accuracy)."""
