@@ -67,25 +67,26 @@ def flops_per_me(process, ngood):
 
 
 def profile_traffic(process, precision):
-    """DRAM bytes per event of the dominant (amplitude) kernel from the committed ncu summary of this build, or None:
-    (dram__bytes_read.sum + dram__bytes_write.sum) / events of the captured launch."""
-    path = os.path.join(ROOT, "profiles", f"r2_{process}_{precision}_pipeline_ncu_full.txt")
-    if not os.path.exists(path):
-        return None, None
-    txt = open(path).read()
-    m = re.search(r"# events per captured amplitude launch: (\d+)", txt)
-    blocks = txt.split("\nKernel Name")
-    for b in blocks:
-        if "amp_kernel" not in b.split("\n")[0]:
+    """DRAM bytes per event of the dominant kernel (amplitude kernel of the pipeline, or the event kernel) from the
+    committed ncu summary of this build, or None: (dram__bytes_read.sum + dram__bytes_write.sum) / events of the
+    captured launch."""
+    for kind, kernel in (("pipeline", "amp_kernel"), ("event", "event_kernel")):
+        path = os.path.join(ROOT, "profiles", f"r2_{process}_{precision}_{kind}_ncu_full.txt")
+        if not os.path.exists(path):
             continue
-        tot = 0.0
-        for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
-            mm = re.search(re.escape(key) + r" \[(\w+)\] = ([0-9.eE+-]+)", b)
-            if not mm:
-                return None, None
-            tot += float(mm.group(2)) * {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}[mm.group(1)]
-        if m:
-            return tot / int(m.group(1)), os.path.relpath(path, ROOT)
+        txt = open(path).read()
+        m = re.search(r"# events per captured (?:amplitude )?launch: (\d+)", txt)
+        for b in txt.split("\nKernel Name"):
+            if kernel not in b.split("\n")[0]:
+                continue
+            tot = 0.0
+            for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                mm = re.search(re.escape(key) + r" \[(\w+)\] = ([0-9.eE+-]+)", b)
+                if not mm:
+                    return None, None
+                tot += float(mm.group(2)) * {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}[mm.group(1)]
+            if m:
+                return tot / int(m.group(1)), os.path.relpath(path, ROOT)
     return None, None
 
 
@@ -323,7 +324,7 @@ def main():
             "peak_clocks": cs_peak.summary(),
             "traffic": (tr * nevt if tr is not None else None),
             "traffic_source": tr_src,
-            "traffic_note": "DRAM bytes of the amplitude kernel per step, scaled per event from the ncu capture named in "
+            "traffic_note": "DRAM bytes of the dominant kernel per step, scaled per event from the ncu capture named in "
                             "traffic_source; the path is FMA-bound, not HBM-bound",
             "tensor_peaks": ({"dmma_m8n8k4_f64": mma_peak("dmma", local), "tf32_m16n8k8": mma_peak("tf32", local),
                               "note": "me_mma_peak, measured in this run; the colour contraction (K2) uses DMMA in the fp64 build "

@@ -88,9 +88,15 @@ template <typename T> ME_HD T mdot(mom4<T> a, mom4<T> b) {
 // Minkowski product, no complex conjugation
 template <typename T> ME_HD cx<T> mdot(const vec4<T>& a, const vec4<T>& b) {
   cx<T> r = a.c[0] * b.c[0];
+#if !defined(ME_MDOT_FMA) || ME_MDOT_FMA
   r = fnma(a.c[1], b.c[1], r);   // four FMAs per component (r - a*b as a product and a subtraction is six operations)
   r = fnma(a.c[2], b.c[2], r);
   r = fnma(a.c[3], b.c[3], r);
+#else
+  r = r - a.c[1] * b.c[1];
+  r = r - a.c[2] * b.c[2];
+  r = r - a.c[3] * b.c[3];
+#endif
   return r;
 }
 template <typename T> ME_HD cx<T> mdot(mom4<T> k, const vec4<T>& a) {

@@ -1,0 +1,41 @@
+"""The self-contained path (me_generate -> me_compute, the standalone application of PAPER.md:41) against closed-form
+cross sections: sigma = <ME x phase-space weight> / (2 s) over flat RAMBO points must reproduce SURVEY.md 8(c) P2
+(e+ e- -> mu+ mu-, 0.04722784 pb) and P4 (g g -> t tbar at Gamma_t = 0, 6.860453 pb) within the Monte Carlo error.
+Also the measured-peak entry points used by bench.py's roofline."""
+import math
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+GEV2_TO_PB = 0.3893793721e9
+
+
+@pytest.mark.parametrize("process,params,sigma_pb", [("ee_mumu", None, 0.04722784), ("gg_tt", dict(wt=0.0), 6.860453)])
+def test_cross_section_from_device_made_events(process, params, sigma_pb):
+    import torch
+    from paper_2503_21935_b200.me import MatrixElement
+    m = MatrixElement(process, "fp64", params=params)
+    n, s1, s2 = 1 << 20, 0.0, 0.0
+    for it in range(4):
+        mom, gs, rh, rc, wt = m.generate(n, seed=5, start=it * n, alphas=0.118, want_weight=True)
+        if it == 0:
+            m.filter_helicities(mom, gs)
+        me = m.compute(mom, gs)[0]
+        x = me * wt
+        s1 += float(x.sum()); s2 += float((x * x).sum())
+    torch.cuda.synchronize()
+    ntot = 4 * n
+    mean = s1 / ntot
+    err = math.sqrt(max(s2 / ntot - mean * mean, 0.0) / ntot)
+    flux = 2.0 * 1500.0**2
+    sigma, dsigma = mean / flux * GEV2_TO_PB, err / flux * GEV2_TO_PB
+    assert abs(sigma - sigma_pb) < 4.0 * dsigma and dsigma < 2e-3 * sigma_pb, (sigma, dsigma)
+    m.close()
+
+
+def test_measured_peaks_are_sane():
+    from paper_2503_21935_b200.me import fma_peak, mma_peak
+    f64, f32, dmma, tf32 = fma_peak("fp64"), fma_peak("fp32"), mma_peak("dmma"), mma_peak("tf32")
+    assert 20.0 < f64 < 45.0 and 50.0 < f32 < 90.0      # B200: 37 / 74 TFLOP/s nominal
+    assert 0.8 * f64 < dmma < 1.25 * f64                 # DMMA runs on the FP64 units
+    assert tf32 > 2.0 * f32                              # the TF32 tensor pipe is a pipe of its own
