@@ -179,11 +179,13 @@ class Group:
         n = self.n
         # per-op counts derived line by line from me_group.cuh (v3_acc, v4_acc) and me_ops.cuh (row_slash, row_slash_add,
         # row_prop, row_col, mdot): complex multiply 6, complex fma 8, real*complex fma 4
-        V3, V4, SL, SLA, PROP, COL, DOT = 162, 188, 64, 72, 82, 30, 30
+        # (V3: 30 + 8 + 8 for the three Minkowski products, 16 for the momentum combinations from kA and the task's
+        # total momentum, 4 x 24 for the update; + 4 per task for twice the total momentum)
+        V3, V4, SL, SLA, PROP, COL, DOT = 158, 188, 64, 72, 82, 30, 30
         tree = 0
         for L in range(2, n + 1):
             nt = len(self.level_seqs[L])
-            tree += nt * ((L - 1) * V3 + (L - 1) * (L - 2) // 2 * V4 + 8)
+            tree += nt * ((L - 1) * V3 + (L - 1) * (L - 2) // 2 * V4 + 8 + 4)
         tree += len(self.level_seqs[n]) * (4 * DOT + 8)
         walk = 0
         rest = n - 1

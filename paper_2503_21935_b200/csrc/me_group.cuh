@@ -183,15 +183,17 @@ template <> struct GrpSlot<float> {
 };
 
 // acc += (A.B)(kA-kB) + ((kA+2kB).A) B - ((2kA+kB).B) A      (three-gluon vertex, propagator applied later)
+// kB is not loaded: with Kt = kA + kB the momentum of the task's sequence (one load per task, kt2 = 2 Kt),
+// kA - kB = 2 kA - Kt,  kA + 2 kB = 2 Kt - kA,  -(2 kA + kB) = -(kA + Kt): the tree is bound by shared-memory traffic
 template <typename T>
-__device__ __forceinline__ void v3_acc(vec4<T>& acc, const vec4<T>& A, const vec4<T>& B, const T* kA, const T* kB) {
+__device__ __forceinline__ void v3_acc(vec4<T>& acc, const vec4<T>& A, const vec4<T>& B, const T* kA, const T (&kt)[4], const T (&kt2)[4]) {
   const cx<T> ab = mdot(A, B);
   mom4<T> kab, k1, k2;
 #pragma unroll
   for (int i = 0; i < 4; i++) {
-    kab.c[i] = kA[i] - kB[i];
-    k1.c[i] = kA[i] + T(2) * kB[i];
-    k2.c[i] = -(T(2) * kA[i] + kB[i]);
+    kab.c[i] = T(2) * kA[i] - kt[i];
+    k1.c[i] = kt2[i] - kA[i];
+    k2.c[i] = -(kA[i] + kt[i]);
   }
   const cx<T> ca = mdot(k1, A), cb = mdot(k2, B);
 #pragma unroll
@@ -250,15 +252,15 @@ __device__ __forceinline__ float2 mdot2(const float (&k)[4], const float2 (&A)[4
   return rmac2(r, -k[3], A[3]);
 }
 __device__ __forceinline__ void v3_acc(vec4<float>& acc, const vec4<float>& A, const vec4<float>& B, const float* kA,
-                                       const float* kB) {
+                                       const float (&kt)[4], const float (&kt2)[4]) {
   float2 a[4], b[4];
   float kab[4], k1[4], k2[4];
 #pragma unroll
   for (int i = 0; i < 4; i++) {
     a[i] = pk(A.c[i]); b[i] = pk(B.c[i]);
-    kab[i] = kA[i] - kB[i];
-    k1[i] = kA[i] + 2.f * kB[i];
-    k2[i] = -(2.f * kA[i] + kB[i]);
+    kab[i] = 2.f * kA[i] - kt[i];
+    k1[i] = kt2[i] - kA[i];
+    k2[i] = -(kA[i] + kt[i]);
   }
   const float2 ab = mdot2(a, b), ca = mdot2(k1, a), cb = mdot2(k2, b);
 #pragma unroll
@@ -294,7 +296,7 @@ __device__ __forceinline__ void v4_acc(vec4<float>& acc, const vec4<float>& A, c
 template <typename T> struct TreeAcc {
   vec4<T> acc;
   __device__ __forceinline__ void zero() { acc = zero_vec4<T>(); }
-  __device__ __forceinline__ void v3(const vec4<T>& A, const vec4<T>& B, const T* kA, const T* kB) { v3_acc(acc, A, B, kA, kB); }
+  __device__ __forceinline__ void v3(const vec4<T>& A, const vec4<T>& B, const T* kA, const T (&kt)[4], const T (&kt2)[4]) { v3_acc(acc, A, B, kA, kt, kt2); }
   __device__ __forceinline__ void v4(const vec4<T>& A, const vec4<T>& B, const vec4<T>& C) { v4_acc(acc, A, B, C); }
   __device__ __forceinline__ vec4<T> finish(T s) const {
     vec4<T> r;
@@ -330,15 +332,15 @@ template <> struct TreeAcc<float> {
     P[i] = __ffma2_rn(make_float2(-c.x, -c.x), v, P[i]);
     Q[i] = __ffma2_rn(make_float2(-c.y, -c.y), v, Q[i]);
   }
-  __device__ __forceinline__ void v3(const vec4<float>& A, const vec4<float>& B, const float* kA, const float* kB) {
+  __device__ __forceinline__ void v3(const vec4<float>& A, const vec4<float>& B, const float* kA, const float (&kt)[4], const float (&kt2)[4]) {
     float2 a[4], b[4];
     float kab[4], k1[4], k2[4];
 #pragma unroll
     for (int i = 0; i < 4; i++) {
       a[i] = pk(A.c[i]); b[i] = pk(B.c[i]);
-      kab[i] = kA[i] - kB[i];
-      k1[i] = kA[i] + 2.f * kB[i];
-      k2[i] = -(2.f * kA[i] + kB[i]);
+      kab[i] = 2.f * kA[i] - kt[i];
+      k1[i] = kt2[i] - kA[i];
+      k2[i] = -(kA[i] + kt[i]);
     }
     const float2 ab = mdot_pq(a, b), ca = mdot2(k1, a), cb = mdot2(k2, b);
 #pragma unroll
@@ -572,31 +574,58 @@ __device__ __forceinline__ void grp_tree_level(const GrpEvent<T, G::n>& ev, T* s
       const unsigned h0 = __ldg(tw);
       TreeAcc<T> tacc;
       tacc.zero();
+      T kt[4], kt2[4];   // momentum of the task's sequence and twice it
+      {
+        const T* q = ev.Ksub[(h0 >> 8) & 31u];
+#pragma unroll
+        for (int i = 0; i < 4; i++) { kt[i] = q[i]; kt2[i] = q[i] + q[i]; }
+      }
+      // Static levels: the three-gluon terms load every prefix seq[:m] (as A) and every suffix seq[m:] (as B) of the
+      // sequence; the four-gluon term with split points (i, k) needs the prefix i, the suffix k and the middle block, so
+      // it takes the first two from registers and loads only the middle one (9 instead of 15 operand loads per task
+      // at the top level of n = 4: the tree is bound by shared-memory traffic).  Only without per-operand signs (twins).
+      constexpr bool CACHE = (LS > 2) && (G::signs == 0);
+      constexpr int NC = (LS > 2) ? LS - 2 : 1;
+      vec4<T> pre[NC], suf[NC];   // pre[m - 1] = Jord(seq[:m]), m = 1 .. L - 2;  suf[m - 2] = Jord(seq[m:]), m = 2 .. L - 1
       auto term3 = [&](int j) {
         const unsigned w = __ldg(tw + 2 + j);
         ME_ASSERT((w & 255u) < (unsigned)G::nslot && ((w >> 8) & 255u) < (unsigned)G::nslot);
         const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
         const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
-        tacc.v3(A, B, ev.Ksub[(w >> 16) & 31u], ev.Ksub[(w >> 21) & 31u]);
+        if constexpr (CACHE) {
+          const int m = j + 1;
+          if (m <= LS - 2) pre[m - 1] = A;
+          if (m >= 2) suf[m - 2] = B;
+        }
+        tacc.v3(A, B, ev.Ksub[(w >> 16) & 31u], kt, kt2);
       };
-      auto term4 = [&](int j) {
+      auto term4 = [&](int j, int i, int k) {
         const unsigned w = __ldg(tw + 2 + NV3 + j);
         ME_ASSERT((w & 255u) < (unsigned)G::nslot && ((w >> 8) & 255u) < (unsigned)G::nslot && ((w >> 16) & 255u) < (unsigned)G::nslot);
-        const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
         const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
-        const vec4<T> C = GrpSlot<T>::ld(slots, (w >> 16) & 255u, 0u);
-        tacc.v4(A, B, C);
+        if constexpr (CACHE) {
+          tacc.v4(pre[i - 1], B, suf[k - 2]);
+        } else {
+          const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
+          const vec4<T> C = GrpSlot<T>::ld(slots, (w >> 16) & 255u, 0u);
+          tacc.v4(A, B, C);
+        }
       };
       if constexpr (LS > 0) {
+        // term j of the three-gluon list splits the sequence after j + 1 gluons; the four-gluon list runs over the
+        // split points (i, k), 1 <= i < k <= L - 1, in that order (emit_group.py level_table)
 #pragma unroll
         for (int j = 0; j < LS - 1; j++) term3(j);
+        int idx = 0;
 #pragma unroll
-        for (int j = 0; j < (LS - 1) * (LS - 2) / 2; j++) term4(j);
+        for (int i = 1; i < LS; i++)
+#pragma unroll
+          for (int k = i + 1; k < LS; k++) { term4(idx, i, k); idx++; }
       } else {
 #pragma unroll(UT)
         for (int j = 0; j < NV3; j++) term3(j);
 #pragma unroll(UT)
-        for (int j = 0; j < NV4; j++) term4(j);
+        for (int j = 0; j < NV4; j++) term4(j, 1, 2);
       }
       const vec4<T> acc = tacc.finish(ev.ik[(h0 >> 8) & 31u]);
       if (!TOP) {
