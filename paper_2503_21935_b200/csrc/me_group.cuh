@@ -416,7 +416,17 @@ struct GrpGeom {
   // is 32 mod 128
   static constexpr int RAW = (G::nslot + (GrpInit<G>::GLOBAL ? 0 : G::ninit)) * 8;
   static constexpr int UNIT = 32 / (int)sizeof(T);  // T units in 32 bytes
-  static constexpr int GS = ((RAW + 4 * UNIT - 1) / (4 * UNIT)) * (4 * UNIT) + UNIT;
+  // Group stride = a multiple of 128 bytes + PAD.  The lanes r of neighbouring groups read the same slot numbers (same
+  // tables), so the pad decides whether the two groups of a quarter-warp meet in the same banks: fp64 (64-byte slots,
+  // chunk swizzle) 32 bytes; fp32 (32-byte slots at 2 (s mod 4) + chunk) 16 bytes, which puts the second group on the odd
+  // 16-byte positions (modelled wavefronts of the slot accesses of gg_ttgg 588 -> 382 per group pair, ideal 192; measured
+  // +4.8 % gg_ttgg fp32, +3.4 % gg_ttggg fp32; the fp64 builds are best at 32: pads 16 / 48 / 64 measured 2-4 % slower)
+#ifdef ME_GS_PAD_BYTES
+  static constexpr int PAD = ME_GS_PAD_BYTES / (int)sizeof(T);
+#else
+  static constexpr int PAD = (sizeof(T) == 4) ? 16 / (int)sizeof(T) : UNIT;
+#endif
+  static constexpr int GS = ((RAW + 4 * UNIT - 1) / (4 * UNIT)) * (4 * UNIT) + PAD;
   static constexpr int EVB = (((int)sizeof(GrpEvent<T, G::n>) + 127) / 128) * 128;
   static constexpr int SMEM = EVB + GPW * GS * (int)sizeof(T);
 };
