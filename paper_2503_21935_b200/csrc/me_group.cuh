@@ -182,6 +182,28 @@ template <> struct GrpSlot<float> {
   }
 };
 
+// a or -a (neg = 1): sign bits flipped on the integer pipe
+__device__ __forceinline__ vec4<double> vsgn(const vec4<double>& a, unsigned neg) {
+  const int m = (int)(neg << 31);
+  vec4<double> r;
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    r.c[i].re = __hiloint2double(__double2hiint(a.c[i].re) ^ m, __double2loint(a.c[i].re));
+    r.c[i].im = __hiloint2double(__double2hiint(a.c[i].im) ^ m, __double2loint(a.c[i].im));
+  }
+  return r;
+}
+__device__ __forceinline__ vec4<float> vsgn(const vec4<float>& a, unsigned neg) {
+  const int m = (int)(neg << 31);
+  vec4<float> r;
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    r.c[i].re = __int_as_float(__float_as_int(a.c[i].re) ^ m);
+    r.c[i].im = __int_as_float(__float_as_int(a.c[i].im) ^ m);
+  }
+  return r;
+}
+
 // acc += (A.B)(kA-kB) + ((kA+2kB).A) B - ((2kA+kB).B) A      (three-gluon vertex, propagator applied later)
 // kB is not loaded: with Kt = kA + kB the momentum of the task's sequence (one load per task, kt2 = 2 Kt),
 // kA - kB = 2 kA - Kt,  kA + 2 kB = 2 Kt - kA,  -(2 kA + kB) = -(kA + Kt): the tree is bound by shared-memory traffic
@@ -593,28 +615,29 @@ __device__ __forceinline__ void grp_tree_level(const GrpEvent<T, G::n>& ev, T* s
       // Static levels: the three-gluon terms load every prefix seq[:m] (as A) and every suffix seq[m:] (as B) of the
       // sequence; the four-gluon term with split points (i, k) needs the prefix i, the suffix k and the middle block, so
       // it takes the first two from registers and loads only the middle one (9 instead of 15 operand loads per task
-      // at the top level of n = 4: the tree is bound by shared-memory traffic).  Only without per-operand signs (twins).
-      constexpr bool CACHE = (LS > 2) && (G::signs == 0);
+      // at the top level of n = 4: the tree is bound by shared-memory traffic). 
+      constexpr bool CACHE = (LS > 2);
+      constexpr bool SG = (G::signs != 0);   // operand words carry a sign (no twin slots): applied to A at every use
       constexpr int NC = (LS > 2) ? LS - 2 : 1;
       vec4<T> pre[NC], suf[NC];   // pre[m - 1] = Jord(seq[:m]), m = 1 .. L - 2;  suf[m - 2] = Jord(seq[m:]), m = 2 .. L - 1
       auto term3 = [&](int j) {
         const unsigned w = __ldg(tw + 2 + j);
         ME_ASSERT((w & 255u) < (unsigned)G::nslot && ((w >> 8) & 255u) < (unsigned)G::nslot);
-        const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
+        const vec4<T> Ar = GrpSlot<T>::template ld<false>(slots, w & 255u, 0u);
         const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
         if constexpr (CACHE) {
           const int m = j + 1;
-          if (m <= LS - 2) pre[m - 1] = A;
+          if (m <= LS - 2) pre[m - 1] = Ar;
           if (m >= 2) suf[m - 2] = B;
         }
-        tacc.v3(A, B, ev.Ksub[(w >> 16) & 31u], kt, kt2);
+        tacc.v3(SG ? vsgn(Ar, w >> 31) : Ar, B, ev.Ksub[(w >> 16) & 31u], kt, kt2);
       };
       auto term4 = [&](int j, int i, int k) {
         const unsigned w = __ldg(tw + 2 + NV3 + j);
         ME_ASSERT((w & 255u) < (unsigned)G::nslot && ((w >> 8) & 255u) < (unsigned)G::nslot && ((w >> 16) & 255u) < (unsigned)G::nslot);
         const vec4<T> B = GrpSlot<T>::ld(slots, (w >> 8) & 255u, 0u);
         if constexpr (CACHE) {
-          tacc.v4(pre[i - 1], B, suf[k - 2]);
+          tacc.v4(SG ? vsgn(pre[i - 1], w >> 31) : pre[i - 1], B, suf[k - 2]);
         } else {
           const vec4<T> A = GrpSlot<T>::template ld<(G::signs != 0)>(slots, w & 255u, w >> 31);
           const vec4<T> C = GrpSlot<T>::ld(slots, (w >> 16) & 255u, 0u);
@@ -690,13 +713,20 @@ template <class G, typename T, typename TC>
 __device__ __forceinline__ void grp_tree(const GrpEvent<T, G::n>& ev, T* slots, TC* X, int r, bool active) {
   // one copy of the tree code per level with the term loops unrolled (n = 4: +2 % fp64, +5 % fp32, measured), or one
   // copy for all levels with run-time loops
+  // (2: only the top level, which holds most of the tree's work, as a compile-time constant)
 #ifdef ME_TREE_STATIC
-  constexpr bool STATIC = (ME_TREE_STATIC != 0);
+  constexpr int STATIC = ME_TREE_STATIC;
 #else
-  constexpr bool STATIC = (G::n <= 4);
+  // measured: n = 4 all levels static (+2 % fp64, +5 % fp32); n = 5 fp32 top level only (+4.8 %; all levels +2 %); n = 5
+  // fp64 / mixed run-time levels (top level static -7 %, all static -28 %: 168 registers, 3200 instructions)
+  constexpr int STATIC = (G::n <= 4) ? 1 : ((sizeof(T) == 4) ? 2 : 0);
 #endif
-  if constexpr (STATIC) {
+  if constexpr (STATIC == 1) {
     grp_tree_static<G, T, TC, 2>(ev, slots, X, r, active);
+  } else if constexpr (STATIC == 2) {
+#pragma unroll 1
+    for (int L = 2; L < G::n; L++) grp_tree_level<G, T, TC, 0>(ev, slots, X, r, active, L);
+    grp_tree_level<G, T, TC, G::n>(ev, slots, X, r, active, G::n);
   } else {
 #pragma unroll 1
     for (int L = 2; L <= G::n; L++) grp_tree_level<G, T, TC, 0>(ev, slots, X, r, active, L);
