@@ -689,13 +689,11 @@ __device__ __forceinline__ void grp_tree_level(const GrpEvent<T, G::n>& ev, T* s
           }
         } else {
           // ... in "init" slot t of shared memory, read by the leaves of the walk
-          T* ji = slots + (G::nslot + t) * 8;
+          // (stored like a current slot, chunk v = Q(v).J: same swizzle, same conflict pattern as the other slots)
+          vec4<T> ini;
 #pragma unroll
-          for (int v = 0; v < 4; v++) {
-            const vec4<T> q = GrpVec<T>::ld(ev.Q[v], 0u);
-            const cx<T> a = mdot(q, acc);
-            ji[2 * v] = a.re; ji[2 * v + 1] = a.im;
-          }
+          for (int v = 0; v < 4; v++) ini.c[v] = mdot(GrpVec<T>::ld(ev.Q[v], 0u), acc);
+          GrpSlot<T>::st(slots, G::nslot + t, ini);
         }
       }
     }
@@ -791,10 +789,10 @@ struct GrpWalkCtx {
       for (int k = 0; k < NV; k++) { TC x, y; ld2(q + 2 * k, x, y); ini[k][0] = T(x); ini[k][1] = T(y); }
     } else {
       ME_ASSERT((w & 255u) >= (unsigned)G::nslot && (w & 255u) < (unsigned)(G::nslot + G::ninit));
-      const T* ji = slots + (w & 255u) * 8 + 2 * v0;
       const T sg = (w >> 31) ? T(-1) : T(1);
+      const vec4<T> iv = GrpSlot<T>::template ld<false>(slots, w & 255u, 0u);
 #pragma unroll
-      for (int k = 0; k < NV; k++) { ini[k][0] = sg * ji[2 * k]; ini[k][1] = sg * ji[2 * k + 1]; }
+      for (int k = 0; k < NV; k++) { ini[k][0] = sg * iv.c[v0 + k].re; ini[k][1] = sg * iv.c[v0 + k].im; }
     }
 #pragma unroll
     for (int b = 0; b < 2; b++) {
