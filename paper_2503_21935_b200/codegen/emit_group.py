@@ -149,6 +149,7 @@ class Group:
             st = self.role_stream(s1)
             nstream = len(st)
             roles += st
+        roles.append(0)   # one word of padding: the walk may read one word ahead of the last role's stream
         o(f"__device__ const unsigned int kGrpRole_{self.name}[] = {{{', '.join(str(x) for x in roles)}}};")
         o(f"struct Grp_{self.name} {{")
         o(f"  static constexpr int n = {n}, npar = {n + 2}, ncomb = {1 << (n + 2)}, ncol = {len(self.flows)}, "
