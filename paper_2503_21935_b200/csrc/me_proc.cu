@@ -22,6 +22,14 @@
 #ifndef ME_MINB
 #define ME_MINB 1
 #endif
+#ifdef ME_MINB_OVERRIDE   // experiments (ME_B200_NVCC_FLAGS): register cap through the minimum number of resident blocks
+#undef ME_MINB
+#define ME_MINB ME_MINB_OVERRIDE
+#endif
+#ifdef ME_NT_OVERRIDE
+#undef ME_NT
+#define ME_NT ME_NT_OVERRIDE
+#endif
 
 #if ME_PREC == 0
 typedef double T_amp;
