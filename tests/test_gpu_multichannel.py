@@ -81,3 +81,13 @@ def test_multichannel_errors(torch_cuda):
         m.compute_multichannel(mom, None, torch.zeros(8, dtype=torch.int32, device="cuda"))
     assert m.channel_table() == []
     m.close()
+    # the mixed EW+QCD process has no channel kernel either
+    m = MatrixElement("gux_taptamggux", "fp64")
+    mom = torch.from_numpy(I.make_momenta("gux_taptamggux", 8, seed=1)).cuda()
+    gs = torch.from_numpy(I.make_gs(8, seed=1)).cuda()
+    m.filter_helicities(mom, gs)
+    with pytest.raises(MEError):
+        m.compute_multichannel(mom, gs, torch.zeros(8, dtype=torch.int32, device="cuda"))
+    assert m.channel_table() == [] and m.ndiag == 100 and m.ncol == 6 and m.denom == 192
+    assert np.array_equal(m.color_table()[0], [0, 4, 5])
+    m.close()
