@@ -544,9 +544,12 @@ int me_compute_host(me_handle* h, const double* momenta, const double* gs, const
   int rc = ensure(h, &h->d_stage, &h->stage_bytes, 2 * slot);
   if (rc) return rc;
   const bool sh = selhel && rndhel, sc = selcol && rndcol;
-  int64_t k = 0;
-  for (int64_t e0 = 0; e0 < nevt; e0 += chunk, k++) {
-    const int64_t n = (nevt - e0 < chunk) ? (nevt - e0) : chunk;
+  // the first chunk is an eighth of the others: its copy-in is the only one no kernel hides
+  const int64_t first = (chunk / 8 > 4096) ? chunk / 8 : chunk;
+  int64_t k = 0, n = 0;
+  for (int64_t e0 = 0; e0 < nevt; e0 += n, k++) {
+    n = (k == 0) ? first : chunk;
+    if (n > nevt - e0) n = nevt - e0;
     const int b = (int)(k & 1);
     char* base = (char*)h->d_stage + (size_t)b * slot;
     double* d_mom = (double*)base;
