@@ -37,7 +37,8 @@ PER_HELICITY_ACCOUNTING = {"gg_ttgg": 30331 * 64 + 672}
 
 METRIC = "matrix elements/sec (MEs/s) for gg->ttbar gg fp64 & fp32 on 1 B200; % of FMA peak"
 UNIT = "MEs/s"
-ALPHAS = {"ee_mumu": 0.118, "gg_tt": 0.118, "gg_ttg": 0.118, "gg_ttgg": None, "gg_ttggg": 0.118, "gux_taptamggux": None}
+ALPHAS = {"ee_mumu": 0.118, "gg_tt": 0.118, "gg_ttg": 0.118, "gg_ttgg": None, "gg_ttggg": 0.118, "gux_taptamux": None, "gux_taptamgux": None,
+          "gux_taptamggux": None}
 DTYPE = {"fp64": "f64", "fp32": "f32", "mixed": "f64+f32"}
 GROUP = ("gg_ttgg", "gg_ttggg")   # lane-group pipeline: colour contraction on the tensor cores
 
@@ -162,7 +163,7 @@ def cpu_baseline(process, seconds_target=15.0):
     """The oracle as it stands, on this box's host cores, on a bounded sample of the same workload, and the
     oracle's own count of FLOPs per ME ("counted mode": the same source compiled with an operation-counting scalar)."""
     from oracle import oracle as O
-    n0 = {"ee_mumu": 16384, "gg_tt": 16384, "gg_ttg": 4096, "gg_ttgg": 256, "gg_ttggg": 16, "gux_taptamggux": 2048}[process]
+    n0 = {"ee_mumu": 16384, "gg_tt": 16384, "gg_ttg": 4096, "gg_ttgg": 256, "gg_ttggg": 16, "gux_taptamggux": 2048}.get(process, 16384)
     mom, gs = oracle_inputs(process, n0)
     O.me(process, mom[:8], gs[:8])
     t = time.perf_counter(); O.me(process, mom, gs); dt = time.perf_counter() - t
@@ -185,7 +186,7 @@ def run_reference(a):
         return
     from oracle import oracle as O
     process = a.process
-    n0 = {"ee_mumu": 16384, "gg_tt": 16384, "gg_ttg": 16384, "gg_ttgg": 8192, "gg_ttggg": 64, "gux_taptamggux": 16384}[process]
+    n0 = {"ee_mumu": 16384, "gg_tt": 16384, "gg_ttg": 16384, "gg_ttgg": 8192, "gg_ttggg": 64, "gux_taptamggux": 16384}.get(process, 16384)
     mom, gs = oracle_inputs(process, n0)
     mask = O.good_helicities(process, mom[: min(n0, 256)], gs[: min(n0, 256)])
     for _ in range(a.warmup):

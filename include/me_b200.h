@@ -69,7 +69,8 @@ enum {
   ME_ERR_NOMEM = -5
 };
 
-/* process: "ee_mumu" | "gg_tt" | "gg_ttg" | "gg_ttgg" | "gg_ttggg" | "gux_taptamggux"; precision: ME_FP64/ME_FP32/ME_MIXED
+/* process: "ee_mumu" | "gg_tt" | "gg_ttg" | "gg_ttgg" | "gg_ttggg" | "gux_taptamux" | "gux_taptamgux" | "gux_taptamggux"
+ * (g ubar -> tau+ tau- ubar + 0, 1, 2 further gluons); precision: ME_FP64/ME_FP32/ME_MIXED
  * (mixed = Feynman diagrams in fp64, colour quadratic form in fp32); device: CUDA ordinal. */
 int me_create(me_handle** out, const char* process, int precision, const me_params* params, int device);
 int me_destroy(me_handle* h);

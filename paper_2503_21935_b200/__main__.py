@@ -19,7 +19,8 @@ GEV2_TO_PB = 0.3893793721e9
 
 def main():
     ap = argparse.ArgumentParser(prog="python -m paper_2503_21935_b200")
-    ap.add_argument("--process", default="gg_ttgg", choices=["ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg", "gux_taptamggux"])
+    ap.add_argument("--process", default="gg_ttgg", choices=["ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg", "gux_taptamux", "gux_taptamgux",
+                                                              "gux_taptamggux"])
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"])
     ap.add_argument("--nevt", type=int, default=16384, help="events per iteration (one me_compute call)")
     ap.add_argument("--iterations", type=int, default=4)

@@ -24,6 +24,8 @@ ME_DECL(gg_tt)
 ME_DECL(gg_ttg)
 ME_DECL(gg_ttgg)
 ME_DECL(gg_ttggg)
+ME_DECL(gux_taptamux)
+ME_DECL(gux_taptamgux)
 ME_DECL(gux_taptamggux)
 
 // multichannel (me_proc_diag.cu), gg processes only
@@ -62,7 +64,12 @@ const ProcDesc kProcs[] = {
     { "ee_mumu", 4, 0, 2, 4, {0}, 0, { me_launch_ee_mumu_p0, me_launch_ee_mumu_p1, me_launch_ee_mumu_p2 }, nullptr, nullptr, nullptr, kChanKeys_ee_mumu },
     ME_ROW(gg_tt, 4, 2, 3, 256, {0, 1}), ME_ROW(gg_ttg, 5, 3, 16, 256, {0, 1, 4}),
     ME_ROW(gg_ttgg, 6, 4, 123, 512, {0, 1, 4, 5}), ME_ROW(gg_ttggg, 7, 5, 1240, 1536, {0, 1, 4, 5, 6}),
-    // g ubar -> tau+ tau- g g ubar: 0 g, 1 ubar, 2 tau+, 3 tau-, 4 5 g, 6 ubar
+    // g ubar -> tau+ tau- + (n-1) g + ubar (PAPER.md:110-122 is n = 3): 0 g, 1 ubar, 2 tau+, 3 tau-,
+    // 4.. g, last ubar
+    { "gux_taptamux", 5, 1, 4, 96, {0}, 0,
+      { me_launch_gux_taptamux_p0, me_launch_gux_taptamux_p1, me_launch_gux_taptamux_p2 }, nullptr, nullptr, nullptr, kChanKeys_gux_taptamux },
+    { "gux_taptamgux", 6, 2, 16, 96, {0, 4}, 0,
+      { me_launch_gux_taptamgux_p0, me_launch_gux_taptamgux_p1, me_launch_gux_taptamgux_p2 }, nullptr, nullptr, nullptr, kChanKeys_gux_taptamgux },
     { "gux_taptamggux", 7, 3, 100, 192, {0, 4, 5}, 0,
       { me_launch_gux_taptamggux_p0, me_launch_gux_taptamggux_p1, me_launch_gux_taptamggux_p2 }, nullptr, nullptr, nullptr, kChanKeys_gux_taptamggux },
 };
@@ -341,6 +348,8 @@ void cmat_of(const me_handle* h, const int** num, int* den) {
   else if (!strcmp(n, "gg_tt")) { *num = kCmat_gg_tt; *den = kCden_gg_tt; }
   else if (!strcmp(n, "gg_ttg")) { *num = kCmat_gg_ttg; *den = kCden_gg_ttg; }
   else if (!strcmp(n, "gg_ttgg")) { *num = kCmat_gg_ttgg; *den = kCden_gg_ttgg; }
+  else if (!strcmp(n, "gux_taptamux")) { *num = kCmat_gux_taptamux; *den = kCden_gux_taptamux; }
+  else if (!strcmp(n, "gux_taptamgux")) { *num = kCmat_gux_taptamgux; *den = kCden_gux_taptamgux; }
   else if (!strcmp(n, "gux_taptamggux")) { *num = kCmat_gux_taptamggux; *den = kCden_gux_taptamggux; }
   else { *num = kCmat_gg_ttggg; *den = kCden_gg_ttggg; }
 }

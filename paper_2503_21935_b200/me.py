@@ -107,7 +107,7 @@ class MatrixElement:
         v = [ctypes.c_int() for _ in range(5)]
         self._check(self._L.me_info(self._h, *[ctypes.byref(x) for x in v]))
         self.npar, self.ncomb, self.ncol, self.ndiag, self.denom = (x.value for x in v)
-        self.ngluon = {"ee_mumu": 0, "gux_taptamggux": 3}.get(process, self.npar - 2)
+        self.ngluon = {"ee_mumu": 0, "gux_taptamux": 1, "gux_taptamgux": 2, "gux_taptamggux": 3}.get(process, self.npar - 2)
 
     def _check(self, rc):
         if rc != 0:

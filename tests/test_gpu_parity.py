@@ -13,13 +13,14 @@ pytestmark = pytest.mark.gpu
 TOL = {"fp64": 1e-10, "mixed": 1e-5, "fp32": 1e-3}
 # events per parity case: several 128-thread tiles plus a ragged tail; the oracle finishes in seconds
 NEVT = {"ee_mumu": 16384, "gg_tt": 8192 + 77, "gg_ttg": 4096 + 77, "gg_ttgg": 1024 + 77, "gg_ttggg": 128 + 13,
-        "gux_taptamggux": 2048 + 77}
-ALPHAS = {"ee_mumu": 0.118, "gg_tt": 0.118, "gg_ttg": 0.118, "gg_ttgg": None, "gg_ttggg": 0.118, "gux_taptamggux": None}
+        "gux_taptamggux": 2048 + 77, "gux_taptamux": 8192 + 77, "gux_taptamgux": 4096 + 77}
+ALPHAS = {"ee_mumu": 0.118, "gg_tt": 0.118, "gg_ttg": 0.118, "gg_ttgg": None, "gg_ttggg": 0.118, "gux_taptamggux": None, "gux_taptamux": None, "gux_taptamgux": None}
 BUILDS = [("ee_mumu", "fp64"), ("gg_tt", "fp64"), ("gg_tt", "fp32"), ("gg_ttg", "fp64"), ("gg_ttg", "fp32"),
           ("gg_ttg", "mixed"), ("gg_ttgg", "fp64"), ("gg_ttgg", "fp32"), ("gg_ttgg", "mixed"),
           ("gg_ttggg", "fp64"), ("gg_ttggg", "fp32"), ("gg_ttggg", "mixed"),
           # mixed EW+QCD class (Table 4)
-          ("gux_taptamggux", "fp64"), ("gux_taptamggux", "fp32"), ("gux_taptamggux", "mixed")]
+          ("gux_taptamggux", "fp64"), ("gux_taptamggux", "fp32"), ("gux_taptamggux", "mixed"),
+          ("gux_taptamux", "fp64"), ("gux_taptamux", "fp32"), ("gux_taptamgux", "fp64"), ("gux_taptamgux", "fp32")]
 
 
 @pytest.fixture(scope="module")

@@ -9,7 +9,7 @@ from oracle import rambo as I
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("process", ["ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg", "gux_taptamggux"])
+@pytest.mark.parametrize("process", ["ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg", "gux_taptamux", "gux_taptamggux"])
 def test_generate_matches_harness(process):
     import torch
     from paper_2503_21935_b200.me import MatrixElement
