@@ -62,3 +62,42 @@ def test_one_gluon_drell_yan_against_the_closed_form_on_the_gpu():
     # flat RAMBO without cuts: nearly collinear points lose digits in the closed form's own invariants
     assert np.median(rel) < 1e-13 and np.quantile(rel, 0.999) < 1e-9 and rel.max() < 1e-6
     m.close()
+
+
+def test_two_to_two_closed_forms_event_by_event_on_the_gpu():
+    """SURVEY.md 8(c) P1 and P3 evaluated in numpy from the device-made momenta, against the CUDA path directly:
+    gg -> t tbar at Gamma_t = 0:  ME = g_s^4 [1/(6 t1 t2) - 3/8] [t1^2 + t2^2 + rho - rho^2/(4 t1 t2)], t_i = 2 k_i.p_t / s;
+    e+ e- -> mu+ mu-:  ME = u^2 (|A_LL|^2 + |A_RR|^2) + t^2 (|A_LR|^2 + |A_RL|^2), A_XY = e^2/s + g_X g_Y/(s - MZ^2 + i MZ GZ)."""
+    import numpy as np
+    from paper_2503_21935_b200.me import MatrixElement
+    dot = lambda a, b: a[:, 0] * b[:, 0] - (a[:, 1:] * b[:, 1:]).sum(1)
+    n = 1 << 16
+    m = MatrixElement("gg_tt", "fp64", params=dict(wt=0.0))
+    mom, gs, rh, rc = m.generate(n, seed=6)
+    m.filter_helicities(mom, gs)
+    me = m.compute(mom, gs)[0].cpu().numpy()
+    p, g = mom.cpu().numpy(), gs.cpu().numpy()
+    s = 1500.0**2
+    t1, t2, rho = 2.0 * dot(p[:, 0], p[:, 2]) / s, 2.0 * dot(p[:, 1], p[:, 2]) / s, 4.0 * 173.0**2 / s
+    closed = g**4 * (1.0 / (6.0 * t1 * t2) - 0.375) * (t1**2 + t2**2 + rho - rho**2 / (4.0 * t1 * t2))
+    assert np.max(np.abs(me - closed) / closed) < 1e-10
+    m.close()
+
+    m = MatrixElement("ee_mumu", "fp64")
+    mom, gs, rh, rc = m.generate(n, seed=6)
+    m.filter_helicities(mom, None)
+    me = m.compute(mom, None)[0].cpu().numpy()
+    p = mom.cpu().numpy()
+    mz, wz, alpha, gf = 91.188, 2.441, 1.0 / 132.507, 1.16639e-5
+    mw2 = 0.5 * mz**2 + math.sqrt(0.25 * mz**4 - math.pi * alpha * mz**2 / (math.sqrt(2.0) * gf))
+    sw2 = 1.0 - mw2 / mz**2
+    e2 = 4.0 * math.pi * alpha
+    gz = math.sqrt(e2 / (sw2 * (1.0 - sw2)))
+    gl, gr = gz * (sw2 - 0.5), gz * sw2
+    prop = 1.0 / (s - mz * mz + 1j * mz * wz)
+    a = {x + y: e2 / s + cx * cy * prop for x, cx in (("L", gl), ("R", gr)) for y, cy in (("L", gl), ("R", gr))}
+    t = -2.0 * dot(p[:, 1], p[:, 3])    # (p_e- - p_mu-)^2
+    u = -2.0 * dot(p[:, 1], p[:, 2])    # (p_e- - p_mu+)^2
+    closed = u**2 * (abs(a["LL"])**2 + abs(a["RR"])**2) + t**2 * (abs(a["LR"])**2 + abs(a["RL"])**2)
+    assert np.max(np.abs(me - closed) / closed) < 1e-10
+    m.close()
