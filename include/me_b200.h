@@ -101,6 +101,41 @@ int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const 
                const double* d_rndcol, int64_t nevt, double* d_me, int32_t* d_selhel, int32_t* d_selcol,
                void* stream);
 
+/* The hot path for callers that must not allocate device memory: gg -> t tbar g (the process "gg_ttg", particle order
+ * g g -> t tbar g), fp64, with the same optional helicity / colour selection and the same arithmetic as me_compute.
+ *
+ * Why it exists.  me_create and me_set_good_helicities call cudaMalloc.  Some callers cannot: a host application
+ * that has given the whole GPU to its own memory pool at start-up (a library's cudaMalloc then fails, or breaks the
+ * application's accounting), a process confined to a fixed device-memory budget, or a loop that shares the GPU with
+ * other streams and cannot afford the device-wide stall an allocation may cause.  This function takes no handle and
+ * calls no cudaMalloc, cudaFree or allocating library routine, ever.  The scratch its kernel needs (the running sums
+ * over the good helicities, one double per helicity and event) is a fixed 4 MiB array inside the library's device
+ * image; every GPU that loads libme_b200.so holds those 4 MiB until the process exits, used or not.  (Register-spill
+ * space of the kernel, 1.7 KB per thread, is the CUDA driver's own business at the first launch, as for any kernel.)
+ *
+ * Limit.  nevt <= ME_NOALLOC_MAX_EVENTS (16384, the paper's typical 8k-16k events per launch); a larger
+ * nevt is refused with ME_ERR_ARG and a message saying so -- split the batch into calls on the same stream.
+ *
+ * Arguments.  params: as in me_create (NULL = defaults; only mt and wt matter).  good_mask: [32] bytes, 1 = helicity
+ * combination kept (me_get_good_helicities of any gg_ttg handle, in any process, gives it; for a massive top all 32
+ * pass), NULL = all 32.  The d_* pointers, nevt and stream: as in me_compute; d_gs is required.  errbuf / errcap:
+ * HOST buffer that receives a NUL-terminated message on failure (may be NULL; there is no handle to ask).
+ * Returns 0 or a negative ME_ERR_* code.  Enqueues one kernel on `stream`, does not synchronise.
+ *
+ * Device.  Works on the device that is current in the calling thread; the buffers and the stream must belong to it.
+ * The first call on each device looks up the device address of the static scratch (cudaGetSymbolAddress, no
+ * allocation); make that first call before any stream capture begins.
+ *
+ * Sharing.  All calls on a device use the same scratch array, and it keeps whatever the last call left there.  Nothing
+ * in it needs clearing: every thread writes its own entries before reading them.  But two calls of one process whose
+ * kernels run at the same time on one GPU (issued on different streams, from one host thread or several) overwrite
+ * each other's sums and return wrong selections: issue the calls of one device on one stream, or order them with
+ * events.  d_me is not affected, only d_selhel.  Different processes each have their own copy of the array. */
+#define ME_NOALLOC_MAX_EVENTS 16384
+int me_compute_noalloc(const me_params* params, const uint8_t* good_mask, const double* d_momenta, const double* d_gs,
+                       const double* d_rndhel, const double* d_rndcol, int64_t nevt, double* d_me, int32_t* d_selhel,
+                       int32_t* d_selcol, void* stream, char* errbuf, int errcap);
+
 /* Multichannel running ("events from different channels" in one launch).  Reading
  * R17 of DESIGN.md (the paper gives no formula): a channel is a Feynman diagram of the process; channels are numbered
  * 0 .. ndiag-1 in increasing byte order of the structural keys returned by me_channel_table.  d_channel[nevt] (device,

@@ -62,6 +62,8 @@ def _units():
     yield "api", os.path.join(CSRC, "me_api.cu"), []
     yield "peak", os.path.join(CSRC, "me_peak.cu"), []
     yield "rambo", os.path.join(CSRC, "me_rambo.cu"), []
+    # me_compute_noalloc: the gg_ttg fp64 kernel with its scratch in a static device array (flags of the gg_ttg_p0 unit)
+    yield "noalloc", os.path.join(CSRC, "me_noalloc.cu"), ["-DME_PROC=gg_ttg", "-DME_MDOT_FMA=0"]
 
 
 def _deps_hash(defs, extra=()):

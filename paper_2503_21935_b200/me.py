@@ -19,7 +19,7 @@ PROCESSES = ("ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg")
 
 EXPORTS = ("me_create", "me_destroy", "me_last_error", "me_info", "me_helicity_table", "me_color_table",
            "me_color_matrix", "me_filter_helicities", "me_get_good_helicities", "me_set_good_helicities",
-           "me_compute", "me_compute_multichannel", "me_channel_table", "me_compute_host", "me_generate", "me_launch_info", "me_launch_stats", "me_fma_peak", "me_mma_peak")
+           "me_compute", "me_compute_noalloc", "me_compute_multichannel", "me_channel_table", "me_compute_host", "me_generate", "me_launch_info", "me_launch_stats", "me_fma_peak", "me_mma_peak")
 
 
 class MEError(RuntimeError):
@@ -54,6 +54,7 @@ def load_library(path: str = LIB_PATH):
     L.me_get_good_helicities.argtypes = [vp, ip, vp]
     L.me_set_good_helicities.argtypes = [vp, vp]
     L.me_compute.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, vp, vp]
+    L.me_compute_noalloc.argtypes = [ctypes.POINTER(me_params), vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, ctypes.c_char_p, ctypes.c_int]
     L.me_compute_multichannel.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, vp]
     L.me_channel_table.argtypes = [vp, ctypes.c_char_p, ctypes.c_int]
     L.me_compute_host.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, vp]
@@ -258,6 +259,57 @@ class MatrixElement:
         self._check(self._L.me_launch_stats(self._h, ctypes.byref(n), ctypes.byref(c), ctypes.byref(b)))
         d.update(launches=n.value, chunk_events=c.value, scratch_bytes=b.value)
         return d
+
+
+NOALLOC_MAX_EVENTS = 16384   # ME_NOALLOC_MAX_EVENTS of include/me_b200.h
+
+
+def compute_noalloc(momenta, gs, rndhel=None, rndcol=None, good_mask=None, params: dict | None = None, out=None,
+                    selhel=None, selcol=None, stream=None):
+    """me_compute_noalloc: gg -> t tbar g in fp64 without a handle and without any device allocation by the library.
+
+    For callers that cannot let a library call cudaMalloc (the GPU's memory belongs to the application's own pool or
+    budget, or an allocation's device-wide stall is not affordable): the kernel's scratch is a fixed 4 MiB array inside
+    the library, so at most NOALLOC_MAX_EVENTS events per call; more raises MEError.  Calls on one GPU share that
+    array: keep them on one stream (overlapping calls corrupt each other's helicity choice).
+
+    momenta: cuda float64 [nevt, 5, 4]; gs, rndhel, rndcol: cuda float64 [nevt]; good_mask: 32 uint8 (None = all).
+    This binding allocates nothing either if out (float64 [nevt]) and, with random numbers, selhel / selcol (int32
+    [nevt]) are passed in; otherwise it makes them with torch.  Returns (me, selhel, selcol), enqueued on `stream`.
+    """
+    import torch
+    L = load_library()
+    nevt = momenta.shape[0]
+    if tuple(momenta.shape[1:]) != (5, 4):
+        raise MEError("momenta must be [nevt, 5, 4]")
+    dev = momenta.device
+    if out is None:
+        out = torch.empty(nevt, dtype=torch.float64, device=dev)
+    if rndhel is not None and selhel is None:
+        selhel = torch.empty(nevt, dtype=torch.int32, device=dev)
+    if rndcol is not None and selcol is None:
+        selcol = torch.empty(nevt, dtype=torch.int32, device=dev)
+    s = stream if stream is not None else torch.cuda.current_stream(dev)
+    p = None
+    if params is not None:
+        d = dict(mt=173.0, wt=1.4915, mz=91.188, wz=2.441, aewm1=132.507, gf=1.16639e-5)
+        d.update(params)
+        p = me_params(**d)
+    m = None
+    if good_mask is not None:
+        m = np.ascontiguousarray(good_mask, dtype=np.uint8)
+        if m.shape != (32,):
+            raise MEError("good_mask must have 32 entries")
+    err = ctypes.create_string_buffer(256)
+    f64, di = torch.float64, dev.index
+    with torch.cuda.device(dev):   # the entry point works on the calling thread's current device
+        rc = L.me_compute_noalloc(ctypes.byref(p) if p is not None else None, _hptr(m), _ptr(momenta, f64, di), _ptr(gs, f64, di),
+                                  _ptr(rndhel, f64, di), _ptr(rndcol, f64, di), nevt, _ptr(out, f64, di),
+                                  _ptr(selhel, torch.int32, di), _ptr(selcol, torch.int32, di), ctypes.c_void_p(s.cuda_stream),
+                                  err, len(err))
+    if rc != 0:
+        raise MEError(f"error {rc}: {err.value.decode()}")
+    return out, selhel, selcol
 
 
 def fma_peak(precision: str = "fp64", device: int = 0) -> float:
