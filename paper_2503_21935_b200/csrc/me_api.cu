@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <initializer_list>
 #include <new>
 #include <string>
 
@@ -268,6 +269,8 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
       for (int i = 0; i < 7 && e == cudaSuccess; i++) e = cudaEventCreateWithFlags(evs[i], cudaEventDisableTiming);
       if (e != cudaSuccess) {
         int rc = cuda_fail(nullptr, e, "me_create: pipeline streams");
+        for (cudaStream_t s : {px.sa, px.sb, px.s2}) if (s) cudaStreamDestroy(s);   // px was zeroed: non-null = created
+        for (int i = 0; i < 7; i++) if (*evs[i]) cudaEventDestroy(*evs[i]);
         cudaFree(h->d_scratch); cudaFree(h->d_frac);
         delete h;
         return rc;
@@ -553,6 +556,12 @@ int me_compute_host(me_handle* h, const double* momenta, const double* gs, const
   int rc = ensure(h, &h->d_stage, &h->stage_bytes, 2 * slot);
   if (rc) return rc;
   const bool sh = selhel && rndhel, sc = selcol && rndcol;
+  // error exit of the chunk loop: earlier chunks may still be copying into the caller's buffers or using the staging slots;
+  // nothing may be in flight when the caller gets control back
+  auto drain = [h](int code) {
+    cudaStreamSynchronize(h->s_in); cudaStreamSynchronize(h->own_stream); cudaStreamSynchronize(h->s_out);
+    return code;
+  };
   // the first chunk is an eighth of the others: its copy-in is the only one no kernel hides
   const int64_t first = (chunk / 8 > 4096) ? chunk / 8 : chunk;
   int64_t k = 0, n = 0;
@@ -570,25 +579,25 @@ int me_compute_host(me_handle* h, const double* momenta, const double* gs, const
     int32_t* d_sc = (int32_t*)(base + bm + 4 * b8 + b4);
     const size_t nn = (size_t)n;
     // copy in (the slot's inputs are free once the compute of chunk k - 2 has finished)
-    if (k >= 2 && (e = cudaStreamWaitEvent(h->s_in, h->ev_comp[b], 0)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: wait");
-    if ((e = cudaMemcpyAsync(d_mom, momenta + (size_t)e0 * h->npar * 4, nn * h->npar * 32, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return cuda_fail(h, e, "H2D momenta");
-    if (gs && (e = cudaMemcpyAsync(d_gs, gs + e0, nn * 8, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return cuda_fail(h, e, "H2D gs");
-    if (sh && (e = cudaMemcpyAsync(d_rh, rndhel + e0, nn * 8, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return cuda_fail(h, e, "H2D rndhel");
-    if (sc && (e = cudaMemcpyAsync(d_rc, rndcol + e0, nn * 8, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return cuda_fail(h, e, "H2D rndcol");
-    if ((e = cudaEventRecord(h->ev_in[b], h->s_in)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: record");
+    if (k >= 2 && (e = cudaStreamWaitEvent(h->s_in, h->ev_comp[b], 0)) != cudaSuccess) return drain(cuda_fail(h, e, "me_compute_host: wait"));
+    if ((e = cudaMemcpyAsync(d_mom, momenta + (size_t)e0 * h->npar * 4, nn * h->npar * 32, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return drain(cuda_fail(h, e, "H2D momenta"));
+    if (gs && (e = cudaMemcpyAsync(d_gs, gs + e0, nn * 8, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return drain(cuda_fail(h, e, "H2D gs"));
+    if (sh && (e = cudaMemcpyAsync(d_rh, rndhel + e0, nn * 8, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return drain(cuda_fail(h, e, "H2D rndhel"));
+    if (sc && (e = cudaMemcpyAsync(d_rc, rndcol + e0, nn * 8, cudaMemcpyHostToDevice, h->s_in)) != cudaSuccess) return drain(cuda_fail(h, e, "H2D rndcol"));
+    if ((e = cudaEventRecord(h->ev_in[b], h->s_in)) != cudaSuccess) return drain(cuda_fail(h, e, "me_compute_host: record"));
     // compute (the slot's outputs are free once the copy-out of chunk k - 2 has finished)
-    if ((e = cudaStreamWaitEvent(h->own_stream, h->ev_in[b], 0)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: wait");
-    if (k >= 2 && (e = cudaStreamWaitEvent(h->own_stream, h->ev_out[b], 0)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: wait");
+    if ((e = cudaStreamWaitEvent(h->own_stream, h->ev_in[b], 0)) != cudaSuccess) return drain(cuda_fail(h, e, "me_compute_host: wait"));
+    if (k >= 2 && (e = cudaStreamWaitEvent(h->own_stream, h->ev_out[b], 0)) != cudaSuccess) return drain(cuda_fail(h, e, "me_compute_host: wait"));
     rc = me_compute(h, d_mom, gs ? d_gs : nullptr, sh ? d_rh : nullptr, sc ? d_rc : nullptr, n, d_me,
                     sh ? d_sh : nullptr, sc ? d_sc : nullptr, h->own_stream);
-    if (rc) return rc;
-    if ((e = cudaEventRecord(h->ev_comp[b], h->own_stream)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: record");
+    if (rc) return drain(rc);
+    if ((e = cudaEventRecord(h->ev_comp[b], h->own_stream)) != cudaSuccess) return drain(cuda_fail(h, e, "me_compute_host: record"));
     // copy out
-    if ((e = cudaStreamWaitEvent(h->s_out, h->ev_comp[b], 0)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: wait");
-    if ((e = cudaMemcpyAsync(me_out + e0, d_me, nn * 8, cudaMemcpyDeviceToHost, h->s_out)) != cudaSuccess) return cuda_fail(h, e, "D2H me");
-    if (sh && (e = cudaMemcpyAsync(selhel + e0, d_sh, nn * 4, cudaMemcpyDeviceToHost, h->s_out)) != cudaSuccess) return cuda_fail(h, e, "D2H selhel");
-    if (sc && (e = cudaMemcpyAsync(selcol + e0, d_sc, nn * 4, cudaMemcpyDeviceToHost, h->s_out)) != cudaSuccess) return cuda_fail(h, e, "D2H selcol");
-    if ((e = cudaEventRecord(h->ev_out[b], h->s_out)) != cudaSuccess) return cuda_fail(h, e, "me_compute_host: record");
+    if ((e = cudaStreamWaitEvent(h->s_out, h->ev_comp[b], 0)) != cudaSuccess) return drain(cuda_fail(h, e, "me_compute_host: wait"));
+    if ((e = cudaMemcpyAsync(me_out + e0, d_me, nn * 8, cudaMemcpyDeviceToHost, h->s_out)) != cudaSuccess) return drain(cuda_fail(h, e, "D2H me"));
+    if (sh && (e = cudaMemcpyAsync(selhel + e0, d_sh, nn * 4, cudaMemcpyDeviceToHost, h->s_out)) != cudaSuccess) return drain(cuda_fail(h, e, "D2H selhel"));
+    if (sc && (e = cudaMemcpyAsync(selcol + e0, d_sc, nn * 4, cudaMemcpyDeviceToHost, h->s_out)) != cudaSuccess) return drain(cuda_fail(h, e, "D2H selcol"));
+    if ((e = cudaEventRecord(h->ev_out[b], h->s_out)) != cudaSuccess) return drain(cuda_fail(h, e, "me_compute_host: record"));
   }
   if ((e = cudaStreamSynchronize(h->s_out)) != cudaSuccess || (e = cudaStreamSynchronize(h->own_stream)) != cudaSuccess ||
       (e = cudaStreamSynchronize(h->s_in)) != cudaSuccess)

@@ -463,9 +463,6 @@ template <class G> struct XGeom {
 // Arguments of the three kernels of one chunk of events (pointers already offset to the chunk)
 struct PipeArgs {
   LaunchArgs a;
-#ifdef ME_DEBUG_TIMES
-  unsigned long long* dbg;   // [4]: first start / last end of the amplitude kernel, of the colour kernel (globaltimer ns)
-#endif
   void* ev;                  // GrpEvent<T, N>[nevt]
   void* xt;                  // TC[nevt][ncombo][ncol][8] (+ one group of slack)
   const void* cfrag;         // 120 flows: C' in MMA fragment order (global memory), else unused
@@ -1039,10 +1036,6 @@ __global__ void __launch_bounds__(32, MINB) amp_kernel(const PipeArgs p) {
   EV& ev = *reinterpret_cast<EV*>(smem_raw);
   T* gbase = reinterpret_cast<T*>(smem_raw + GE::EVB);
   const int lane = threadIdx.x;
-#ifdef ME_DEBUG_TIMES
-  struct Stamp { unsigned long long* d; __device__ Stamp(unsigned long long* q) : d(q) { if (d && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); atomicMin(d, t); } }
-                 __device__ ~Stamp() { if (d && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); atomicMax(d + 1, t); } } } stamp(p.dbg);
-#endif
   const int gi = lane / LPG, r = lane - gi * LPG;
   const int nunit = (p.ncombo + GPW - 1) / GPW;
   T* slots = gbase + (size_t)((gi < GPW) ? gi : 0) * GE::GS;
@@ -1329,10 +1322,6 @@ __global__ void __launch_bounds__(ColGeom<G, TC>::WARPS * 32) colour_kernel(cons
   constexpr bool CFG = CG::CF_GLOBAL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-#ifdef ME_DEBUG_TIMES
-  struct Stamp { unsigned long long* d; __device__ Stamp(unsigned long long* q) : d(q) { if (d && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); atomicMin(d, t); } }
-                 __device__ ~Stamp() { if (d && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); atomicMax(d + 1, t); } } } stamp(p.dbg ? p.dbg + 2 : nullptr);
-#endif
   constexpr size_t CFB = CFG ? 0 : CG::CF * sizeof(TC);
   double* mh = reinterpret_cast<double*>(smem_raw + CFB + (size_t)warp * CG::PERW);  // [NCOMB]
   double* wcs = mh + NCOMB;                                                          // [NCOL]

@@ -53,14 +53,21 @@ struct CMat {
 template <int MODE, typename TA, typename TCo>
 static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo* info, bool dry) {
   auto kern = me::event_kernel<Proc, TA, TCo, CMat, MODE, ME_NT, ME_MINB>;
-  int dev = 0, sms = 0, per_sm = 0;
+  // size of the persistent grid, asked once per device (not per call)
+  static int grid_cached[64];   // SMs x resident blocks per SM on each device ordinal, 0 = not asked yet
+  int dev = 0;
   cudaError_t err = cudaGetDevice(&dev);
-  if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, ME_NT, 0);
   if (err != cudaSuccess) return (int)err;
-  if (per_sm < 1) per_sm = 1;
+  if (dev < 0 || dev >= 64) return (int)cudaErrorInvalidDevice;
+  if (grid_cached[dev] == 0) {
+    int sms = 0, per_sm = 0;
+    err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, ME_NT, 0);
+    if (err != cudaSuccess) return (int)err;
+    grid_cached[dev] = sms * (per_sm < 1 ? 1 : per_sm);
+  }
   long long ntiles = (a.nevt + ME_NT - 1) / ME_NT;
-  long long blocks = (long long)sms * per_sm;
+  long long blocks = grid_cached[dev];
   if (a.blocks > 0) blocks = a.blocks;
   if (blocks > ntiles) blocks = ntiles;
   if (blocks < 1) blocks = 1;

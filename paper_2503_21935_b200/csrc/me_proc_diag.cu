@@ -34,14 +34,21 @@ int ME_CAT(me_launch_diag_, ME_PROC)(const me::LaunchArgs& a, const int* d_chann
   constexpr int PT = ((1 << Diag::n) + Diag::n + 6 <= 32) ? 32 : 64;
   me::setup_kernel<double, Diag::n><<<(unsigned)((a.nevt * PT + 127) / 128), 128, 0, st>>>(a, (EV*)scratch);
   auto k = me::diag_kernel<Diag>;
-  cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, DG::SMEM);
+  // shared-memory limit and persistent-grid size of the kernel, set once per device (not per call)
+  static int grid_cached[64];   // SMs x resident blocks per SM on each device ordinal, 0 = not set up yet
+  int dev = 0;
+  cudaError_t err = cudaGetDevice(&dev);
   if (err != cudaSuccess) return (int)err;
-  int dev = 0, sms = 0, per_sm = 1;
-  err = cudaGetDevice(&dev);
-  if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, DG::NT, DG::SMEM);
-  if (err != cudaSuccess) return (int)err;
-  long long blocks = (long long)sms * (per_sm < 1 ? 1 : per_sm);
+  if (dev < 0 || dev >= 64) return (int)cudaErrorInvalidDevice;
+  if (grid_cached[dev] == 0) {
+    int sms = 0, per_sm = 1;
+    err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, DG::SMEM);
+    if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, DG::NT, DG::SMEM);
+    if (err != cudaSuccess) return (int)err;
+    grid_cached[dev] = sms * (per_sm < 1 ? 1 : per_sm);
+  }
+  long long blocks = grid_cached[dev];
   if (blocks > a.nevt) blocks = a.nevt;
   me::DiagArgs p;
   p.a = a; p.ev = scratch; p.channel = d_channel; p.num = d_num; p.den = d_den;

@@ -103,18 +103,24 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
   }
   if (dry || a.nevt == 0) return 0;
   if (p.ncombo == 0 || chunk < 1 || !a.scratch) return (int)cudaErrorInvalidValue;
-  // shared memory: what ME_MINB amplitude warps need and no more (the rest of the 256 KB stays L1 for the table words)
-  int carve = (int)((size_t)ME_MINB * (GE::SMEM + 1024) * 100 / (228 * 1024)) + 1;
-  if (carve > 100) carve = 100;
-  int k1_smem = GE::SMEM;
-  if (const char* pad = getenv("ME_B200_AMP_PAD_KB")) { k1_smem += atoi(pad) * 1024; carve = 100; }   // experiments: fewer resident warps
-  err = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, k1_smem);
-  if (err == cudaSuccess) err = cudaFuncSetAttribute(k1, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
-  if (err == cudaSuccess) err = cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, CG::SMEM);
-  int k2_per_sm = 1;
-  if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&k2_per_sm, k2, CG::WARPS * 32, CG::SMEM);
-  if (err != cudaSuccess) return (int)err;
-  if (k2_per_sm < 1) k2_per_sm = 1;
+  // Once per device (not per call: a 256-event step is a few tens of microseconds): the kernels' shared-memory limits
+  // and the colour kernel's residency.  Shared memory of K1: what ME_MINB amplitude warps need and no more (the rest of
+  // the 256 KB stays L1 for the table words).
+  constexpr int k1_smem = GE::SMEM;
+  static int k2_cached[64];   // colour-kernel blocks per SM on each device ordinal, 0 = not set up yet
+  if (dev < 0 || dev >= 64) return (int)cudaErrorInvalidDevice;
+  int k2_per_sm = k2_cached[dev];
+  if (k2_per_sm == 0) {
+    int carve = (int)((size_t)ME_MINB * (GE::SMEM + 1024) * 100 / (228 * 1024)) + 1;
+    if (carve > 100) carve = 100;
+    err = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, k1_smem);
+    if (err == cudaSuccess) err = cudaFuncSetAttribute(k1, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
+    if (err == cudaSuccess) err = cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, CG::SMEM);
+    if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&k2_per_sm, k2, CG::WARPS * 32, CG::SMEM);
+    if (err != cudaSuccess) return (int)err;
+    if (k2_per_sm < 1) k2_per_sm = 1;
+    k2_cached[dev] = k2_per_sm;   // same value from every thread that gets here first
+  }
   if (CG::CF_GLOBAL) {
     void* sym = nullptr;
     static_assert(sizeof(TCo) == sizeof(T_col), "the filter (fp64) is compiled in the fp64 unit only");
@@ -131,16 +137,6 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     if (err == cudaSuccess) err = cudaStreamWaitEvent(px->s2, px->fork, 0);
     if (err != cudaSuccess) return (int)err;
   }
-#ifdef ME_DEBUG_TIMES
-  static unsigned long long* dbg = nullptr;
-  const bool times = MODE != me::MODE_FILTER && getenv("ME_B200_TIMES") && nchunks <= 64;
-  if (times) {
-    if (!dbg) cudaMalloc(&dbg, 64 * 4 * sizeof(unsigned long long));
-    unsigned long long init[64 * 4];
-    for (int i = 0; i < 64 * 4; i++) init[i] = (i & 1) ? 0ull : ~0ull;
-    cudaMemcpy(dbg, init, sizeof(init), cudaMemcpyHostToDevice);
-  }
-#endif
   long long c = 0;
   for (long long e0 = 0; e0 < a.nevt; e0 += chunk, c++) {
     const long long n = (a.nevt - e0 < chunk) ? (a.nevt - e0) : chunk;
@@ -155,9 +151,7 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     p.a.me = a.me ? a.me + e0 : nullptr;
     p.a.selhel = a.selhel ? a.selhel + e0 : nullptr;
     p.a.selcol = a.selcol ? a.selcol + e0 : nullptr;
-#ifdef ME_DEBUG_TIMES
-    p.dbg = times ? dbg + 4 * c : nullptr;
-#endif
+    p.a.channel = a.channel ? a.channel + e0 : nullptr;   // multichannel: the colour kernel indexes it with the chunk-local event
     p.ev = base;
     p.xt = base + align_up((size_t)n * evb, 256);
     constexpr int PT = ((1 << N) + N + 6 <= 32) ? 32 : 64;
@@ -183,17 +177,6 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     err = cudaGetLastError();
     if (err != cudaSuccess) return (int)err;
   }
-#ifdef ME_DEBUG_TIMES
-  if (times) {
-    cudaDeviceSynchronize();
-    unsigned long long t[64 * 4];
-    cudaMemcpy(t, dbg, sizeof(t), cudaMemcpyDeviceToHost);
-    const unsigned long long t0 = t[0];
-    for (long long i = 0; i < nchunks; i++)
-      fprintf(stderr, "chunk %2lld  K1 %9.1f .. %9.1f us   K2 %9.1f .. %9.1f us\n", i, (t[4 * i] - t0) * 1e-3, (t[4 * i + 1] - t0) * 1e-3,
-              (t[4 * i + 2] - t0) * 1e-3, (t[4 * i + 3] - t0) * 1e-3);
-  }
-#endif
   if (px) {  // join: the caller's stream continues after the last colour kernel (s2 is in order, and follows sa / sb)
     err = cudaStreamWaitEvent(st, px->k2[(int)((c - 1) % NPART)], 0);
     if (err != cudaSuccess) return (int)err;

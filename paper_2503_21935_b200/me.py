@@ -15,7 +15,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libme_b200.so")
 PRECISIONS = {"fp64": 0, "fp32": 1, "mixed": 2}
-PROCESSES = ("ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg")
+PROCESSES = ("ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg", "gux_taptamux", "gux_taptamgux", "gux_taptamggux")
 
 EXPORTS = ("me_create", "me_destroy", "me_last_error", "me_info", "me_helicity_table", "me_color_table",
            "me_color_matrix", "me_filter_helicities", "me_get_good_helicities", "me_set_good_helicities",

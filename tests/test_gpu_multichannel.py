@@ -71,6 +71,36 @@ def test_multichannel_matches_oracle(torch_cuda, process, precision):
     m.close()
 
 
+@pytest.mark.parametrize("process,n", [("gg_ttgg", 2 * 4736 + 1234), ("gg_ttggg", 900)])
+def test_multichannel_colour_selection_over_several_chunks(torch_cuda, process, n):
+    """The lane-group pipeline cuts a batch into chunks; every chunk must read ITS events' channels.  One call over several
+    chunks against two calls of unequal size (bit-identical), and every selected flow allowed for the event's own channel."""
+    from oracle import oracle as O
+    from paper_2503_21935_b200.me import MatrixElement
+    torch = torch_cuda
+    dev = torch.device("cuda:0")
+    d = lambda x: torch.from_numpy(x).to(dev)
+    mom, gs = d(I.make_momenta(process, n, seed=9)), d(I.make_gs(n, seed=9, alphas=ALPHAS[process]))
+    rh, rc = (d(x) for x in I.make_rnd(n, seed=9))
+    ndiag = O.info(process)["ndiag"]
+    chan_np = (I.uniforms(9, 7, 0, n) * ndiag).astype(np.int32)
+    chan = d(chan_np)
+    m = MatrixElement(process, "fp64")
+    m.filter_helicities(mom, gs)
+    one = m.compute_multichannel(mom, gs, chan, rh, rc)
+    torch.cuda.synchronize()
+    assert m.launch_info()["chunk_events"] < n, "the case must span several chunks"
+    k = n // 3 + 1
+    a = m.compute_multichannel(mom[:k].contiguous(), gs[:k].contiguous(), chan[:k].contiguous(), rh[:k].contiguous(), rc[:k].contiguous())
+    b = m.compute_multichannel(mom[k:].contiguous(), gs[k:].contiguous(), chan[k:].contiguous(), rh[k:].contiguous(), rc[k:].contiguous())
+    torch.cuda.synchronize()
+    for i in range(5):
+        assert torch.equal(torch.cat([a[i], b[i]]), one[i]), f"output {i} depends on the split"
+    allowed = O.channel_flows(process)
+    assert np.all(allowed[chan_np, one[2].cpu().numpy()])
+    m.close()
+
+
 def test_multichannel_errors(torch_cuda):
     from paper_2503_21935_b200.me import MatrixElement, MEError
     torch = torch_cuda
