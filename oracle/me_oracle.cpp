@@ -69,6 +69,14 @@ static inline bool operator>(real_t a, real_t b) { return a.v > b.v; }
 static inline bool operator>=(real_t a, real_t b) { return a.v >= b.v; }
 static inline real_t SQRT(real_t a) { g_ops.sqrt++; return real_t(std::sqrt(a.v)); }
 static inline double to_double(real_t a) { return a.v; }
+#elif defined(ORC_QUAD)
+// Quadruple-precision build (-DORC_QUAD -> libme_oracle_quad.so): the same source with a 113-bit scalar (libquadmath).
+// The arbiter of the accuracy-tail test: where the fp64 oracle and the fp64 CUDA path disagree beyond the tolerance
+// (cancellations in nearly collinear events), this build says which of the two is off.
+#include <quadmath.h>
+typedef __float128 real_t;
+static inline real_t SQRT(real_t a) { return sqrtq(a); }
+static inline double to_double(real_t a) { return (double)a; }
 #else
 typedef double real_t;
 static inline double SQRT(double a) { return std::sqrt(a); }

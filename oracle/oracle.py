@@ -21,9 +21,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "me_oracle.cpp")
 _LIB = os.path.join(_HERE, "libme_oracle.so")
 _LIB_COUNT = os.path.join(_HERE, "libme_oracle_count.so")   # same source, -DORC_COUNT (counted mode)
+_LIB_QUAD = os.path.join(_HERE, "libme_oracle_quad.so")     # same source, -DORC_QUAD (113-bit scalar, libquadmath)
 _lock = threading.Lock()
 _lib = None
 _lib_count = None
+_lib_quad = None
 
 PROC_ID = {"ee_mumu": 0, "gg_tt": 1, "gg_ttg": 2, "gg_ttgg": 3, "gg_ttggg": 4,
            "gux_taptamux": 5, "gux_taptamgux": 6, "gux_taptamggux": 7}
@@ -33,12 +35,12 @@ DEFAULT_PARAMS = dict(mt=173.0, wt=1.4915, mz=91.188, wz=2.441, aewm1=132.507, g
 
 def build(force: bool = False) -> str:
     """Compile the oracle shared libraries (g++ -O2 -fopenmp) if missing or stale: the plain one and the
-    operation-counting one (same source with -DORC_COUNT)."""
+    operation-counting one (same source with -DORC_COUNT); and the quadruple-precision one (-DORC_QUAD)."""
     with _lock:
-        for target, extra in ((_LIB, []), (_LIB_COUNT, ["-DORC_COUNT"])):
+        for target, extra in ((_LIB, []), (_LIB_COUNT, ["-DORC_COUNT"]), (_LIB_QUAD, ["-DORC_QUAD"])):
             if force or not os.path.exists(target) or os.path.getmtime(target) < os.path.getmtime(_SRC):
                 tmp = target + ".tmp%d" % os.getpid()
-                cmd = ["g++", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c++14"] + extra + [_SRC, "-o", tmp]
+                cmd = ["g++", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c++14"] + extra + [_SRC, "-o", tmp] + (["-lquadmath"] if "-DORC_QUAD" in extra else [])
                 subprocess.check_call(cmd)
                 os.replace(tmp, target)
     return _LIB
@@ -301,6 +303,32 @@ def count_ops(process, momenta1, gs, mask=None, params=None) -> dict:
     d["flops"] = sum(d.values())
     d["me"] = raw.value / i["denom"]
     return d
+
+
+def me_quad(process, momenta, gs, params=None, mask=None, nthreads=0) -> np.ndarray:
+    """ME[nevt] like me(), from the quadruple-precision build of the same source (-DORC_QUAD: every amplitude operation
+    in __float128, the result rounded to double at the end).  Some 50 times slower than me(): meant for the few events
+    where the fp64 oracle and the fp64 CUDA path disagree beyond the tolerance, to say which of the two is off
+    (tests/test_gpu_fullsize.py).  Pinned in tests/test_oracle_quad.py."""
+    global _lib_quad
+    if _lib_quad is None:
+        build()
+        L = ctypes.CDLL(_LIB_QUAD)
+        dp = ctypes.POINTER(ctypes.c_double)
+        L.orc_me_helicities.argtypes = [ctypes.c_int, dp, dp, dp, ctypes.c_int64, ctypes.c_void_p, dp, dp, ctypes.c_int]
+        _lib_quad = L
+    i = info(process)
+    mom = np.ascontiguousarray(momenta, dtype=np.float64)
+    nevt = mom.shape[0]
+    assert mom.shape == (nevt, i["npar"], 4)
+    g = np.ascontiguousarray(np.broadcast_to(np.asarray(gs, dtype=np.float64), (nevt,)))
+    mhel = np.zeros((nevt, i["ncomb"]), dtype=np.float64)
+    p = _params(params)
+    m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    rc = _lib_quad.orc_me_helicities(PROC_ID[process], _dp(p), _dp(mom), _dp(g), nevt, None if m is None else m.ctypes.data,
+                                     _dp(mhel), None, int(nthreads))
+    assert rc == 0
+    return mhel.sum(axis=1) / i["denom"]
 
 
 def num_threads() -> int:

@@ -70,14 +70,19 @@ def test_accuracy_tail_every_event(process, nevt):
         me = m.compute(d_mom, d_gs)[0].cpu().numpy()
         rel = np.abs(me - ref) / ref
         bad = np.nonzero(rel > tol)[0]
-        # An event may exceed the tolerance only if the ORACLE's own rounding noise on it does: Lorentz invariance
-        # (pin P6) measures that noise as the spread of the oracle's value over a few frames.  Seen for one nearly
-        # collinear gluon pair (s_45 / s = 1e-6) of the all-massless process in fp64.
-        assert len(bad) <= max(1, nevt // 4096), f"{precision}: {len(bad)} events above {tol}"
-        for e in bad:
-            noise = max(abs(O.me(process, I.lorentz_transform(mom[e:e + 1], seed=s), gs[e:e + 1])[0] - ref[e]) / ref[e]
-                        for s in range(1, 7))
-            assert rel[e] <= tol + 2.0 * noise, f"{precision}: event {e}: rel diff {rel[e]:.3e}, oracle frame noise {noise:.3e}"
+        # Where the fp64 oracle and the CUDA path disagree beyond the tolerance, the quadruple-precision build of the
+        # oracle (O.me_quad, same source with a 113-bit scalar; pinned in tests/test_oracle_quad.py) decides: the CUDA
+        # value must agree with IT within the stated tolerance.  No allowance beyond that (DESIGN.md section 8,
+        # "accuracy tail"): seen for one nearly collinear gluon pair (s_45 / s = 1e-6) of the all-massless process,
+        # where the fp64 oracle itself is frame dependent at 2e-11.
+        assert len(bad) <= 64, f"{precision}: {len(bad)} events above {tol} against the fp64 oracle"
+        if len(bad):
+            refq = O.me_quad(process, mom[bad], gs[bad])
+            relq = np.abs(me[bad] - refq) / refq
+            worst = int(np.argmax(relq))
+            assert relq.max() <= tol, (f"{precision}: event {bad[worst]}: rel diff {relq[worst]:.3e} against the quad oracle "
+                                       f"({rel[bad[worst]]:.3e} against the fp64 oracle, which is off the quad one by "
+                                       f"{abs(ref[bad[worst]] / refq[worst] - 1):.3e})")
         if precision == "fp32":
             assert np.median(rel) <= 1e-5
         m.close()
