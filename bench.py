@@ -35,6 +35,11 @@ from paper_2503_21935_b200.shard import max_over_ranks, rank_range  # noqa: E402
 # SURVEY.md 8(d) accounting ("each distinct current once per helicity"): FLOPs of the one-event-per-thread code
 PER_HELICITY_ACCOUNTING = {"gg_ttgg": 30331 * 64 + 672}
 
+# FLOPs the kernels EXECUTE per ME according to ncu (thread-level FP64 instruction counts of the committed capture): the
+# generator's count is 1.5 % above it for the amplitude kernel, so a fraction from it is printed too
+EXECUTED_NCU = {("gg_ttgg", "fp64"): {"flops_per_me": 861206 + 64 * 1202 + 1080, "source": "profiles/r2_gg_ttgg_fp64_pipeline_ncu_full.txt: "
+                                      "amplitude kernel 1.411e10 FP64 FLOP / 16384 events = 861206 (generator: 875584); colour and setup kernels as the generator counts them"}}
+
 METRIC = "matrix elements/sec (MEs/s) for gg->ttbar gg fp64 & fp32 on 1 B200; % of FMA peak"
 UNIT = "MEs/s"
 ALPHAS = {"ee_mumu": 0.118, "gg_tt": 0.118, "gg_ttg": 0.118, "gg_ttgg": None, "gg_ttggg": 0.118, "gux_taptamux": None, "gux_taptamgux": None,
@@ -180,6 +185,74 @@ def cpu_baseline(process, seconds_target=15.0):
                           "4x4 matrices, each distinct current once per helicity, colour sum as the plain double sum)"}
 
 
+# The other BASELINE.json configs and the Table-4 process, at their sizes: timed in the
+# default run on rank 0 and reported under "configs" (the headline line stays gg_ttgg = C4)
+CONFIGS = (("ee_mumu", 16384, ("fp64",)), ("gg_tt", 524288, ("fp64", "fp32")), ("gg_ttg", 524288, ("fp64", "fp32", "mixed")),
+           ("gg_ttggg", 262144, ("fp64", "fp32", "mixed")), ("gux_taptamggux", 524288, ("fp64", "fp32", "mixed")))
+
+
+def bench_configs(torch, MatrixElement, local, peaks, nominal, steps=10, warmup=3):
+    """MEs/s and roofline fraction of every (process, precision) of CONFIGS: me_compute with selection on, inputs made on
+    the device, CUDA events on the launch stream, clocks sampled during each timed region."""
+    res = {}
+    for proc, n, precs in CONFIGS:
+        gen = MatrixElement(proc, "fp64", device=local)
+        mom, gs, rh, rc = gen.generate(n, seed=1, alphas=0.0 if ALPHAS[proc] is None else ALPHAS[proc])
+        gen.close()
+        dev = mom.device
+        bufs = (mom, gs, rh, rc, torch.empty(n, dtype=torch.float64, device=dev),
+                torch.empty(n, dtype=torch.int32, device=dev), torch.empty(n, dtype=torch.int32, device=dev))
+        res[proc] = {}
+        for prec in precs:
+            m = MatrixElement(proc, prec, device=local)
+            mask = m.filter_helicities(mom, gs)
+            torch.cuda.synchronize()
+            with ClockSampler(local) as cs:
+                _, per = time_device(torch, m, bufs, steps, warmup)
+            info = m.launch_info()
+            m.close()
+            ms = float(np.mean(per))
+            ngood = int(mask.sum())
+            fl_all, fl_fma, _ = flops_per_me(proc, ngood)
+            on_tensor = proc in GROUP and prec != "fp64"
+            fl = fl_fma if on_tensor else fl_all
+            pipe = "fp32" if prec == "fp32" else "fp64"
+            ach = fl * n / (ms * 1e-3) * 1e-12
+            res[proc][prec] = {"value": n / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "nevt": n, "steps": steps, "warmup": warmup,
+                               "good_helicities": ngood, "flops_per_me": fl, "tflops": ach, "roofline_frac": ach / peaks[pipe],
+                               "roofline_frac_nominal": ach / nominal[pipe], "colour_on_tensor_cores": on_tensor,
+                               "clocks": cs.summary(), "launch": info}
+    return res
+
+
+def bench_multichannel(torch, MatrixElement, local, process="gg_ttgg", n=65536, steps=10, warmup=3):
+    """me_compute_multichannel (reading R17): events of random channels in one call, fp64."""
+    m = MatrixElement(process, "fp64", device=local)
+    mom, gs, rh, rc = m.generate(n, seed=1, alphas=0.0 if ALPHAS[process] is None else ALPHAS[process])
+    m.filter_helicities(mom, gs)
+    chan = torch.randint(0, m.ndiag, (n,), dtype=torch.int32, device=mom.device, generator=torch.Generator(device=mom.device).manual_seed(1))
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        m.compute_multichannel(mom, gs, chan, rh, rc)
+    torch.cuda.synchronize()
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    e0.record(stream)
+    for _ in range(steps):
+        m.compute_multichannel(mom, gs, chan, rh, rc)
+    e1.record(stream)
+    sh, sc = (torch.empty(n, dtype=torch.int32, device=mom.device) for _ in range(2))
+    out = torch.empty(n, dtype=torch.float64, device=mom.device)
+    for _ in range(steps):
+        m.compute(mom, gs, rh, rc, out=out, selhel=sh, selcol=sc)
+    e2.record(stream)
+    torch.cuda.synchronize()
+    t_mc, t_me = e0.elapsed_time(e1) / steps, e1.elapsed_time(e2) / steps
+    m.close()
+    return {"workload": process, "nevt": n, "value": n / (t_mc * 1e-3), "unit": UNIT, "ms_per_step": t_mc,
+            "me_compute_ms_per_step_same_batch": t_me, "diagram_kernel_share": max(0.0, 1.0 - t_me / t_mc),
+            "api": "me_compute_multichannel: me_compute + the diagram-by-diagram kernel for num / den, random channels in one call"}
+
+
 def run_reference(a):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -299,6 +372,10 @@ def main():
             peak = fma_peak(prec_peak, local)
             for _ in range(3):   # a few more runs so that the sampler sees the microbenchmark under load
                 peak = max(peak, fma_peak(prec_peak, local))
+        # the FP64 units serve DFMA and DMMA alike: the measured peak of the pipe is the higher of the two microbenchmarks
+        peak_chain, peak_dmma = peak, (mma_peak("dmma", local) if prec_peak == "fp64" else None)
+        if peak_dmma is not None:
+            peak = max(peak_chain, peak_dmma)
         props = torch.cuda.get_device_properties(local)
         max_mhz = clocks.get("sm_max_mhz") or 1965.0
         nominal = props.multi_processor_count * (64 if prec_peak == "fp64" else 128) * 2 * max_mhz * 1e-6
@@ -320,8 +397,15 @@ def main():
                             + ("; the colour contraction of this build runs on the TF32 tensor cores, so only the "
                                "amplitude part is credited against the FMA peak" if on_tensor else ""),
             "frac_all_flops": fl_all * nevt / (step_ms * 1e-3) * 1e-12 / peak,
+            "flops_per_me_executed_ncu": (EXECUTED_NCU.get((process, a.precision))),
+            "frac_executed_ncu": (EXECUTED_NCU[(process, a.precision)]["flops_per_me"] * nevt / (step_ms * 1e-3) * 1e-12 / peak
+                                  if (process, a.precision) in EXECUTED_NCU else None),
             "tensor_flops_per_me": (fl_all - fl_fma) if on_tensor else 0,
-            "peak_source": f"me_fma_peak({prec_peak}): register-resident FMA chains measured on this GPU in this run (best of 4)",
+            "peak_source": (f"max of me_fma_peak(fp64) = {peak_chain:.2f} (register-resident DFMA chains, best of 4) and "
+                            f"me_mma_peak(dmma) = {peak_dmma:.2f} (DMMA m8n8k4 runs on the same FP64 units), measured on this GPU in this run"
+                            if peak_dmma is not None else
+                            f"me_fma_peak({prec_peak}): register-resident FMA chains measured on this GPU in this run (best of 4)"),
+            "peak_fma_chain": peak_chain,
             "peak_clocks": cs_peak.summary(),
             "traffic": (tr * nevt if tr is not None else None),
             "traffic_source": tr_src,
@@ -362,7 +446,7 @@ def main():
                 continue
             m2, mk2, tot2, per2, clk2, info2 = bench_precision(prec, a.steps, a.warmup, False)
             ms2 = float(np.mean(per2))
-            pk = fma_peak("fp32" if prec == "fp32" else "fp64", local)
+            pk = fma_peak("fp32", local) if prec == "fp32" else max(fma_peak("fp64", local), mma_peak("dmma", local))
             ot = process in GROUP and prec != "fp64"
             ach = (fl_fma if ot else fl_all) * nevt / (ms2 * 1e-3) * 1e-12
             others[prec] = {"value": nevt / (ms2 * 1e-3), "unit": UNIT, "ms_per_step": ms2, "launch": info2,
@@ -406,6 +490,18 @@ def main():
                                  "generate_plus_compute_mes_per_s": a.steps * nevt / (e1.elapsed_time(e2) * 1e-3),
                                  "api": "me_generate (seeded RAMBO on the device) + me_compute"}
         m4.close()
+        if process == "gg_ttgg" and nevt == 1 << 20:   # the default run only
+            max_mhz = clocks.get("sm_max_mhz") or 1965.0
+            sms = torch.cuda.get_device_properties(local).multi_processor_count
+            peaks = {"fp64": max(fma_peak("fp64", local), mma_peak("dmma", local)), "fp32": fma_peak("fp32", local)}
+            nominal = {"fp64": sms * 64 * 2 * max_mhz * 1e-6, "fp32": sms * 128 * 2 * max_mhz * 1e-6}
+            line["configs"] = bench_configs(torch, MatrixElement, local, peaks, nominal)
+            line["configs_note"] = ("BASELINE.json configs C1-C3, C5 and the Table-4 process at their sizes, 10 timed steps each after 3 "
+                                    "warm-ups, selection on; roofline_frac against the measured peaks %s TFLOP/s (fp64 = max of DFMA "
+                                    "chain and DMMA), roofline_frac_nominal against %s; fp32 / mixed of the lane-group processes credit "
+                                    "the amplitude FLOPs only (colour contraction on the TF32 tensor cores)"
+                                    % ({k: round(v, 2) for k, v in peaks.items()}, {k: round(v, 2) for k, v in nominal.items()}))
+            line["multichannel"] = bench_multichannel(torch, MatrixElement, local)
         cb = cpu_baseline(process)
         line["roofline"]["flops_per_me_oracle"] = cb.pop("flops_per_me_counted")
         line["roofline"]["flops_per_me_oracle_note"] = cb.pop("flops_note")

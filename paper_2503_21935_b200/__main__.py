@@ -5,7 +5,7 @@ me_compute, nothing on the host.
     python -m paper_2503_21935_b200 --process gg_ttgg --precision fp64 --nevt 16384 --iterations 4 [--select]
 
 Prints the mean ME, the flat-phase-space estimate of the cross section where it is defined and the throughput.
-Also the small driver of the compute-sanitizer runs whose summaries are under profiles/.
+Also the small driver of the ncu captures whose summaries are under profiles/.
 """
 from __future__ import annotations
 
