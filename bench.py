@@ -59,6 +59,8 @@ def parse():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-sweep", action="store_true", help="skip the events-per-launch sweep 2^8..2^22")
     ap.add_argument("--no-extras", action="store_true", help="skip fp32/mixed lines, cpu_baseline and e2e")
+    ap.add_argument("--multichannel-only", action="store_true",
+                    help="only the me_compute_multichannel leg (the command of the ncu capture of the diagram kernel)")
     return ap.parse_args()
 
 
@@ -303,6 +305,9 @@ def main():
 
     from paper_2503_21935_b200.me import MatrixElement, fma_peak, mma_peak
 
+    if a.multichannel_only:
+        print(json.dumps(bench_multichannel(torch, MatrixElement, 0, process=a.process, steps=a.steps, warmup=a.warmup)))
+        return
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))

@@ -25,19 +25,26 @@ struct DiagArgs {
 };
 
 template <class D> struct DiagGeom {
-  static constexpr int NT = (D::n >= 4) ? 128 : 32;
+  // Threads per event.  The levels of gg -> t tbar g g hold 6 .. 45 tasks (159 closures): one warp wastes a quarter of
+  // its thread slots there, four warps two thirds, and wait at eight barriers per helicity (ncu, round 3: barrier stall
+  // 7.5 per issued instruction with 128 threads).  Five gluons have levels of 10 .. 510 tasks and 1890 closures.
+  static constexpr int NT = (D::n >= 5) ? 128 : 32;
+  // A slot (4 complex doubles) takes SS = 10 doubles: with 80-byte strides the 16-byte accesses of eight neighbouring
+  // slots fall into eight different bank groups (with 64-byte strides they met four to a group: 3.8e9 bank conflicts
+  // on 2.3e9 ideal wavefronts in the same capture)
+  static constexpr int SS = 10;
   static constexpr int EVB = (((int)sizeof(GrpEvent<double, D::n>) + 127) / 128) * 128;
-  static constexpr int SMEM = EVB + (D::ntree + D::nnode) * 64;   // event data, tree currents, quark-line prefixes
+  static constexpr int SMEM = EVB + (D::ntree + D::nnode) * SS * 8;   // event data, tree currents, quark-line prefixes
 };
 
 template <class D>
 __global__ void __launch_bounds__(DiagGeom<D>::NT) diag_kernel(const DiagArgs p) {
-  constexpr int N = D::n, NPAR = N + 2, NT = DiagGeom<D>::NT;
+  constexpr int N = D::n, NPAR = N + 2, NT = DiagGeom<D>::NT, SS = DiagGeom<D>::SS;
   typedef GrpEvent<double, N> EV;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   EV& ev = *reinterpret_cast<EV*>(smem_raw);
   double* trees = reinterpret_cast<double*>(smem_raw + DiagGeom<D>::EVB);
-  double* chain = trees + D::ntree * 8;
+  double* chain = trees + D::ntree * SS;
   __shared__ double red[2][NT / 32];
   const int tid = threadIdx.x;
   const LaunchArgs& a = p.a;
@@ -60,7 +67,7 @@ __global__ void __launch_bounds__(DiagGeom<D>::NT) diag_kernel(const DiagArgs p)
         const int lam = ((h >> (NPAR - 1 - pp)) & 1) ? 1 : -1;
         polbasis<double> pb;
         for (int c = 0; c < 3; c++) { pb.e1[c] = ev.pol[tid][c]; pb.e2[c] = ev.pol[tid][3 + c]; }
-        GrpVec<double>::st(trees + tid * 8, polvec(pb, lam, pp >= 2));
+        GrpVec<double>::st(trees + tid * SS, polvec(pb, lam, pp >= 2));
       }
       if (tid == N) {
         const int ht = (h >> (NPAR - 1 - 2)) & 1;
@@ -74,8 +81,8 @@ __global__ void __launch_bounds__(DiagGeom<D>::NT) diag_kernel(const DiagArgs p)
         for (int t = D::tree_off(L - 2) + tid; t < D::tree_off(L - 1); t += NT) {
           const unsigned* w = D::tree() + 4 * t;
           const unsigned w0 = __ldg(w), w1 = __ldg(w + 1), w2 = __ldg(w + 2), w3 = __ldg(w + 3);
-          const vec4<double> A = GrpVec<double>::ld(trees + (w1 & 0xffffu) * 8, 0u);
-          const vec4<double> B = GrpVec<double>::ld(trees + (w1 >> 16) * 8, 0u);
+          const vec4<double> A = GrpVec<double>::ld(trees + (w1 & 0xffffu) * SS, 0u);
+          const vec4<double> B = GrpVec<double>::ld(trees + (w1 >> 16) * SS, 0u);
           const double ik = ev.ik[w2 >> 16];
           vec4<double> J;
           if (((w0 >> 16) & 15u) == 0u) {
@@ -83,13 +90,13 @@ __global__ void __launch_bounds__(DiagGeom<D>::NT) diag_kernel(const DiagArgs p)
             for (int c = 0; c < 4; c++) { kA.c[c] = ev.Ksub[w3 & 255u][c]; kB.c[c] = ev.Ksub[(w3 >> 8) & 255u][c]; }
             J = vvv_current(A, B, kA, kB, ik);
           } else {
-            const vec4<double> C = GrpVec<double>::ld(trees + (w2 & 0xffffu) * 8, 0u);
+            const vec4<double> C = GrpVec<double>::ld(trees + (w2 & 0xffffu) * SS, 0u);
             vec4<double> J0, J1, J2;
             vvvv_currents(A, B, C, ik, J0, J1, J2);
             const unsigned term = (w0 >> 20) & 3u;
             J = (term == 0u) ? J0 : ((term == 1u) ? J1 : J2);
           }
-          GrpVec<double>::st(trees + (w0 & 0xffffu) * 8, J);
+          GrpVec<double>::st(trees + (w0 & 0xffffu) * SS, J);
         }
         __syncthreads();
       }
@@ -98,15 +105,15 @@ __global__ void __launch_bounds__(DiagGeom<D>::NT) diag_kernel(const DiagArgs p)
       for (int d = 0; d < D::nchainlev; d++) {
         for (int t = D::chain_off(d) + tid; t < D::chain_off(d + 1); t += NT) {
           const unsigned w0 = __ldg(D::chain() + 2 * t), w1 = __ldg(D::chain() + 2 * t + 1);
-          const spin4<double> R = ld_spin<double>(chain + (w0 >> 16) * 8);
-          const vec4<double> J = GrpVec<double>::ld(trees + (w1 & 0xffffu) * 8, 0u);
+          const spin4<double> R = ld_spin<double>(chain + (w0 >> 16) * SS);
+          const vec4<double> J = GrpVec<double>::ld(trees + (w1 & 0xffffu) * SS, 0u);
           const unsigned m = w1 >> 16;
           mom4<double> q;
           for (int c = 0; c < 4; c++) q.c[c] = ev.qsub[m][c];
           const spin4<double> X = row_prop(row_slash(R, J), q, ev.mt, mk<double>(ev.gd[m][0], ev.gd[m][1]));
           vec4<double> o;
           for (int c = 0; c < 4; c++) o.c[c] = X.c[c];
-          GrpVec<double>::st(chain + (w0 & 0xffffu) * 8, o);
+          GrpVec<double>::st(chain + (w0 & 0xffffu) * SS, o);
         }
         __syncthreads();
       }
@@ -114,8 +121,8 @@ __global__ void __launch_bounds__(DiagGeom<D>::NT) diag_kernel(const DiagArgs p)
       const spin4<double> vv = ld_spin<double>(ev.v[htb]);
       for (int t = tid; t < D::nclos; t += NT) {
         const unsigned w0 = __ldg(D::clos() + 2 * t), ch = __ldg(D::clos() + 2 * t + 1);
-        const spin4<double> R = ld_spin<double>(chain + (w0 & 0xffffu) * 8);
-        const vec4<double> J = GrpVec<double>::ld(trees + (w0 >> 16) * 8, 0u);
+        const spin4<double> R = ld_spin<double>(chain + (w0 & 0xffffu) * SS);
+        const vec4<double> J = GrpVec<double>::ld(trees + (w0 >> 16) * SS, 0u);
         const double a2 = norm2(row_col(row_slash(R, J), vv));
         den += a2;
         num += ((int)ch == mych) ? a2 : 0.0;
