@@ -28,7 +28,14 @@ template <class D> struct DiagGeom {
   // Threads per event.  The levels of gg -> t tbar g g hold 6 .. 45 tasks (159 closures): one warp wastes a quarter of
   // its thread slots there, four warps two thirds, and wait at eight barriers per helicity (ncu, round 3: barrier stall
   // 7.5 per issued instruction with 128 threads).  Five gluons have levels of 10 .. 510 tasks and 1890 closures.
-  static constexpr int NT = (D::n >= 5) ? 128 : 32;
+#ifndef ME_DIAG_NT4
+#define ME_DIAG_NT4 32    // threads per event for four gluons (32 / 64 / 128 measured: 25.3 / 28.2 / 34.5 ms per 65536 events)
+#endif
+#ifndef ME_DIAG_NT5
+#define ME_DIAG_NT5 256   // threads per event for five gluons (145 KB of slots: one block per SM; 64 / 128 / 256 / 512 / 1024
+                          // threads measured: 56.9 / 37.5 / 33.6 / 33.7 / 43.6 ms per 4096 events)
+#endif
+  static constexpr int NT = (D::n >= 5) ? ME_DIAG_NT5 : ((D::n == 4) ? ME_DIAG_NT4 : 32);
   // A slot (4 complex doubles) takes SS = 10 doubles: with 80-byte strides the 16-byte accesses of eight neighbouring
   // slots fall into eight different bank groups (with 64-byte strides they met four to a group: 3.8e9 bank conflicts
   // on 2.3e9 ideal wavefronts in the same capture)
