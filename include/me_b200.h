@@ -14,10 +14,14 @@
  * Conventions (readings R1-R16)
  *   - all `d_*` arguments are DEVICE pointers owned by the caller (8-byte aligned; int32 outputs 4-byte);
  *     everything else is a HOST pointer.  `stream` is a cudaStream_t passed as void*; work is enqueued
- *     on it and NOT synchronised unless stated.  The library allocates device memory only in me_create (for
- *     gg_ttgg / gg_ttggg: ~1 GiB of pipeline scratch holding one chunk of events between the three kernels of the
- *     path), me_filter_helicities / me_set_good_helicities (selection scratch of the small processes) and
- *     me_compute_host (staging, grows only); me_destroy frees it.  me_compute never allocates.  Every call makes
+ *     on it and NOT synchronised unless stated.  Device memory the library allocates: a 1 KB table in me_create;
+ *     the selection scratch of the small processes in me_filter_helicities / me_set_good_helicities; staging in
+ *     me_compute_host (grows only); and, for gg_ttgg / gg_ttggg, the pipeline scratch that holds a chunk of events
+ *     between the three kernels of the path (23 KB per gg_ttgg event, 245 KB per gg_ttggg event in fp64).  That
+ *     scratch follows the batch size: me_reserve sizes it up front; otherwise me_filter_helicities / me_compute grow
+ *     it (cudaFree + cudaMalloc, which waits for the device) when a batch LARGER than any before arrives, up to 1 GiB per
+ *     handle, beyond which a batch runs in more chunks.  A call no larger than an earlier one, or than what me_reserve
+ *     was given, never allocates.  me_destroy frees everything.  Every call makes
  *     the handle's device current while it runs and restores the caller's current device before returning.
  *   - one handle serves one stream at a time: calls on the same handle from different streams must not overlap
  *     on the device (the scratch is per handle); use one handle per stream for concurrency.
@@ -93,10 +97,15 @@ int me_filter_helicities(me_handle* h, const double* d_momenta, const double* d_
 int me_get_good_helicities(const me_handle* h, int* ngood, uint8_t* mask);
 int me_set_good_helicities(me_handle* h, const uint8_t* mask);
 
+/* Sizes the pipeline scratch of a gg_ttgg / gg_ttggg handle for calls of up to max_events_per_call events (at most
+ * 1 GiB; see the conventions above), so that no later me_filter_helicities / me_compute of that size allocates.  Costs
+ * nothing for the other processes.  May be called before or after the helicity filter; never shrinks. */
+int me_reserve(me_handle* h, int64_t max_events_per_call);
+
 /* The hot path.  d_me[nevt] receives ME (fp64 in every build).  If d_rndhel and d_selhel are given,
  * d_selhel[nevt] receives the first good h with r_hel * S < sum_{h' <= h} |M_h'|^2 (last good one if
  * rounding leaves none); likewise d_rndcol/d_selcol with the weights w_c = sum_{h good} |J_c(h)|^2
- * (reading R11).  Enqueues on `stream`, does not synchronise, allocates nothing in steady state. */
+ * (reading R11).  Enqueues on `stream`, does not synchronise, allocates nothing in steady state (see me_reserve). */
 int me_compute(me_handle* h, const double* d_momenta, const double* d_gs, const double* d_rndhel,
                const double* d_rndcol, int64_t nevt, double* d_me, int32_t* d_selhel, int32_t* d_selcol,
                void* stream);

@@ -189,9 +189,41 @@ int size_cum(me_handle* h) {
   return rc;
 }
 
+// Pipeline scratch of the lane-group processes for a call of nevt events in `mode`: grows (never shrinks) up to the cap of
+// scratch_target().  A call whose preferred chunks fit what the handle already owns does not allocate.
+int reserve_scratch(me_handle* h, int64_t nevt, int mode) {
+  if (!h->have_pipe || nevt <= 0) return 0;
+  me::LaunchArgs a;
+  memset(&a, 0, sizeof(a));
+  a.nevt = nevt;
+  a.good = h->good;
+  a.good.mask[0] = a.good.mask[1] = h->good.n ? 0ull : ~0ull;   // no list yet (me_reserve before the filter): all rows
+  for (int i = 0; i < a.good.n; i++) a.good.mask[a.good.h[i] >> 6] |= 1ull << (a.good.h[i] & 63);
+  me::LaunchInfo info;
+  memset(&info, 0, sizeof(info));
+  int ce = h->proc->fn[mode == me::MODE_FILTER ? 0 : h->precision](a, mode, nullptr, &info, 1);
+  if (ce) return cuda_fail(h, (cudaError_t)ce, "pipeline scratch geometry");
+  const size_t cap = scratch_target();
+  size_t want = (size_t)info.scratch_wanted;
+  if (want > cap) want = cap;
+  if (want <= h->scratch_bytes) return 0;
+  if (want < 2 * h->scratch_bytes) want = (2 * h->scratch_bytes < cap) ? 2 * h->scratch_bytes : cap;   // few growth steps
+  return ensure(h, &h->d_scratch, &h->scratch_bytes, want);   // cudaFree waits for the work that still uses the old one
+}
+
 }  // namespace
 
 extern "C" {
+
+int me_reserve(me_handle* h, int64_t max_events_per_call) {
+  if (!h) return ME_ERR_ARG;
+  if (max_events_per_call < 0) return fail(h, ME_ERR_ARG, "me_reserve: negative event count");
+  DeviceGuard guard(h->device);
+  if (guard.err != cudaSuccess) return cuda_fail(h, guard.err, "me_reserve");
+  int rc = reserve_scratch(h, max_events_per_call < 16384 ? max_events_per_call : 16384, me::MODE_FILTER);
+  if (!rc) rc = reserve_scratch(h, max_events_per_call, me::MODE_SELECT);
+  return rc;
+}
 
 int me_create(me_handle** out, const char* process, int precision, const me_params* params, int device) {
   if (!out || !process) return fail(nullptr, ME_ERR_ARG, "me_create: null argument");
@@ -247,16 +279,7 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
       return rc;
     }
     if (i0.scratch_per_event > 0 || i1.scratch_per_event > 0) {
-      size_t want = scratch_target();
-      const size_t floor_bytes = 64 * (size_t)(i0.scratch_per_event > i1.scratch_per_event ? i0.scratch_per_event : i1.scratch_per_event);
-      if (want < floor_bytes) want = floor_bytes;
-      if ((e = cudaMalloc(&h->d_scratch, want)) != cudaSuccess) {
-        int rc = fail(nullptr, ME_ERR_NOMEM, std::string("me_create: pipeline scratch: ") + cudaGetErrorString(e));
-        cudaFree(h->d_frac);
-        delete h;
-        return rc;
-      }
-      h->scratch_bytes = want;
+      // the scratch itself is sized by the batches that arrive (reserve_scratch below) or by me_reserve
       // internal streams: two for the setup + amplitude kernels of alternating chunks, a high-priority one for the
       // colour kernels; events carry the dependencies (nothing is synchronised on the host)
       int lo = 0, hi = 0;
@@ -271,7 +294,7 @@ int me_create(me_handle** out, const char* process, int precision, const me_para
         int rc = cuda_fail(nullptr, e, "me_create: pipeline streams");
         for (cudaStream_t s : {px.sa, px.sb, px.s2}) if (s) cudaStreamDestroy(s);   // px was zeroed: non-null = created
         for (int i = 0; i < 7; i++) if (*evs[i]) cudaEventDestroy(*evs[i]);
-        cudaFree(h->d_scratch); cudaFree(h->d_frac);
+        cudaFree(h->d_frac);
         delete h;
         return rc;
       }
@@ -387,6 +410,7 @@ int me_filter_helicities(me_handle* h, const double* d_momenta, const double* d_
   cudaStream_t st = (cudaStream_t)stream;
   if ((e = cudaMemsetAsync(h->d_frac, 0, 128 * sizeof(unsigned long long), st)) != cudaSuccess)
     return cuda_fail(h, e, "me_filter_helicities: memset");
+  if ((rc = reserve_scratch(h, nevt < 16384 ? nevt : 16384, me::MODE_FILTER)) != 0) return rc;
   me::LaunchArgs a;
   memset(&a, 0, sizeof(a));
   a.mom = d_momenta; a.gs = d_gs; a.nevt = nevt < 16384 ? nevt : 16384;
@@ -448,6 +472,7 @@ static int compute_core(me_handle* h, const double* d_momenta, const double* d_g
   if (nevt == 0) return ME_OK;
   DeviceGuard guard(h->device);
   if (guard.err != cudaSuccess) return cuda_fail(h, guard.err, "me_compute");
+  if ((rc = reserve_scratch(h, nevt, me::MODE_SELECT)) != 0) return rc;   // allocates only for a batch larger than any before
   me::LaunchArgs a;
   memset(&a, 0, sizeof(a));
   a.mom = d_momenta; a.gs = d_gs; a.rndhel = d_rndhel; a.rndcol = d_rndcol; a.nevt = nevt;

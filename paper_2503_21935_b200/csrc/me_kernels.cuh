@@ -55,6 +55,7 @@ struct LaunchInfo {
   long long cum_slots;          // one-event-per-thread kernel, MODE_SELECT scratch: doubles per good helicity
   long long scratch_per_event;  // lane-group pipeline: scratch bytes per event of a chunk (0: not used)
   long long chunk;              // lane-group pipeline: events per chunk with the scratch given
+  long long scratch_wanted;     // lane-group pipeline: scratch bytes with which a call of a.nevt events runs in its preferred chunks
   int launches;                 // kernels enqueued by the call
 };
 

@@ -82,6 +82,7 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     info->cum_slots = blocks * ME_NT;
     info->scratch_per_event = 0;
     info->chunk = 0;
+    info->scratch_wanted = 0;
     info->launches = (a.nevt > 0) ? 1 : 0;
   }
   if (dry || a.nevt == 0) return 0;

@@ -76,7 +76,7 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
   const size_t half = (a.scratch_bytes / NPART) & ~(size_t)255;
   long long cap = (half > slack) ? (long long)((half - slack) / per_event) : 0;   // events per half
   if (cap > (1 << 20)) cap = 1 << 20;
-  const long long min_chunk = (8 * 1184 + nunit - 1) / nunit;   // >= 8 waves of amplitude warps on 148 SMs
+  const long long min_chunk = (8 * 1184 + nunit - 1) / (nunit > 0 ? nunit : 1);   // >= 8 waves of amplitude warps on 148 SMs
   long long chunk = cap;
   if (chunk > 0 && a.nevt > 0) {
     long long want = (a.nevt + 2 * NPART - 1) / (2 * NPART);      // aim at two rounds of the parts per call
@@ -99,6 +99,14 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     info->cum_slots = 0;
     info->scratch_per_event = (long long)(sizeof(EV) + (size_t)GE::NGRP * grpb);
     info->chunk = chunk;
+    {  // what this batch would like to have: NPART parts of its preferred chunk (all combinations), whatever a.scratch_bytes is
+      long long want = (a.nevt + 2 * NPART - 1) / (2 * NPART);
+      if (want < min_chunk) want = min_chunk;
+      if (want > a.nevt) want = a.nevt;
+      if (want > (1 << 20)) want = 1 << 20;
+      if (want < 1) want = 1;
+      info->scratch_wanted = (long long)NPART * (long long)(align_up((size_t)want * (size_t)info->scratch_per_event + slack, 256) + 256);
+    }
     info->launches = (int)(3 * nchunks) + (CG::CF_GLOBAL ? 1 : 0);
   }
   if (dry || a.nevt == 0) return 0;

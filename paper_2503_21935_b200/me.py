@@ -19,7 +19,7 @@ PROCESSES = ("ee_mumu", "gg_tt", "gg_ttg", "gg_ttgg", "gg_ttggg", "gux_taptamux"
 
 EXPORTS = ("me_create", "me_destroy", "me_last_error", "me_info", "me_helicity_table", "me_color_table",
            "me_color_matrix", "me_filter_helicities", "me_get_good_helicities", "me_set_good_helicities",
-           "me_compute", "me_compute_noalloc", "me_compute_multichannel", "me_channel_table", "me_compute_host", "me_generate", "me_launch_info", "me_launch_stats", "me_fma_peak", "me_mma_peak")
+           "me_compute", "me_reserve", "me_compute_noalloc", "me_compute_multichannel", "me_channel_table", "me_compute_host", "me_generate", "me_launch_info", "me_launch_stats", "me_fma_peak", "me_mma_peak")
 
 
 class MEError(RuntimeError):
@@ -53,6 +53,7 @@ def load_library(path: str = LIB_PATH):
     L.me_filter_helicities.argtypes = [vp, vp, vp, i64, vp]
     L.me_get_good_helicities.argtypes = [vp, ip, vp]
     L.me_set_good_helicities.argtypes = [vp, vp]
+    L.me_reserve.argtypes = [vp, i64]
     L.me_compute.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, vp, vp]
     L.me_compute_noalloc.argtypes = [ctypes.POINTER(me_params), vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, ctypes.c_char_p, ctypes.c_int]
     L.me_compute_multichannel.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, vp]
@@ -167,6 +168,10 @@ class MatrixElement:
         if m.shape != (self.ncomb,):
             raise MEError("mask must have ncomb entries")
         self._check(self._L.me_set_good_helicities(self._h, _hptr(m)))
+
+    def reserve(self, max_events_per_call: int):
+        """me_reserve: size the pipeline scratch (gg_ttgg / gg_ttggg) for calls of up to that many events."""
+        self._check(self._L.me_reserve(self._h, int(max_events_per_call)))
 
     # ---- hot path
     def compute(self, momenta, gs=None, rndhel=None, rndcol=None, out=None, selhel=None, selcol=None, stream=None):

@@ -271,3 +271,30 @@ def test_lane_group_pipeline_is_deterministic_and_chunk_independent(torch_cuda, 
     for i in range(3):
         assert torch_cuda.equal(torch_cuda.cat([a[i], b[i]]), runs[0][i])
     m.close()
+
+
+def test_pipeline_scratch_follows_the_batch_size(torch_cuda):
+    """gg_ttgg: a fresh handle owns no pipeline scratch; small batches take little; me_reserve sizes it up front; a call no
+    larger than an earlier one does not change it; results do not depend on the scratch size."""
+    from paper_2503_21935_b200.me import MatrixElement
+    torch = torch_cuda
+    case = oracle_case("gg_ttgg")
+    mom, gs = torch.from_numpy(case["mom"]).cuda(), torch.from_numpy(case["gs"]).cuda()
+    m = MatrixElement("gg_ttgg", "fp64")
+    assert m.launch_info()["scratch_bytes"] == 0
+    m.filter_helicities(mom[:64].contiguous(), gs[:64].contiguous())
+    small, _, _ = m.compute(mom[:300].contiguous(), gs[:300].contiguous())
+    torch.cuda.synchronize()
+    s0 = m.launch_info()["scratch_bytes"]
+    assert 0 < s0 < (64 << 20)
+    m.compute(mom[:200].contiguous(), gs[:200].contiguous())
+    assert m.launch_info()["scratch_bytes"] == s0
+    m.reserve(1 << 20)
+    s1 = m.launch_info()["scratch_bytes"]
+    assert s1 == (1 << 30)
+    big, _, _ = m.compute(mom, gs)
+    torch.cuda.synchronize()
+    assert m.launch_info()["scratch_bytes"] == s1
+    assert torch.equal(big[:300], small)
+    assert np.abs(big.cpu().numpy() / case["sel"]["me"] - 1).max() <= 1e-10
+    m.close()
