@@ -34,6 +34,10 @@ TUNE = {
     ("gg_ttgg", 0): (32, 8), ("gg_ttgg", 1): (32, 18), ("gg_ttgg", 2): (32, 8),
 }
 DEFAULT_TUNE = (128, 1)
+# lane-group units whose colour kernel runs on the amplitude kernel's own stream rather than on the high-priority one
+# (round 3, 262144 / 2^20 events: gg_ttggg fp64 242.2 -> 239.9 ms, gg_ttgg fp32 22.85 -> 22.61 ms; gg_ttgg fp64 loses
+# 9 % (47.3 -> 52.0 ms) and gg_ttggg fp32 gains 0.3 %, so they keep the high-priority stream; mixed not measured)
+K2_SAME_STREAM = {("gg_ttggg", 0), ("gg_ttgg", 1)}
 # extra nvcc flags for experiments, e.g. ME_B200_NVCC_FLAGS="-DME_UNROLL_T=2" (part of the units' hashes)
 # for the units whose name starts with one of ME_B200_NVCC_UNITS (comma separated; default: all)
 EXTRA = os.environ.get("ME_B200_NVCC_FLAGS", "").split()
@@ -55,6 +59,8 @@ def _units():
                 # complex Minkowski products as product + subtraction: with the all-FMA form this unit spills 130 bytes
                 # more per thread and runs 13 % slower (measured); every other unit gains from the FMA form
                 defs.append("-DME_MDOT_FMA=0")
+            if (p, prec) in K2_SAME_STREAM:
+                defs.append("-DME_K2_SAME_STREAM")
             src = "me_proc_group.cu" if p in GROUP_LAYOUT else "me_proc.cu"
             yield f"{p}_p{prec}", os.path.join(CSRC, src), defs
     for p in DIAG_PROCS:

@@ -1282,9 +1282,15 @@ template <class G, typename TC> struct ColGeom {
   // become resident beside the amplitude warps of the following chunk and run under them (high-priority stream).
   // 120 flows: C' is 30-61 KB in shared memory, shared by the 8 warps of a block.  (A copy in global memory read by
   // one-warp blocks was measured: 4.6 TB/s of L2 traffic in fp32, the amplitude kernel beside it 20 % slower.)
-  static constexpr int WARPS = (G::ncol <= 24) ? 1 : 8;
+#ifndef ME_K2_WARPS
+#define ME_K2_WARPS 8   // warps per block for 120 flows.  Round 3, gg_ttggg 262144 events, (warps per block, colour warps per
+#endif                  // SM) = (8, 8) / (4, 4) / (4, 8) / (16, 16): fp64 242.2 / 243.2 / 241.7 / 246.4 ms, fp32 113.4 / 113.4 /
+#ifndef ME_K2_WPS       // 112.4 / 123.3 ms: within 1 % except the last, (8, 8) kept
+#define ME_K2_WPS 8
+#endif
+  static constexpr int WARPS = (G::ncol <= 24) ? 1 : ME_K2_WARPS;
   static constexpr bool CF_GLOBAL = false;
-  static constexpr int WPS = (G::ncol <= 24) ? 32 : 8;   // colour warps per SM (grid sizing; 4, 8, 16, 32 measured)
+  static constexpr int WPS = (G::ncol <= 24) ? 32 : ME_K2_WPS;   // colour warps per SM (grid sizing; 4, 8, 16, 32 measured)
   static constexpr int GPT = ColFrag<G::ncol, TC>::GPT, NCOL = G::ncol;
   static constexpr int CF = XGeom<G>::NPAIR * 64;                        // TC elements of C' in fragment order
   static constexpr int PERW = (int)sizeof(double) * ((1 << (G::n + 2)) + NCOL);   // per warp: |M_h|^2, colour weights

@@ -164,6 +164,11 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
     p.xt = base + align_up((size_t)n * evb, 256);
     constexpr int PT = ((1 << N) + N + 6 <= 32) ? 32 : 64;
     cudaStream_t s1 = px ? (hf ? px->sb : px->sa) : st, s2 = px ? px->s2 : st;
+#ifdef ME_K2_SAME_STREAM
+    // units for which it measured faster (build.py): the colour kernel follows the amplitude kernel of its chunk on the same
+    // low-priority stream instead of cutting in on the high-priority one (no SM is drained for it ahead of time)
+    s2 = s1;
+#endif
     if (px && c >= NPART && (err = cudaStreamWaitEvent(s1, px->k2[part], 0)) != cudaSuccess) return (int)err;  // part free again
 #if defined(ME_CHECK) && ME_CHECK
     // self-check build: the part of the scratch this chunk uses starts as NaN
@@ -188,6 +193,10 @@ static int launch_mode(const me::LaunchArgs& a, cudaStream_t st, me::LaunchInfo*
   if (px) {  // join: the caller's stream continues after the last colour kernel (s2 is in order, and follows sa / sb)
     err = cudaStreamWaitEvent(st, px->k2[(int)((c - 1) % NPART)], 0);
     if (err != cudaSuccess) return (int)err;
+#ifdef ME_K2_SAME_STREAM
+    // the colour kernels of the last two chunks ran on different streams: wait for both
+    if (c >= 2 && (err = cudaStreamWaitEvent(st, px->k2[(int)((c - 2) % NPART)], 0)) != cudaSuccess) return (int)err;
+#endif
   }
   return 0;
 }
