@@ -19,8 +19,8 @@
  *     me_compute_host (grows only); and, for gg_ttgg / gg_ttggg, the pipeline scratch that holds a chunk of events
  *     between the three kernels of the path (23 KB per gg_ttgg event, 245 KB per gg_ttggg event in fp64).  That
  *     scratch follows the batch size: me_reserve sizes it up front; otherwise me_filter_helicities / me_compute grow
- *     it (cudaFree + cudaMalloc, which waits for the device) when a batch LARGER than any before arrives, up to 1 GiB per
- *     handle, beyond which a batch runs in more chunks.  A call no larger than an earlier one, or than what me_reserve
+ *     it (cudaFree + cudaMalloc, which waits for the device) when a batch LARGER than any before arrives, up to 2 GiB (gg_ttgg) or
+ *     8 GiB (gg_ttggg) per handle, beyond which a batch runs in more chunks.  A call no larger than an earlier one, or than what me_reserve
  *     was given, never allocates.  me_destroy frees everything.  Every call makes
  *     the handle's device current while it runs and restores the caller's current device before returning.
  *   - one handle serves one stream at a time: calls on the same handle from different streams must not overlap
@@ -98,7 +98,7 @@ int me_get_good_helicities(const me_handle* h, int* ngood, uint8_t* mask);
 int me_set_good_helicities(me_handle* h, const uint8_t* mask);
 
 /* Sizes the pipeline scratch of a gg_ttgg / gg_ttggg handle for calls of up to max_events_per_call events (at most
- * 1 GiB; see the conventions above), so that no later me_filter_helicities / me_compute of that size allocates.  Costs
+ * 2 GiB / 8 GiB; see the conventions above), so that no later me_filter_helicities / me_compute of that size allocates.  Costs
  * nothing for the other processes.  May be called before or after the helicity filter; never shrinks. */
 int me_reserve(me_handle* h, int64_t max_events_per_call);
 

@@ -163,11 +163,14 @@ struct DeviceGuard {
   }
 };
 
-// bytes of pipeline scratch: ME_B200_SCRATCH_MB (for experiments) or 1 GiB
-size_t scratch_target() {
+// Cap of the pipeline scratch of a handle: 2 GiB for gg_ttgg, 8 GiB for gg_ttggg (only batches that want it get there,
+// see reserve_scratch), or ME_B200_SCRATCH_MB.  Measured on B200 (round 3, caps 1 / 2 / 4 / 8 GiB): gg_ttggg fp64, 262144
+// events per call: 239.4 / 237.7 / 236.8 / 236.3 ms (larger chunks, fewer chunk tails); gg_ttgg fp64, 2^20 events: 47.34 /
+// 46.91 / 47.48 / 47.54 ms (beyond 2 GiB the chunks' jamps stop fitting the L2 as well).
+size_t scratch_target(int ngluon) {
   const char* s = getenv("ME_B200_SCRATCH_MB");
   long mb = s ? atol(s) : 0;
-  if (mb < 16) mb = 1024;
+  if (mb < 16) mb = (ngluon >= 5) ? 8192 : 2048;
   return (size_t)mb << 20;
 }
 
@@ -190,7 +193,7 @@ int size_cum(me_handle* h) {
 }
 
 // Pipeline scratch of the lane-group processes for a call of nevt events in `mode`: grows (never shrinks) up to the cap of
-// scratch_target().  A call whose preferred chunks fit what the handle already owns does not allocate.
+// scratch_target(ngluon).  A call whose preferred chunks fit what the handle already owns does not allocate.
 int reserve_scratch(me_handle* h, int64_t nevt, int mode) {
   if (!h->have_pipe || nevt <= 0) return 0;
   me::LaunchArgs a;
@@ -203,7 +206,7 @@ int reserve_scratch(me_handle* h, int64_t nevt, int mode) {
   memset(&info, 0, sizeof(info));
   int ce = h->proc->fn[mode == me::MODE_FILTER ? 0 : h->precision](a, mode, nullptr, &info, 1);
   if (ce) return cuda_fail(h, (cudaError_t)ce, "pipeline scratch geometry");
-  const size_t cap = scratch_target();
+  const size_t cap = scratch_target(h->proc->ngl);
   size_t want = (size_t)info.scratch_wanted;
   if (want > cap) want = cap;
   if (want <= h->scratch_bytes) return 0;

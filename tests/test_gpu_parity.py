@@ -291,7 +291,7 @@ def test_pipeline_scratch_follows_the_batch_size(torch_cuda):
     assert m.launch_info()["scratch_bytes"] == s0
     m.reserve(1 << 20)
     s1 = m.launch_info()["scratch_bytes"]
-    assert s1 == (1 << 30)
+    assert s1 == (2 << 30)   # the cap of a gg_ttgg handle
     big, _, _ = m.compute(mom, gs)
     torch.cuda.synchronize()
     assert m.launch_info()["scratch_bytes"] == s1
